@@ -1,0 +1,196 @@
+"""CPU oracle for the KPM/LSQT DOS path -- TEST INFRASTRUCTURE ONLY.
+
+ctypes wrapper around oracle/libgtbo.so (built from oracle/*.cpp by
+oracle/build.py).  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package; the product
+(paper_2509_06525_b200) never does and shares no code with it.
+See oracle/gtbo.h for the cited definition of every function.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+OK, ERR_INVALID_ARG, ERR_BOX_TOO_SMALL, ERR_ELL_OVERFLOW = 0, -1, -2, -3
+
+
+class OracleError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        super().__init__(f"oracle {where} failed with status {status}")
+        self.status = status
+
+
+class _Model(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite", C.c_void_p), ("t0", C.c_void_p),
+                ("r0", C.c_double), ("beta", C.c_double), ("onsite_shift", C.c_void_p)]
+
+
+class _Ell(C.Structure):
+    _fields_ = [("n", C.c_int64), ("width", C.c_int32), ("cols", C.c_void_p),
+                ("vals", C.c_void_p), ("diag", C.c_void_p)]
+
+
+@dataclass
+class Ell:
+    """Host ELL matrix in the canonical export layout (slot-major [width][n])."""
+    n: int
+    width: int
+    cols: np.ndarray            # int32 [width, n]
+    vals: np.ndarray            # float64 [width, n]
+    diag: Optional[np.ndarray]  # float64 [n] or None
+
+    def _c(self) -> _Ell:
+        return _Ell(self.n, self.width, self.cols.ctypes.data, self.vals.ctypes.data,
+                    self.diag.ctypes.data if self.diag is not None else None)
+
+    def to_dense(self) -> np.ndarray:
+        h = np.zeros((self.n, self.n))
+        rows = np.arange(self.n)
+        for k in range(self.width):
+            np.add.at(h, (rows, self.cols[k]), self.vals[k])
+        if self.diag is not None:
+            h[rows, rows] += self.diag
+        return h
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.gtbo_mix64.restype = C.c_uint64
+        _lib.gtbo_mix64.argtypes = [C.c_uint64]
+        _lib.gtbo_hash.restype = C.c_uint64
+        _lib.gtbo_hash.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64]
+        _lib.gtbo_uniform.restype = C.c_double
+        _lib.gtbo_uniform.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64]
+    return _lib
+
+
+def _f64(x) -> np.ndarray:
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _i32(x) -> np.ndarray:
+    return np.ascontiguousarray(x, dtype=np.int32)
+
+
+def _check(st: int, where: str) -> None:
+    if st != OK:
+        raise OracleError(st, where)
+
+
+def mix64(z: int) -> int:
+    return lib().gtbo_mix64(C.c_uint64(z & (2**64 - 1)))
+
+
+def hash64(seed: int, r: int, i: int) -> int:
+    return lib().gtbo_hash(C.c_uint64(seed & (2**64 - 1)), C.c_uint32(r), C.c_uint64(i))
+
+
+def uniform(seed: int, r: int, i: int) -> float:
+    return lib().gtbo_uniform(C.c_uint64(seed & (2**64 - 1)), C.c_uint32(r), C.c_uint64(i))
+
+
+def neighbor_counts(pos, box, pbc, cutoff: float, method: int = 1):
+    pos = _f64(pos)
+    n = pos.shape[0]
+    box, pbc = _f64(box), _i32(pbc)
+    counts = np.zeros(n, dtype=np.int32)
+    width = C.c_int32(0)
+    st = lib().gtbo_neighbor_counts(C.c_void_p(pos.ctypes.data), C.c_int64(n),
+                                    C.c_void_p(box.ctypes.data), C.c_void_p(pbc.ctypes.data),
+                                    C.c_double(cutoff), C.c_int32(method),
+                                    C.c_void_p(counts.ctypes.data), C.byref(width))
+    _check(st, "neighbor_counts")
+    return counts, int(width.value)
+
+
+def build_hamiltonian(pos, species, box, pbc, cutoff: float, onsite, t0, r0: float = 1.0,
+                      beta: float = 0.0, onsite_shift=None, width: Optional[int] = None,
+                      method: int = 1, with_diag: bool = True) -> Ell:
+    pos, species = _f64(pos), _i32(species)
+    n = pos.shape[0]
+    box, pbc = _f64(box), _i32(pbc)
+    onsite, t0 = _f64(onsite), _f64(t0)
+    shift = _f64(onsite_shift) if onsite_shift is not None else None
+    if width is None:
+        _, width = neighbor_counts(pos, box, pbc, cutoff, method)
+    H = Ell(n, width, np.zeros((width, n), dtype=np.int32), np.zeros((width, n)),
+            np.zeros(n) if with_diag else None)
+    model = _Model(onsite.shape[0], onsite.ctypes.data, t0.ctypes.data, r0, beta,
+                   shift.ctypes.data if shift is not None else None)
+    hc = H._c()
+    st = lib().gtbo_build_hamiltonian(C.c_void_p(pos.ctypes.data), C.c_void_p(species.ctypes.data),
+                                      C.c_int64(n), C.c_void_p(box.ctypes.data),
+                                      C.c_void_p(pbc.ctypes.data), C.c_double(cutoff),
+                                      C.byref(model), C.c_int32(method), C.byref(hc))
+    _check(st, "build_hamiltonian")
+    return H
+
+
+def spectral_bounds(H: Ell):
+    out = np.zeros(2)
+    hc = H._c()
+    _check(lib().gtbo_spectral_bounds(C.byref(hc), C.c_void_p(out.ctypes.data)), "spectral_bounds")
+    return float(out[0]), float(out[1])
+
+
+def random_phase_fill(seed: int, r0: int, R: int, n: int) -> np.ndarray:
+    phi = np.zeros((n, R, 2))
+    st = lib().gtbo_random_phase_fill(C.c_uint64(seed & (2**64 - 1)), C.c_int32(r0), C.c_int32(R),
+                                      C.c_int64(n), C.c_void_p(phi.ctypes.data))
+    _check(st, "random_phase_fill")
+    return phi
+
+
+def kpm_moments(H: Ell, a: float, b: float, M: int, R: int = 1, seed: int = 0, mode: int = 0,
+                algo: int = 0, return_im: bool = False):
+    mu = np.zeros(M)
+    im = C.c_double(0.0)
+    hc = H._c()
+    st = lib().gtbo_kpm_moments(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(M),
+                                C.c_int32(R), C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode),
+                                C.c_int32(algo), C.c_void_p(mu.ctypes.data), C.byref(im))
+    _check(st, "kpm_moments")
+    return (mu, float(im.value)) if return_im else mu
+
+
+def kpm_step_rows(H: Ell, a: float, b: float, first: bool, phi_prev, phi_cur, rows) -> np.ndarray:
+    phi_cur = _f64(phi_cur)
+    R = phi_cur.shape[1]
+    phi_prev = _f64(phi_prev) if phi_prev is not None else None
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    out = np.zeros((rows.shape[0], R, 2))
+    hc = H._c()
+    st = lib().gtbo_kpm_step_rows(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(int(first)),
+                                  C.c_int32(R),
+                                  C.c_void_p(phi_prev.ctypes.data if phi_prev is not None else None),
+                                  C.c_void_p(phi_cur.ctypes.data), C.c_void_p(rows.ctypes.data),
+                                  C.c_int64(rows.shape[0]), C.c_void_p(out.ctypes.data))
+    _check(st, "kpm_step_rows")
+    return out
+
+
+def jackson(M: int) -> np.ndarray:
+    g = np.zeros(M)
+    _check(lib().gtbo_jackson(C.c_int32(M), C.c_void_p(g.ctypes.data)), "jackson")
+    return g
+
+
+def dos(mu, a: float, b: float, energies, kernel: int = 1, scale: float = 1.0) -> np.ndarray:
+    mu, energies = _f64(mu), _f64(energies)
+    rho = np.zeros(energies.shape[0])
+    st = lib().gtbo_dos(C.c_void_p(mu.ctypes.data), C.c_int32(mu.shape[0]), C.c_double(a),
+                        C.c_double(b), C.c_int32(kernel), C.c_void_p(energies.ctypes.data),
+                        C.c_int32(energies.shape[0]), C.c_double(scale),
+                        C.c_void_p(rho.ctypes.data))
+    _check(st, "dos")
+    return rho

@@ -1,0 +1,123 @@
+/*
+ * gtbo.h -- CPU ORACLE for the KPM / LSQT density-of-states path of GPUTB
+ * (arxiv/paper_2509_06525).  TEST INFRASTRUCTURE ONLY.
+ *
+ * This is a plain, slow, obviously-correct restatement of what the hot path
+ * computes, written from the paper and from BASELINE.json:north_star
+ * (the paper names the ingredients of the method at PAPER.md:55 (sec. 2.4) but
+ * prints no recursion; the textbook KPM identities used are written out in
+ * SURVEY.md sec. 8(c) C1-C7 and restated beside each function below).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load this library.  The product (the CUDA path
+ * under paper_2509_06525_b200/) never does, and shares no code, header,
+ * table or helper with it: this header is private to oracle/.
+ *
+ * All pointers are HOST pointers.  All arrays are caller-owned.
+ * Layouts (the interface contract of the boundary):
+ *   pos      double [n][3]            Cartesian coordinates, Angstrom, unwrapped
+ *   species  int32  [n]
+ *   ELL      cols int32 [width][n], vals double [width][n]  (slot-major);
+ *            row i's entries sorted by ascending column; padding slots have
+ *            col = i and val = +0.0;  diag double [n] or NULL (= all zero)
+ *   phi      double [n][R][2]         complex128, vectors interleaved per atom
+ *   mu       double [M]
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"): every function below is
+ * pinned by something other than itself -- closed-form honeycomb eigenvalues,
+ * closed-walk counts, numpy eigvalsh on tiny lattices, brute force O(N^2)
+ * neighbour lists, the published splitmix64 first output, Jackson-kernel
+ * positivity / normalisation.  No function here is "parity unpinned".
+ */
+#ifndef GTBO_H
+#define GTBO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  GTBO_OK = 0,
+  GTBO_ERR_INVALID_ARG = -1,
+  GTBO_ERR_BOX_TOO_SMALL = -2, /* a periodic length < 2*cutoff            */
+  GTBO_ERR_ELL_OVERFLOW = -3   /* a row needs more slots than `width`     */
+};
+
+/* Hopping model of Eq. 1 reduced to one orbital per atom:
+ *   t_ij = t0[s_i][s_j]                       if beta == 0
+ *   t_ij = t0[s_i][s_j]*exp(-beta*(r/r0 - 1)) otherwise
+ *   eps_i = onsite[s_i] (+ onsite_shift[i] if onsite_shift != NULL)        */
+typedef struct gtbo_model {
+  int32_t n_species;
+  const double* onsite;       /* [n_species]              eV */
+  const double* t0;           /* [n_species][n_species]   eV */
+  double r0;
+  double beta;
+  const double* onsite_shift; /* [n] or NULL              eV */
+} gtbo_model;
+
+typedef struct gtbo_ell {
+  int64_t n;
+  int32_t width;
+  int32_t* cols; /* [width][n] */
+  double* vals;  /* [width][n] */
+  double* diag;  /* [n] or NULL */
+} gtbo_ell;
+
+/* --- C2: neighbour sets N(i) = { j != i : r_ij^2 < cutoff^2 } (Eq. 1) ----- */
+/* counts[i] = |N(i)|; returns max_i counts[i] in *width_out.
+ * method 0 = brute force O(n^2); 1 = cell buckets.                          */
+int gtbo_neighbor_counts(const double* pos, int64_t n, const double box[3],
+                         const int32_t pbc[3], double cutoff, int32_t method,
+                         int32_t* counts /* [n] or NULL */, int32_t* width_out);
+
+/* Fill H (caller-allocated, H->width given).  method as above.             */
+int gtbo_build_hamiltonian(const double* pos, const int32_t* species, int64_t n,
+                           const double box[3], const int32_t pbc[3],
+                           double cutoff, const gtbo_model* model,
+                           int32_t method, gtbo_ell* H);
+
+/* --- C7: Gershgorin bounds; lo_hi[0] = E_lo, lo_hi[1] = E_hi --------------- */
+int gtbo_spectral_bounds(const gtbo_ell* H, double lo_hi[2]);
+
+/* --- C3: counter-based random phases ------------------------------------- */
+uint64_t gtbo_mix64(uint64_t z);                         /* splitmix64 output */
+uint64_t gtbo_hash(uint64_t seed, uint32_t r, uint64_t i); /* h(seed, r, i)   */
+double gtbo_uniform(uint64_t seed, uint32_t r, uint64_t i); /* (h>>11)*2^-53  */
+/* phi[i][k] = exp(i*theta), theta = fl(2*pi*u(seed, r0+k, i)), k = 0..R-1    */
+int gtbo_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n,
+                           double* phi);
+
+/* --- C4/C5: Chebyshev moments --------------------------------------------- */
+/* mode 0: R random-phase vectors r = 0..R-1 (seed).
+ * mode 1: exact trace over all n basis vectors (R, seed ignored).
+ * algo 0: direct definition m_n = Re<phi_0|phi_n>, M SpMVs        (C4)
+ * algo 1: doubling identities, ceil(M/2) SpMVs                     (C5)
+ * mu[n] = sum_r m_n^(r) / (n_atoms * R)  (mode 1: / n_atoms).
+ * im_max (optional): max_n |Im sum_r <phi_0|phi_n>| / (n_atoms*R), algo 0.  */
+int gtbo_kpm_moments(const gtbo_ell* H, double a, double b, int32_t M,
+                     int32_t R, uint64_t seed, int32_t mode, int32_t algo,
+                     double* mu, double* im_max);
+
+/* One recursion step on selected rows only (sampled full-size parity):
+ *   first != 0 : out[i] = (H phi_cur - b phi_cur)[i] / a
+ *   first == 0 : out[i] = (H phi_cur - b phi_cur)[i] * (2/a) - phi_prev[i]
+ * phi_* are [n][R][2]; out is [n_rows][R][2].                               */
+int gtbo_kpm_step_rows(const gtbo_ell* H, double a, double b, int32_t first,
+                       int32_t R, const double* phi_prev, const double* phi_cur,
+                       const int64_t* rows, int64_t n_rows, double* out);
+
+/* --- C6: Jackson-damped DOS (Eq. 4) -------------------------- */
+/* kernel 0 = none (g_n = 1), 1 = Jackson.  rho = 0 where |(E-b)/a| >= 1.    */
+int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
+             const double* energies, int32_t G, double scale, double* rho);
+/* g[n], n = 0..M-1 (exported so the kernel itself can be pinned).           */
+int gtbo_jackson(int32_t M, double* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GTBO_H */

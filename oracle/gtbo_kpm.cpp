@@ -1,0 +1,279 @@
+// CPU ORACLE (test infrastructure only; see gtbo.h) -- random-phase vectors,
+// Chebyshev moments and the Jackson-damped density of states.
+//
+// What the paper fixes: the ingredient list of the LSQT stage (PAPER.md:55,
+// sec. 2.4: "orthogonal polynomials (Chebyshev expansion), the kernel
+// polynomial method (KPM), sparse matrix-vector multiplication, and the random
+// phase approximation") and the DOS definition (Eq. 4, printed
+// garbled as "2/0": read rho(E) = (2/Omega) Tr[delta(E - H)]).  The recursion
+// itself is BASELINE.json:north_star's
+//     |phi_{n+1}> = 2 H~ |phi_n> - |phi_{n-1}>,   H~ = (H - b)/a,
+// with moments mu_n = (1/(N R)) sum_r Re <phi_0^r | phi_n^r>.  Steps are written
+// in that order and notation; nothing is blocked,
+// fused or reordered beyond an OpenMP loop over independent rows.
+#include "gtbo.h"
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct cplx {
+  double re, im;
+};
+
+constexpr uint64_t kGamma = 0x9E3779B97F4A7C15ull;  // 2^64 / golden ratio
+
+// y = H x   (row sum in ascending slot order, then the diagonal term)
+void spmv(const gtbo_ell* H, const cplx* x, cplx* y) {
+  const int64_t n = H->n;
+#pragma omp parallel for schedule(static) if (n > 16384)
+  for (int64_t i = 0; i < n; ++i) {
+    double re = 0.0, im = 0.0;
+    for (int32_t k = 0; k < H->width; ++k) {
+      const double v = H->vals[(size_t)k * n + i];
+      const int32_t j = H->cols[(size_t)k * n + i];
+      re = re + v * x[j].re;
+      im = im + v * x[j].im;
+    }
+    if (H->diag) {
+      re = re + H->diag[i] * x[i].re;
+      im = im + H->diag[i] * x[i].im;
+    }
+    y[i].re = re;
+    y[i].im = im;
+  }
+}
+
+// <x|y> = sum_i conj(x_i) y_i
+cplx dotc(const cplx* x, const cplx* y, int64_t n) {
+  double re = 0.0, im = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : re, im) if (n > 16384)
+  for (int64_t i = 0; i < n; ++i) {
+    re += x[i].re * y[i].re + x[i].im * y[i].im;
+    im += x[i].re * y[i].im - x[i].im * y[i].re;
+  }
+  return {re, im};
+}
+
+// phi_1 = H~ phi_0 = (H phi_0 - b phi_0) / a
+void first_step(const gtbo_ell* H, double a, double b, const cplx* p0, cplx* p1) {
+  spmv(H, p0, p1);
+  const int64_t n = H->n;
+  const double s = 1.0 / a;
+#pragma omp parallel for schedule(static) if (n > 16384)
+  for (int64_t i = 0; i < n; ++i) {
+    p1[i].re = (p1[i].re - b * p0[i].re) * s;
+    p1[i].im = (p1[i].im - b * p0[i].im) * s;
+  }
+}
+
+// phi_{n+1} = 2 H~ phi_n - phi_{n-1} = (H phi_n - b phi_n) (2/a) - phi_{n-1}
+void next_step(const gtbo_ell* H, double a, double b, const cplx* pm, const cplx* pn,
+               cplx* pp) {
+  spmv(H, pn, pp);
+  const int64_t n = H->n;
+  const double s = 2.0 / a;
+#pragma omp parallel for schedule(static) if (n > 16384)
+  for (int64_t i = 0; i < n; ++i) {
+    pp[i].re = (pp[i].re - b * pn[i].re) * s - pm[i].re;
+    pp[i].im = (pp[i].im - b * pn[i].im) * s - pm[i].im;
+  }
+}
+
+// Per-vector moments m_n, n = 0..M-1, for one start vector phi_0.
+// algo 0 (C4): m_n = <phi_0|phi_n> by M-1 SpMVs.
+// algo 1 (C5): m_{2n} = 2<phi_n|phi_n> - m_0, m_{2n+1} = 2 Re<phi_{n+1}|phi_n> - m_1.
+void vector_moments(const gtbo_ell* H, double a, double b, int32_t M, int32_t algo,
+                    const std::vector<cplx>& phi0, std::vector<double>& m_re,
+                    std::vector<double>& m_im) {
+  const int64_t n = H->n;
+  m_re.assign(M, 0.0);
+  m_im.assign(M, 0.0);
+  std::vector<cplx> pm(phi0), pn(n), pp(n);
+  if (algo == 0) {
+    cplx d = dotc(phi0.data(), phi0.data(), n);
+    m_re[0] = d.re;
+    m_im[0] = d.im;
+    if (M == 1) return;
+    first_step(H, a, b, pm.data(), pn.data());
+    d = dotc(phi0.data(), pn.data(), n);
+    m_re[1] = d.re;
+    m_im[1] = d.im;
+    for (int32_t k = 2; k < M; ++k) {
+      next_step(H, a, b, pm.data(), pn.data(), pp.data());
+      d = dotc(phi0.data(), pp.data(), n);
+      m_re[k] = d.re;
+      m_im[k] = d.im;
+      pm.swap(pn);
+      pn.swap(pp);
+    }
+  } else {
+    // pm = phi_k, pn = phi_{k+1}
+    first_step(H, a, b, pm.data(), pn.data());
+    const double m0 = dotc(pm.data(), pm.data(), n).re;
+    const double m1 = dotc(pn.data(), pm.data(), n).re;
+    m_re[0] = m0;
+    if (M > 1) m_re[1] = m1;
+    for (int32_t k = 1; 2 * k < M; ++k) {
+      // advance so that pm = phi_k, pn = phi_{k+1}
+      next_step(H, a, b, pm.data(), pn.data(), pp.data());
+      pm.swap(pn);
+      pn.swap(pp);
+      // now pm = phi_k (old pn), pn = phi_{k+1}
+      m_re[2 * k] = 2.0 * dotc(pm.data(), pm.data(), n).re - m0;
+      if (2 * k + 1 < M) m_re[2 * k + 1] = 2.0 * dotc(pn.data(), pm.data(), n).re - m1;
+    }
+  }
+}
+
+}  // namespace
+
+// C3. splitmix64 output function; the i-th output of a splitmix64 stream with
+// initial state s is mix(s + (i+1)*gamma), so the stream is counter-addressable.
+extern "C" uint64_t gtbo_mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// key(seed, r) = mix(seed + (r+1) gamma);  h = mix(key + (i+1) gamma)
+extern "C" uint64_t gtbo_hash(uint64_t seed, uint32_t r, uint64_t i) {
+  const uint64_t key = gtbo_mix64(seed + ((uint64_t)r + 1ull) * kGamma);
+  return gtbo_mix64(key + (i + 1ull) * kGamma);
+}
+
+extern "C" double gtbo_uniform(uint64_t seed, uint32_t r, uint64_t i) {
+  return (double)(gtbo_hash(seed, r, i) >> 11) * 0x1.0p-53;
+}
+
+extern "C" int gtbo_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n,
+                                      double* phi) {
+  if (!phi || R <= 0 || n < 0 || r0 < 0) return GTBO_ERR_INVALID_ARG;
+  for (int64_t i = 0; i < n; ++i)
+    for (int32_t k = 0; k < R; ++k) {
+      const double u = gtbo_uniform(seed, (uint32_t)(r0 + k), (uint64_t)i);
+      const double theta = 6.283185307179586 * u;
+      phi[((size_t)i * R + k) * 2 + 0] = std::cos(theta);
+      phi[((size_t)i * R + k) * 2 + 1] = std::sin(theta);
+    }
+  return GTBO_OK;
+}
+
+extern "C" int gtbo_kpm_moments(const gtbo_ell* H, double a, double b, int32_t M,
+                                int32_t R, uint64_t seed, int32_t mode, int32_t algo,
+                                double* mu, double* im_max) {
+  if (!H || !mu || M <= 0 || H->n <= 0 || !(a > 0.0) || (mode == 0 && R <= 0) ||
+      (mode != 0 && mode != 1) || (algo != 0 && algo != 1))
+    return GTBO_ERR_INVALID_ARG;
+  const int64_t n = H->n;
+  const int64_t n_vec = (mode == 0) ? R : n;
+  // per-vector moments, summed over vectors in index order afterwards.  Vectors
+  // are independent; in exact-trace mode (many short vectors) the loop over
+  // vectors is the parallel one, otherwise the row loops inside are.
+  std::vector<double> all_re((size_t)n_vec * M), all_im((size_t)n_vec * M);
+#pragma omp parallel for schedule(dynamic, 8) if (mode == 1)
+  for (int64_t r = 0; r < n_vec; ++r) {
+    std::vector<double> m_re, m_im;
+    std::vector<cplx> phi0(n);
+    if (mode == 0) {
+      for (int64_t i = 0; i < n; ++i) {
+        const double theta = 6.283185307179586 * gtbo_uniform(seed, (uint32_t)r, (uint64_t)i);
+        phi0[i].re = std::cos(theta);
+        phi0[i].im = std::sin(theta);
+      }
+    } else {
+      std::memset(phi0.data(), 0, sizeof(cplx) * (size_t)n);
+      phi0[r].re = 1.0;  // basis vector e_r
+    }
+    vector_moments(H, a, b, M, algo, phi0, m_re, m_im);
+    for (int32_t k = 0; k < M; ++k) {
+      all_re[(size_t)r * M + k] = m_re[k];
+      all_im[(size_t)r * M + k] = m_im[k];
+    }
+  }
+  std::vector<double> sum_re(M, 0.0), sum_im(M, 0.0);
+  for (int64_t r = 0; r < n_vec; ++r)
+    for (int32_t k = 0; k < M; ++k) {
+      sum_re[k] += all_re[(size_t)r * M + k];
+      sum_im[k] += all_im[(size_t)r * M + k];
+    }
+  const double norm = (mode == 0) ? (double)n * (double)R : (double)n;
+  double worst = 0.0;
+  for (int32_t k = 0; k < M; ++k) {
+    mu[k] = sum_re[k] / norm;
+    worst = std::fmax(worst, std::fabs(sum_im[k] / norm));
+  }
+  if (im_max) *im_max = worst;
+  return GTBO_OK;
+}
+
+extern "C" int gtbo_kpm_step_rows(const gtbo_ell* H, double a, double b, int32_t first,
+                                  int32_t R, const double* phi_prev, const double* phi_cur,
+                                  const int64_t* rows, int64_t n_rows, double* out) {
+  if (!H || !phi_cur || !rows || !out || R <= 0 || (!first && !phi_prev))
+    return GTBO_ERR_INVALID_ARG;
+  const int64_t n = H->n;
+  for (int64_t q = 0; q < n_rows; ++q) {
+    const int64_t i = rows[q];
+    if (i < 0 || i >= n) return GTBO_ERR_INVALID_ARG;
+    for (int32_t r = 0; r < R; ++r)
+      for (int c = 0; c < 2; ++c) {
+        double acc = 0.0;
+        for (int32_t k = 0; k < H->width; ++k) {
+          const int64_t j = H->cols[(size_t)k * n + i];
+          acc = acc + H->vals[(size_t)k * n + i] * phi_cur[((size_t)j * R + r) * 2 + c];
+        }
+        const double own = phi_cur[((size_t)i * R + r) * 2 + c];
+        if (H->diag) acc = acc + H->diag[i] * own;
+        double v;
+        if (first)
+          v = (acc - b * own) * (1.0 / a);
+        else
+          v = (acc - b * own) * (2.0 / a) - phi_prev[((size_t)i * R + r) * 2 + c];
+        out[((size_t)q * R + r) * 2 + c] = v;
+      }
+  }
+  return GTBO_OK;
+}
+
+// C6. Jackson kernel, M-moment convention (A13):
+//   g_n = [(M-n+1) cos(pi n/(M+1)) + sin(pi n/(M+1)) cot(pi/(M+1))] / (M+1)
+extern "C" int gtbo_jackson(int32_t M, double* g) {
+  if (M <= 0 || !g) return GTBO_ERR_INVALID_ARG;
+  const long double pi = 3.141592653589793238462643383279502884L;
+  const long double q = pi / (long double)(M + 1);
+  for (int32_t n = 0; n < M; ++n)
+    g[n] = (double)((((long double)(M - n + 1)) * cosl(q * n) + sinl(q * n) / tanl(q)) /
+                    (long double)(M + 1));
+  return GTBO_OK;
+}
+
+// rho(E) = scale [g_0 mu_0 + 2 sum_{n>=1} g_n mu_n T_n(x)] / (pi a sqrt(1-x^2)),
+// x = (E-b)/a, T_n(x) = cos(n arccos x); rho = 0 for |x| >= 1.
+extern "C" int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
+                        const double* energies, int32_t G, double scale, double* rho) {
+  if (!mu || !energies || !rho || M <= 0 || G < 0 || !(a > 0.0) ||
+      (kernel != 0 && kernel != 1))
+    return GTBO_ERR_INVALID_ARG;
+  std::vector<double> g(M, 1.0);
+  if (kernel == 1) gtbo_jackson(M, g.data());
+  const long double pi = 3.141592653589793238462643383279502884L;
+#pragma omp parallel for schedule(static)
+  for (int32_t j = 0; j < G; ++j) {
+    const double x = (energies[j] - b) / a;
+    if (!(std::fabs(x) < 1.0)) {
+      rho[j] = 0.0;
+      continue;
+    }
+    const long double th = acosl((long double)x);
+    long double s = (long double)g[0] * mu[0];
+    for (int32_t n = 1; n < M; ++n)
+      s += 2.0L * (long double)g[n] * (long double)mu[n] * cosl((long double)n * th);
+    rho[j] = (double)((long double)scale * s /
+                      (pi * (long double)a * sqrtl(1.0L - (long double)x * x)));
+  }
+  return GTBO_OK;
+}
