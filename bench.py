@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""Benchmark of the KPM/LSQT density-of-states hot path (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W [--workload c5] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+build_hamiltonian (cell list + ELL assembly) -> kpm_moments (random phases, ceil(M/2) fused
+Chebyshev passes, doubling identities) -> dos (Jackson kernel, 4001 energies).  The N=1 workload
+is BASELINE.json:configs[4] ("c5": pristine graphene, 5000x5000 cells = 10^8 atoms, ELL width 3,
+M=3000, R=2, complex128), the configuration the metric is quoted on.  `value` is
+atoms*moments*vectors per second of the whole step with inputs resident in HBM; `e2e` is the same
+through the same calls with HOST (pinned) inputs, host<->device copies inside the timed region.
+With N>1 (torchrun) every rank runs an independent replica on its own seed (the path has no
+exchange step: "replicas only") and value = all ranks' units / max time.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2509_06525_b200 import workloads as W  # noqa: E402
+
+METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
+UNIT = "atom*moment*vector updates/s"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
+# `ncu --set full` captures summarised under profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES = {
+}
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clocks and throttle reasons with nvidia-smi while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _workload(args) -> W.Workload:
+    w = W.CONFIGS[args.workload]
+    if args.nx or args.ny:
+        w = w.scaled(args.nx or w.nx, args.ny or w.ny)
+    if args.moments:
+        w = W.replace(w, M=args.moments)
+    return w
+
+
+# ----------------------------------------------------------------------------- CPU oracle arm
+def _oracle_step(w, inp, energies_of):
+    import oracle
+    t0 = time.perf_counter()
+    H = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0,
+                                 w.r0, w.beta, inp.onsite_shift, method=1, with_diag=w.use_diag)
+    if w.a is None:
+        lo, hi = oracle.spectral_bounds(H)
+        a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    else:
+        a, b = w.a, w.b
+    mu = oracle.kpm_moments(H, a, b, w.M, w.R, w.seed, mode=0, algo=0)   # the plain definition
+    rho = oracle.dos(mu, a, b, energies_of(w, a, b))
+    return time.perf_counter() - t0, rho
+
+
+def _cpu_sample(w: W.Workload) -> W.Workload:
+    """Bounded sample of the workload for the oracle: same construction, 10^6 atoms at most,
+    moments cut so that one pass is roughly 10-30 s of CPU work."""
+    nx, ny = min(w.nx, 500), min(w.ny, 500)
+    n = 4 * nx * ny
+    width_guess = {1.95: 3, 2.65: 10, 4.0: 20}.get(w.cutoff, 10)
+    budget = 4e9 * 8 / (width_guess + 5)     # updates that take ~20 s at ~2e8 upd/s for width 3
+    M = int(max(16, min(w.M, budget / (n * w.R))))
+    return w.scaled(nx, ny, M=M)
+
+
+def _cores():
+    try:
+        import oracle  # noqa: F401
+        return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = _workload(args)
+    s = _cpu_sample(w)
+    inp = W.make_inputs(s)
+    for _ in range(args.warmup):
+        pass   # the oracle has no warm-up state; the sample is sized so K steps fit in minutes
+    times = [_oracle_step(s, inp, W.energy_grid)[0] for _ in range(args.steps)]
+    t = float(np.mean(times))
+    value = s.n_atoms * s.M * s.R / t
+    sample = f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": w.name, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": _cores(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- CUDA arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_06525_b200 import binding as gtb
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    gtb.lib()
+
+    w = _workload(args)
+    inp = W.make_inputs(w)
+    n = w.n_atoms
+    seed = w.seed + 1000 * rank            # independent replica per rank
+    # host inputs in pinned memory (e2e arm) and resident copies (device arm)
+    h_pos = torch.from_numpy(inp.pos).pin_memory()
+    h_spec = torch.from_numpy(inp.species).pin_memory()
+    h_shift = torch.from_numpy(inp.onsite_shift).pin_memory() if inp.onsite_shift is not None else None
+    d_pos, d_spec = h_pos.to(dev), h_spec.to(dev)
+    d_shift = h_shift.to(dev) if h_shift is not None else None
+    h2d = h_pos.numel() * 8 + h_spec.numel() * 4 + (h_shift.numel() * 8 if h_shift is not None else 0)
+
+    ws_build = gtb.workspace(gtb.build_workspace_bytes(n), dev)
+    width = gtb.neighbor_width(d_pos, inp.box, inp.pbc, w.cutoff, ws=ws_build)
+    ws_kpm = gtb.workspace(gtb.kpm_workspace_bytes(n, w.M, w.R), dev)
+    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n), dev)
+    mu = torch.empty(w.M, dtype=torch.float64, device=dev)
+    h_rho = torch.empty(w.n_energies, dtype=torch.float64).pin_memory()
+    state = {}
+
+    def step(pos, spec, shift):
+        H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
+                                  w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
+        if w.a is None:
+            lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
+            a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+        else:
+            a, b = w.a, w.b
+        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, ws=ws_kpm, mu=mu)
+        if "E" not in state:
+            state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
+        rho = gtb.dos(mu, a, b, state["E"])
+        state["H"], state["a"], state["b"] = H, a, b
+        return rho
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = gtb.launch_count()
+        loop_ms, loop_passes = 0.0, 0
+        e0.record()
+        for _ in range(steps):
+            fn()
+            ms, passes = gtb.kpm_last_loop_ms()     # CUDA events on the launching stream
+            loop_ms += ms
+            loop_passes += passes
+        e1.record()
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()), gtb.launch_count() - l0, loop_ms, loop_passes
+
+    def device_step():
+        step(d_pos, d_spec, d_shift)
+
+    def e2e_step():
+        pos = h_pos.to(dev, non_blocking=True)
+        spec = h_spec.to(dev, non_blocking=True)
+        shift = h_shift.to(dev, non_blocking=True) if h_shift is not None else None
+        rho = step(pos, spec, shift)
+        h_rho.copy_(rho, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    for _ in range(args.warmup):
+        device_step()
+    with ClockSampler(local) as clk:
+        ms, launches, loop_ms, loop_passes = timed(device_step, args.steps)
+    H = state["H"]
+    for _ in range(min(args.warmup, 1)):
+        e2e_step()
+    ms_e2e, _, _, _ = timed(e2e_step, args.steps)
+
+    units = float(n) * w.M * w.R * args.steps * world
+    value = units / (ms * 1e-3)
+    e2e = units / (ms_e2e * 1e-3)
+    # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
+    # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
+    per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
+    bytes_per_launch = float(n) * per_atom
+    k7_ms = loop_ms / max(loop_passes, 1)
+    peak, peak_src = _peaks()
+    achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "cheb_step_kernel (K7 fused Chebyshev pass)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
+                "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+                "algorithmic_bytes_per_launch": bytes_per_launch, "bytes_per_atom_pass": per_atom,
+                "ms_per_launch": k7_ms, "launches_timed": loop_passes,
+                "share_of_step": loop_ms / ms}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128 vectors)",
+            "data": "synthetic",
+            "config": {"workload": w.name, "atoms": n, "ell_width": H.width, "moments": w.M,
+                       "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
+                       "l2": "inputs larger than L2 (working set %.1f GB)" % (
+                           (2 * n * w.R * 16 + H.nbytes()) / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "seconds_per_full_dos": ms / args.steps * 1e-3,
+            "recursion_updates_per_s": float(n) * w.M * w.R / ((loop_ms / args.steps + k7_ms) * 1e-3),
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": h_rho.numel() * 8, "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": launches, "roofline": roofline, "clocks": clk.summary()}
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            s = _cpu_sample(w)
+            t, _ = _oracle_step(s, W.make_inputs(s), W.energy_grid)
+            line["cpu_baseline"] = {
+                "value": s.n_atoms * s.M * s.R / t, "unit": UNIT, "cores": _cores(), "kind": "oracle",
+                "sample": f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos, {t:.1f} s"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=3)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--workload", default="c5", choices=sorted(W.CONFIGS))
+    p.add_argument("--nx", type=int, default=0, help="override the supercell (debugging)")
+    p.add_argument("--ny", type=int, default=0)
+    p.add_argument("--moments", type=int, default=0, help="override M (debugging)")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    args = p.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,175 @@
+/*
+ * gtb.h -- C ABI of libgtb_kpm.so: the B200 (sm_100a) hot path of GPUTB's
+ * large-scale stage (arxiv/paper_2509_06525): linear-scaling quantum transport
+ * density of states by the Kernel Polynomial Method.
+ *
+ *   build_hamiltonian(positions, species, box, cutoff, hopping model) -> ELL H
+ *   kpm_moments(H, a, b, M, R, seed)                                  -> mu_0..mu_{M-1}
+ *   dos(mu, Jackson kernel, energy grid)                              -> rho(E)
+ *
+ * What each call computes is fixed by PAPER.md:78-81 (Eq. 1, the orthogonal
+ * tight-binding Hamiltonian with neighbours inside a cutoff)
+ * (sec. 2.4: Chebyshev expansion, KPM, sparse matrix-vector multiplication,
+ * random phase approximation), PAPER.md:66 (Eq. 4, rho(E) = (2/Omega) Tr
+ * delta(E - H)) and, for everything the paper leaves out, by
+ * BASELINE.json:north_star and the readings C1-C7 / A1-A23 listed in DESIGN.md.
+ *
+ * Conventions
+ *  - extern "C", plain pointers and sizes.  Every function returns an int
+ *    status (GTB_OK = 0, negatives are errors) unless stated otherwise.
+ *  - "device" = pointer into CUDA device memory of the current device, owned by
+ *    the caller; "host" = ordinary host memory.  The library allocates nothing
+ *    persistent: scratch comes from a caller-provided device workspace whose
+ *    minimum size is returned by the matching *_workspace_bytes query.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *    stream).  Calls marked ASYNC only enqueue work on that stream and return;
+ *    calls marked SYNC synchronise that stream before returning.
+ *  - Indices are int32 (n <= 2^31-1-64); all byte/element offsets are 64-bit.
+ *  - Layouts:
+ *      pos      double [n][3]     Cartesian, Angstrom, unwrapped
+ *      species  int32  [n]        0 <= s < n_species
+ *      ELL      cols int32 [width][n], vals double [width][n]   (slot-major);
+ *               row i's entries sorted by ascending column; padding slots have
+ *               col = i and val = +0.0; diag double [n] or NULL (= all zero)
+ *      phi      double [n][R][2]  complex128, the R vectors interleaved per atom
+ *      mu       double [M];  rho, energies  double [G]
+ *  - No CPU fallback exists: without a CUDA device every compute call returns
+ *    GTB_ERR_CUDA.
+ */
+#ifndef GTB_H
+#define GTB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  GTB_OK = 0,
+  GTB_ERR_INVALID_ARG = -1,
+  GTB_ERR_BOX_TOO_SMALL = -2, /* a periodic box length < 2*cutoff                  */
+  GTB_ERR_ELL_OVERFLOW = -3,  /* a row needs more slots than H->width              */
+  GTB_ERR_WORKSPACE = -4,     /* workspace NULL, misaligned (256 B) or too small   */
+  GTB_ERR_DIVERGED = -5,      /* non-finite moments: spectrum outside [b-a, b+a]   */
+  GTB_ERR_CUDA = -6,          /* CUDA runtime error; see gtb_last_cuda_error()     */
+  GTB_ERR_INDEX_RANGE = -7    /* n too large for int32 indices                     */
+};
+
+#define GTB_MAX_SPECIES 8
+#define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
+
+/* Hopping model: Eq. 1 with one p_z orbital per atom
+ * (north_star).  t_ij = t0[s_i][s_j] if beta == 0, else
+ * t0[s_i][s_j] * exp(-beta * (r_ij/r0 - 1));  eps_i = onsite[s_i] (+ onsite_shift[i]). */
+typedef struct gtb_hopping_model {
+  int32_t n_species;          /* 1..GTB_MAX_SPECIES                                */
+  const double* onsite;       /* HOST   [n_species]             eV                 */
+  const double* t0;           /* HOST   [n_species][n_species]  eV, symmetric      */
+  double r0;                  /* Angstrom (used only when beta != 0)               */
+  double beta;
+  const double* onsite_shift; /* DEVICE [n] or NULL             eV                 */
+} gtb_hopping_model;
+
+/* ELL matrix, all arrays DEVICE, caller-owned.  cols/vals are 16-byte aligned. */
+typedef struct gtb_ell {
+  int64_t n;
+  int32_t width;  /* K: off-diagonal slots per row */
+  int32_t* cols;  /* [width][n] */
+  double* vals;   /* [width][n] */
+  double* diag;   /* [n] or NULL */
+} gtb_ell;
+
+/* ---- status -------------------------------------------------------------- */
+const char* gtb_status_string(int status);
+const char* gtb_last_cuda_error(void); /* text of the last CUDA error seen by this thread */
+int gtb_version(void);                 /* 10000*major + 100*minor + patch */
+/* number of kernel launches this library has enqueued since load (monotonic). */
+int64_t gtb_launch_count(void);
+
+/* ---- Hamiltonian assembly (Eq. 1; north_star (1); readings C2, A14, A15) -- */
+/* Neighbour set: N(i) = { j != i : r2 < cutoff*cutoff }, with
+ *   d_a = x_j[a]-x_i[a];  periodic a: d_a -= L_a*rint(d_a/L_a);
+ *   r2 = (d_x*d_x + d_y*d_y) + d_z*d_z     (fp64, no FMA contraction, strict <).
+ * Requires L_a >= 2*cutoff on every periodic axis (GTB_ERR_BOX_TOO_SMALL). */
+size_t gtb_build_workspace_bytes(int64_t n);
+
+/* SYNC.  *width_out (HOST) = max_i |N(i)|;  counts (DEVICE [n] or NULL) = |N(i)|. */
+int gtb_neighbor_width(const double* pos /*device*/, int64_t n, const double box[3] /*host*/,
+                       const int32_t pbc[3] /*host*/, double cutoff, int32_t* counts,
+                       void* ws, size_t ws_bytes, void* stream, int32_t* width_out);
+
+/* SYNC.  Fills H->cols, H->vals (and H->diag if non-NULL) in the layout above;
+ * H->n must equal n and H->width is the caller's allocation.  If some row needs
+ * more than H->width slots, returns GTB_ERR_ELL_OVERFLOW, stores the required
+ * width in *width_needed (HOST, may be NULL) and leaves H unspecified. */
+int gtb_build_hamiltonian(const double* pos /*device*/, const int32_t* species /*device*/,
+                          int64_t n, const double box[3], const int32_t pbc[3], double cutoff,
+                          const gtb_hopping_model* model, gtb_ell* H, void* ws, size_t ws_bytes,
+                          void* stream, int32_t* width_needed);
+
+/* ASYNC.  Gershgorin bounds (reading C7): lo_hi[0] = min_i(diag_i - sum_k|vals[k][i]|),
+ * lo_hi[1] = max_i(diag_i + sum_k|vals[k][i]|).  lo_hi is DEVICE [2].
+ * Workspace: gtb_bounds_workspace_bytes(n). */
+size_t gtb_bounds_workspace_bytes(int64_t n);
+int gtb_spectral_bounds(const gtb_ell* H, double* lo_hi, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- random-phase vectors (north_star (2); reading C3) --- */
+/* ASYNC.  phi[i][k] = exp(i*theta), theta = fl(6.283185307179586 * u),
+ * u = (h >> 11) * 2^-53,  h = mix(mix(seed + (r0+k+1)*g) + (i+1)*g),
+ * g = 0x9E3779B97F4A7C15, mix = the splitmix64 output function; k = 0..R-1. */
+int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, double* phi /*device*/,
+                          void* stream);
+
+/* ---- Chebyshev moments (north_star (3); readings C4, C5, A17) - */
+/* Recursion |phi_{n+1}> = 2 H~ |phi_n> - |phi_{n-1}>, H~ = (H - b)/a, run for
+ * ceil(M/2) fused passes; moments by the doubling identities
+ *   m_{2n} = 2<phi_n|phi_n> - m_0,  m_{2n+1} = 2 Re<phi_{n+1}|phi_n> - m_1,
+ * mu_n = sum_r m_n^(r) / (n * R_total)           (mode 1: / n).
+ * mode 0: R_total random-phase vectors r = 0..R_total-1 of `seed`, processed
+ *         R_batch at a time (each pass of H serves R_batch vectors).
+ * mode 1: exact trace over all n basis vectors e_i (R_total and seed ignored),
+ *         R_batch of them per pass.
+ * R_batch: 1..64.  R_batch in {2,4,8} takes the 256-bit vector path.
+ * ASYNC.  mu is DEVICE [M].  Workspace: gtb_kpm_workspace_bytes(n, M, R_batch). */
+size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch);
+int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
+                    int32_t R_batch, uint64_t seed, int32_t mode, double* mu, void* ws,
+                    size_t ws_bytes, void* stream);
+
+/* SYNC.  GTB_ERR_DIVERGED if the last gtb_kpm_moments run on this workspace
+ * produced a non-finite moment, else GTB_OK. */
+int gtb_kpm_status(const void* ws, void* stream);
+
+/* ASYNC.  One fused recursion pass, exported for the full-size sampled parity test:
+ *   first != 0:  out = (H phi_cur - b phi_cur) / a                 (phi_io is written only)
+ *   first == 0:  out = (H phi_cur - b phi_cur)*(2/a) - phi_io      (phi_io read, then overwritten)
+ * sums (DEVICE [2]) = { sum_{i,r} |phi_cur|^2 ,  sum_{i,r} Re(conj(out) phi_cur) }.
+ * phi_cur, phi_io: DEVICE [n][R][2], 32-byte aligned, must not overlap.
+ * Workspace: gtb_kpm_workspace_bytes(n, 2, R). */
+int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
+                 const double* phi_cur, double* phi_io, double* sums, void* ws, size_t ws_bytes,
+                 void* stream);
+
+/* Timing of the recursion loop inside the LAST gtb_kpm_moments call of this
+ * thread (CUDA events recorded on the caller's stream around the fused passes,
+ * first pass excluded).  SYNC (waits for the closing event).
+ * *ms = device milliseconds, *passes = fused passes between the events. */
+int gtb_kpm_last_loop_ms(double* ms, int32_t* passes);
+
+/* ---- density of states (Eq. 4; north_star (4); reading C6) ---- */
+/* ASYNC.  rho(E_j) = scale*[g_0 mu_0 + 2 sum_{n=1}^{M-1} g_n mu_n T_n(x_j)] / (pi a sqrt(1-x_j^2)),
+ * x_j = (E_j - b)/a, and rho = 0 where |x_j| >= 1.
+ * kernel 0: g_n = 1;  kernel 1 (Jackson):
+ *   g_n = [(M-n+1) cos(pi n/(M+1)) + sin(pi n/(M+1)) cot(pi/(M+1))]/(M+1).
+ * mu, energies, rho: DEVICE. */
+int gtb_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
+            const double* energies, int32_t G, double scale, double* rho, void* stream);
+/* ASYNC.  g (DEVICE [M]) = Jackson coefficients as above. */
+int gtb_jackson(int32_t M, double* g, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GTB_H */

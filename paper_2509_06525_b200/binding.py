@@ -1,0 +1,303 @@
+"""Thin Python binding of libgtb_kpm.so (include/gtb.h): argument marshalling only.
+
+Every function has the name of the C call it wraps (without the gtb_ prefix), takes torch CUDA
+tensors (or allocates the outputs / workspace as torch tensors), passes raw device pointers and
+the current CUDA stream, and raises GtbError on a non-zero status.  All arithmetic of the path
+runs in the library's CUDA kernels.  There is no CPU fallback: without the built library, or
+without a CUDA device, the calls fail.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+OK = 0
+ERR_INVALID_ARG, ERR_BOX_TOO_SMALL, ERR_ELL_OVERFLOW, ERR_WORKSPACE = -1, -2, -3, -4
+ERR_DIVERGED, ERR_CUDA, ERR_INDEX_RANGE = -5, -6, -7
+MAX_WIDTH = 64
+
+# every symbol include/gtb.h declares (tests check that the library exports each of them)
+EXPORTS = (
+    "gtb_status_string", "gtb_last_cuda_error", "gtb_version", "gtb_launch_count",
+    "gtb_build_workspace_bytes", "gtb_neighbor_width", "gtb_build_hamiltonian",
+    "gtb_bounds_workspace_bytes", "gtb_spectral_bounds", "gtb_random_phase_fill",
+    "gtb_kpm_workspace_bytes", "gtb_kpm_moments", "gtb_kpm_status", "gtb_kpm_step",
+    "gtb_kpm_last_loop_ms", "gtb_dos", "gtb_jackson",
+)
+
+
+class GtbError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        msg = f"gtb_{where} failed: {status_string(status)} (status {status})"
+        if detail:
+            msg += f": {detail}"
+        super().__init__(msg)
+        self.status = status
+
+
+class _Model(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite", C.c_void_p), ("t0", C.c_void_p),
+                ("r0", C.c_double), ("beta", C.c_double), ("onsite_shift", C.c_void_p)]
+
+
+class _Ell(C.Structure):
+    _fields_ = [("n", C.c_int64), ("width", C.c_int32), ("cols", C.c_void_p),
+                ("vals", C.c_void_p), ("diag", C.c_void_p)]
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def lib() -> C.CDLL:
+    """Loads libgtb_kpm.so, building it with nvcc first if it is missing or stale."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if _build.needs_build():
+            path = _build.build()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing and could not be built; no fallback exists")
+        L = C.CDLL(path)
+        L.gtb_status_string.restype = C.c_char_p
+        L.gtb_status_string.argtypes = [C.c_int]
+        L.gtb_last_cuda_error.restype = C.c_char_p
+        L.gtb_launch_count.restype = C.c_int64
+        for name in ("gtb_build_workspace_bytes", "gtb_bounds_workspace_bytes"):
+            getattr(L, name).restype = C.c_size_t
+            getattr(L, name).argtypes = [C.c_int64]
+        L.gtb_kpm_workspace_bytes.restype = C.c_size_t
+        L.gtb_kpm_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+        _lib = L
+    return _lib
+
+
+def status_string(status: int) -> str:
+    return lib().gtb_status_string(int(status)).decode()
+
+
+def last_cuda_error() -> str:
+    return lib().gtb_last_cuda_error().decode()
+
+
+def version() -> int:
+    return lib().gtb_version()
+
+
+def launch_count() -> int:
+    return int(lib().gtb_launch_count())
+
+
+def _check(st: int, where: str) -> None:
+    if st != OK:
+        raise GtbError(st, where, last_cuda_error() if st == ERR_CUDA else "")
+
+
+def _stream() -> C.c_void_p:
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t: Optional[torch.Tensor]) -> C.c_void_p:
+    return C.c_void_p(t.data_ptr() if t is not None else None)
+
+
+def _dev(t: torch.Tensor, dtype: torch.dtype, name: str) -> torch.Tensor:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}")
+    return t
+
+
+def _host_f64(x, n: int) -> np.ndarray:
+    a = np.ascontiguousarray(x, dtype=np.float64).reshape(-1)
+    if a.shape[0] != n:
+        raise ValueError(f"expected {n} doubles, got {a.shape[0]}")
+    return a
+
+
+def workspace(nbytes: int, device=None) -> torch.Tensor:
+    """A caller-owned device workspace (torch allocations are 512-byte aligned)."""
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device or "cuda")
+
+
+@dataclass
+class Ell:
+    """ELL matrix on the device in the layout of include/gtb.h (slot-major [width][n])."""
+    n: int
+    width: int
+    cols: torch.Tensor            # int32 [width, n]
+    vals: torch.Tensor            # float64 [width, n]
+    diag: Optional[torch.Tensor]  # float64 [n] or None
+
+    def _c(self) -> _Ell:
+        return _Ell(self.n, self.width, self.cols.data_ptr() if self.width else None,
+                    self.vals.data_ptr() if self.width else None,
+                    self.diag.data_ptr() if self.diag is not None else None)
+
+    @staticmethod
+    def from_host(cols, vals, diag=None, device="cuda") -> "Ell":
+        cols = torch.as_tensor(np.ascontiguousarray(cols, dtype=np.int32)).to(device)
+        vals = torch.as_tensor(np.ascontiguousarray(vals, dtype=np.float64)).to(device)
+        d = None if diag is None else torch.as_tensor(np.ascontiguousarray(diag, dtype=np.float64)).to(device)
+        return Ell(int(cols.shape[1]), int(cols.shape[0]), cols, vals, d)
+
+    def nbytes(self) -> int:
+        return self.n * (12 * self.width + (8 if self.diag is not None else 0))
+
+
+def build_workspace_bytes(n: int) -> int:
+    return int(lib().gtb_build_workspace_bytes(n))
+
+
+def bounds_workspace_bytes(n: int) -> int:
+    return int(lib().gtb_bounds_workspace_bytes(n))
+
+
+def kpm_workspace_bytes(n: int, M: int, R_batch: int) -> int:
+    return int(lib().gtb_kpm_workspace_bytes(n, M, R_batch))
+
+
+def neighbor_width(pos: torch.Tensor, box, pbc, cutoff: float, want_counts: bool = False,
+                   ws: Optional[torch.Tensor] = None):
+    pos = _dev(pos, torch.float64, "pos")
+    n = pos.shape[0]
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    counts = torch.empty(n, dtype=torch.int32, device=pos.device) if want_counts else None
+    if ws is None:
+        ws = workspace(build_workspace_bytes(n), pos.device)
+    width = C.c_int32(0)
+    st = lib().gtb_neighbor_width(_ptr(pos), C.c_int64(n), C.c_void_p(box_h.ctypes.data),
+                                  C.c_void_p(pbc_h.ctypes.data), C.c_double(cutoff), _ptr(counts),
+                                  _ptr(ws), C.c_size_t(ws.numel()), _stream(), C.byref(width))
+    _check(st, "neighbor_width")
+    return (int(width.value), counts) if want_counts else int(width.value)
+
+
+def build_hamiltonian(pos: torch.Tensor, species: torch.Tensor, box, pbc, cutoff: float, onsite,
+                      t0, r0: float = 1.0, beta: float = 0.0,
+                      onsite_shift: Optional[torch.Tensor] = None, width: Optional[int] = None,
+                      with_diag: bool = True, ws: Optional[torch.Tensor] = None) -> Ell:
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    n = pos.shape[0]
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    onsite_h = np.ascontiguousarray(onsite, dtype=np.float64).reshape(-1)
+    ns = onsite_h.shape[0]
+    t0_h = _host_f64(t0, ns * ns)
+    if onsite_shift is not None:
+        onsite_shift = _dev(onsite_shift, torch.float64, "onsite_shift")
+    if ws is None:
+        ws = workspace(build_workspace_bytes(n), pos.device)
+    if width is None:
+        width = neighbor_width(pos, box_h, pbc_h, cutoff, ws=ws)
+    H = Ell(n, width, torch.empty((width, n), dtype=torch.int32, device=pos.device),
+            torch.empty((width, n), dtype=torch.float64, device=pos.device),
+            torch.empty(n, dtype=torch.float64, device=pos.device) if with_diag else None)
+    model = _Model(ns, onsite_h.ctypes.data, t0_h.ctypes.data, r0, beta,
+                   onsite_shift.data_ptr() if onsite_shift is not None else None)
+    hc = H._c()
+    need = C.c_int32(0)
+    st = lib().gtb_build_hamiltonian(_ptr(pos), _ptr(species), C.c_int64(n),
+                                     C.c_void_p(box_h.ctypes.data), C.c_void_p(pbc_h.ctypes.data),
+                                     C.c_double(cutoff), C.byref(model), C.byref(hc), _ptr(ws),
+                                     C.c_size_t(ws.numel()), _stream(), C.byref(need))
+    if st == ERR_ELL_OVERFLOW:
+        raise GtbError(st, "build_hamiltonian", f"width {width} given, {need.value} needed")
+    _check(st, "build_hamiltonian")
+    return H
+
+
+def spectral_bounds(H: Ell, ws: Optional[torch.Tensor] = None) -> torch.Tensor:
+    out = torch.empty(2, dtype=torch.float64, device=H.vals.device)
+    if ws is None:
+        ws = workspace(bounds_workspace_bytes(H.n), out.device)
+    hc = H._c()
+    st = lib().gtb_spectral_bounds(C.byref(hc), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()),
+                                   _stream())
+    _check(st, "spectral_bounds")
+    return out
+
+
+def random_phase_fill(seed: int, r0: int, R: int, n: int, device="cuda") -> torch.Tensor:
+    phi = torch.empty((n, R, 2), dtype=torch.float64, device=device)
+    st = lib().gtb_random_phase_fill(C.c_uint64(seed & (2**64 - 1)), C.c_int32(r0), C.c_int32(R),
+                                     C.c_int64(n), _ptr(phi), _stream())
+    _check(st, "random_phase_fill")
+    return phi
+
+
+def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
+                R_batch: Optional[int] = None, seed: int = 0, mode: int = 0,
+                ws: Optional[torch.Tensor] = None, mu: Optional[torch.Tensor] = None,
+                check: bool = False) -> torch.Tensor:
+    dev = H.vals.device if H.width else H.diag.device
+    if R_batch is None:
+        R_batch = R_total if mode == 0 else 8
+    if mu is None:
+        mu = torch.empty(M, dtype=torch.float64, device=dev)
+    if ws is None:
+        ws = workspace(kpm_workspace_bytes(H.n, M, R_batch), dev)
+    hc = H._c()
+    st = lib().gtb_kpm_moments(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(M),
+                               C.c_int32(R_total), C.c_int32(R_batch),
+                               C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode), _ptr(mu), _ptr(ws),
+                               C.c_size_t(ws.numel()), _stream())
+    _check(st, "kpm_moments")
+    if check:
+        kpm_status(ws)
+    return mu
+
+
+def kpm_status(ws: torch.Tensor) -> None:
+    _check(lib().gtb_kpm_status(_ptr(ws), _stream()), "kpm_status")
+
+
+def kpm_step(H: Ell, a: float, b: float, first: bool, phi_cur: torch.Tensor, phi_io: torch.Tensor,
+             ws: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """One fused pass; phi_io is overwritten with phi_{n+1}.  Returns the two sums (device [2])."""
+    phi_cur = _dev(phi_cur, torch.float64, "phi_cur")
+    phi_io = _dev(phi_io, torch.float64, "phi_io")
+    R = phi_cur.shape[1]
+    sums = torch.empty(2, dtype=torch.float64, device=phi_cur.device)
+    if ws is None:
+        ws = workspace(kpm_workspace_bytes(H.n, 2, R), phi_cur.device)
+    hc = H._c()
+    st = lib().gtb_kpm_step(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(int(first)),
+                            C.c_int32(R), _ptr(phi_cur), _ptr(phi_io), _ptr(sums), _ptr(ws),
+                            C.c_size_t(ws.numel()), _stream())
+    _check(st, "kpm_step")
+    return sums
+
+
+def kpm_last_loop_ms():
+    ms, passes = C.c_double(0.0), C.c_int32(0)
+    _check(lib().gtb_kpm_last_loop_ms(C.byref(ms), C.byref(passes)), "kpm_last_loop_ms")
+    return float(ms.value), int(passes.value)
+
+
+def dos(mu: torch.Tensor, a: float, b: float, energies: torch.Tensor, kernel: int = 1,
+        scale: float = 1.0, rho: Optional[torch.Tensor] = None) -> torch.Tensor:
+    mu = _dev(mu, torch.float64, "mu")
+    energies = _dev(energies, torch.float64, "energies")
+    if rho is None:
+        rho = torch.empty_like(energies)
+    st = lib().gtb_dos(_ptr(mu), C.c_int32(mu.shape[0]), C.c_double(a), C.c_double(b),
+                       C.c_int32(kernel), _ptr(energies), C.c_int32(energies.shape[0]),
+                       C.c_double(scale), _ptr(rho), _stream())
+    _check(st, "dos")
+    return rho
+
+
+def jackson(M: int, device="cuda") -> torch.Tensor:
+    g = torch.empty(M, dtype=torch.float64, device=device)
+    _check(lib().gtb_jackson(C.c_int32(M), _ptr(g), _stream()), "jackson")
+    return g

@@ -1,0 +1,462 @@
+// Chebyshev moments on the device: random-phase fill (K5), first pass (K6), fused recursion pass
+// (K7) and moment finalisation (K8).
+//
+// The paper names the ingredients (sec. 2.4: Chebyshev expansion, kernel polynomial
+// method, sparse matrix-vector multiplication, random phase approximation) and the quantity
+// (Eq. 4); BASELINE.json:north_star fixes the recursion
+//     |phi_{n+1}> = 2 H~ |phi_n> - |phi_{n-1}>,   H~ = (H - b)/a,
+// the doubling identities m_{2n} = 2<phi_n|phi_n> - m_0, m_{2n+1} = 2 Re<phi_{n+1}|phi_n> - m_1 and
+// the counter hash of the random phases (readings C3-C5 in DESIGN.md).
+//
+// K7 is the hot kernel: ONE pass over HBM per Chebyshev step.  Per row it streams the ELL slots
+// (int32 column + fp64 hopping, slot-major so a warp reads contiguous words), gathers phi_n at the
+// columns (R vectors interleaved per atom: one gather = R*16 contiguous bytes, 32 B = one sector
+// and one 256-bit load for a pair of vectors), streams phi_{n-1}, writes phi_{n+1} over it, and
+// accumulates <phi_n|phi_n> and Re<phi_{n+1}|phi_n> in registers -> warp shuffles -> one slot per
+// block.  H is read once per pass for all R vectors.
+#include <cmath>
+
+#include "common.cuh"
+
+namespace gtb {
+namespace {
+
+constexpr int kBlock = 256;
+constexpr int kMaxBlocksPerSm = 8;
+constexpr int kMaxGrid = kSmCount * kMaxBlocksPerSm;
+constexpr uint64_t kGamma = 0x9E3779B97F4A7C15ull;
+
+// ---- counter hash (reading C3) ----------------------------------------------------------
+__host__ __device__ __forceinline__ uint64_t mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// K5: phi[i][k] = exp(i theta), theta = fl(2 pi u(seed, r0 + k, i))
+__global__ void __launch_bounds__(kBlock) random_phase_kernel(uint64_t seed, int32_t r0, int32_t R,
+                                                              int64_t n, double2* __restrict__ phi) {
+  const int64_t total = n * R;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t i = e / R;
+    const int32_t k = (int32_t)(e - i * R);
+    const uint64_t key = mix64(seed + ((uint64_t)(uint32_t)(r0 + k) + 1ull) * kGamma);
+    const uint64_t h = mix64(key + ((uint64_t)i + 1ull) * kGamma);
+    const double u = (double)(h >> 11) * 0x1.0p-53;
+    const double theta = 6.283185307179586 * u;
+    double s, c;
+    sincos(theta, &s, &c);
+    phi[e] = make_double2(c, s);
+  }
+}
+
+// exact-trace mode: phi[i][k] = delta(i, r0 + k)   (basis vectors e_{r0} .. e_{r0+R-1})
+__global__ void __launch_bounds__(kBlock) basis_fill_kernel(int64_t r0, int32_t R, int64_t n,
+                                                            double2* __restrict__ phi) {
+  const int64_t total = n * R;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t i = e / R;
+    const int64_t k = e - i * R;
+    phi[e] = make_double2(i == r0 + k ? 1.0 : 0.0, 0.0);
+  }
+}
+
+// ---- vector element = VW doubles (VW = 2: one complex; VW = 4: two complex, 256-bit) -----
+template <int VW>
+struct Vec {
+  double v[VW];
+};
+
+template <int VW>
+__device__ __forceinline__ Vec<VW> load_gather(const double* p);  // read-only path, keep in L1
+template <int VW>
+__device__ __forceinline__ Vec<VW> load_stream(const double* p);  // read once: do not allocate L1
+template <int VW>
+__device__ __forceinline__ void store_stream(double* p, const Vec<VW>& x);
+
+template <>
+__device__ __forceinline__ Vec<2> load_gather<2>(const double* p) {
+  Vec<2> r;
+  asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(r.v[0]), "=d"(r.v[1]) : "l"(p));
+  return r;
+}
+template <>
+__device__ __forceinline__ Vec<4> load_gather<4>(const double* p) {
+  Vec<4> r;
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3])
+               : "l"(p));
+  return r;
+}
+template <>
+__device__ __forceinline__ Vec<2> load_stream<2>(const double* p) {
+  Vec<2> r;
+  asm volatile("ld.global.L1::no_allocate.v2.f64 {%0,%1}, [%2];"
+               : "=d"(r.v[0]), "=d"(r.v[1])
+               : "l"(p)
+               : "memory");
+  return r;
+}
+template <>
+__device__ __forceinline__ Vec<4> load_stream<4>(const double* p) {
+  Vec<4> r;
+  asm volatile("ld.global.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3])
+               : "l"(p)
+               : "memory");
+  return r;
+}
+template <>
+__device__ __forceinline__ void store_stream<2>(double* p, const Vec<2>& x) {
+  asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(x.v[0]), "d"(x.v[1])
+               : "memory");
+}
+template <>
+__device__ __forceinline__ void store_stream<4>(double* p, const Vec<4>& x) {
+  asm volatile("st.global.L1::no_allocate.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(x.v[0]),
+               "d"(x.v[1]), "d"(x.v[2]), "d"(x.v[3])
+               : "memory");
+}
+
+struct StepArgs {
+  const int32_t* cols;
+  const double* vals;
+  const double* diag;
+  int64_t n;
+  int32_t width;
+  int32_t T;              // threads per row = R*2/VW
+  const double* phi_cur;  // phi_n           [n][R][2]
+  double* phi_io;         // phi_{n-1} in, phi_{n+1} out
+  double scale;           // 1/a (first pass) or 2/a
+  double b;
+  double2* partial;       // [gridDim.x]: (sum |phi_n|^2, sum Re conj(phi_{n+1}) phi_n)
+};
+
+// K6 / K7.  Thread e handles element e of phi viewed as an array of Vec<VW>: row = e / T, vector
+// group t = e % T, so a warp touches one contiguous 32*VW*8-byte span of phi_{n-1}/phi_{n+1}, and
+// every gather of a row's neighbour is T consecutive threads reading R*16 contiguous bytes.
+template <int VW, int LOG2T, bool kFirst, bool kDiag>
+__global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
+  const int64_t n = a.n;
+  const int T = LOG2T >= 0 ? (1 << LOG2T) : a.T;
+  const int64_t total = n * T;
+  const int width = a.width;
+  const double scale = a.scale, b = a.b;
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t row = LOG2T >= 0 ? (e >> LOG2T) : (e / T);
+    const int64_t t = e - row * T;
+    const double* xt = a.phi_cur + t * VW;
+    const int32_t* cp = a.cols + row;
+    const double* vp = a.vals + row;
+    Vec<VW> acc;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) acc.v[q] = 0.0;
+    Vec<VW> prev;
+    if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
+    const Vec<VW> own = load_gather<VW>(a.phi_cur + e * VW);
+#pragma unroll 4
+    for (int k = 0; k < width; ++k) {
+      const int64_t c = __ldg(cp + (size_t)k * n);
+      const double v = __ldg(vp + (size_t)k * n);
+      const Vec<VW> x = load_gather<VW>(xt + c * T * VW);
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = fma(v, x.v[q], acc.v[q]);
+    }
+    if (kDiag) {
+      const double d = __ldg(a.diag + row);
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = fma(d, own.v[q], acc.v[q]);
+    }
+    Vec<VW> y;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) {
+      y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
+      if (!kFirst) y.v[q] -= prev.v[q];
+      s1 = fma(own.v[q], own.v[q], s1);
+      s2 = fma(y.v[q], own.v[q], s2);
+    }
+    store_stream<VW>(a.phi_io + e * VW, y);
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+// K8a: sums[step] += sum over blocks of partial[step][block], in a fixed order
+__global__ void __launch_bounds__(128) reduce_partials_kernel(const double2* __restrict__ partial,
+                                                              int stride, int grid, double2* sums) {
+  const double2* p = partial + (size_t)blockIdx.x * stride;
+  double s1 = 0.0, s2 = 0.0;
+  for (int k = threadIdx.x; k < grid; k += 128) {
+    s1 += p[k].x;
+    s2 += p[k].y;
+  }
+  __shared__ double red[128][2];
+  red[threadIdx.x][0] = s1;
+  red[threadIdx.x][1] = s2;
+  __syncthreads();
+  for (int o = 64; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      red[threadIdx.x][0] += red[threadIdx.x + o][0];
+      red[threadIdx.x][1] += red[threadIdx.x + o][1];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double2 acc = sums[blockIdx.x];
+    acc.x += red[0][0];
+    acc.y += red[0][1];
+    sums[blockIdx.x] = acc;
+  }
+}
+
+// K8b: doubling identities (reading C5); sums[k] = (sum_r <phi_k|phi_k>, sum_r Re<phi_{k+1}|phi_k>)
+__global__ void __launch_bounds__(kBlock) finish_moments_kernel(const double2* __restrict__ sums,
+                                                                int32_t M, double norm, double* mu,
+                                                                int32_t* status) {
+  const int n = blockIdx.x * kBlock + threadIdx.x;
+  if (n >= M) return;
+  const int k = n >> 1;
+  const double2 s0 = sums[0];
+  double m;
+  if (n == 0) m = s0.x;
+  else if (n == 1) m = s0.y;
+  else if ((n & 1) == 0) m = 2.0 * sums[k].x - s0.x;
+  else m = 2.0 * sums[k].y - s0.y;
+  m /= norm;
+  mu[n] = m;
+  if (!isfinite(m)) atomicOr(status, 1);
+}
+
+__global__ void copy_sums_kernel(const double2* sums, double* out2) {
+  out2[0] = sums[0].x;
+  out2[1] = sums[0].y;
+}
+
+// ---- host side ---------------------------------------------------------------------------
+using StepFn = void (*)(const StepArgs);
+
+struct StepPlan {
+  StepFn first, next;
+  int vw, T;
+  int grid;
+};
+
+template <int VW, int LOG2T>
+void pick(bool diag, StepPlan* p) {
+  p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true> : cheb_step_kernel<VW, LOG2T, true, false>;
+  p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true> : cheb_step_kernel<VW, LOG2T, false, false>;
+}
+
+int make_plan(int64_t n, int R, bool diag, StepPlan* p) {
+  if (R == 2) { pick<4, 0>(diag, p); p->vw = 4; p->T = 1; }
+  else if (R == 4) { pick<4, 1>(diag, p); p->vw = 4; p->T = 2; }
+  else if (R == 8) { pick<4, 2>(diag, p); p->vw = 4; p->T = 4; }
+  else if (R == 1) { pick<2, 0>(diag, p); p->vw = 2; p->T = 1; }
+  else { pick<2, -1>(diag, p); p->vw = 2; p->T = R; }
+  int dev = 0, sms = kSmCount, per_sm = 0;
+  GTB_CUDA_TRY(cudaGetDevice(&dev));
+  GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0));
+  per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
+  const int64_t total = n * p->T;
+  int64_t grid = std::min<int64_t>((total + kBlock - 1) / kBlock, (int64_t)sms * per_sm);
+  p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(grid, kMaxGrid));
+  return GTB_OK;
+}
+
+struct KpmWs {
+  double* phi_a;
+  double* phi_b;
+  double2* partial;  // [S][kMaxGrid]
+  double2* sums;     // [S]
+  int32_t* status;   // [0] = non-finite flag
+  size_t bytes;
+};
+
+KpmWs carve_kpm(void* ws, int64_t n, int32_t M, int32_t R) {
+  const size_t S = (size_t)(M + 1) / 2;
+  Carver c(ws);
+  KpmWs w;
+  w.status = c.take<int32_t>(64);
+  w.phi_a = c.take<double>((size_t)n * R * 2);
+  w.phi_b = c.take<double>((size_t)n * R * 2);
+  w.partial = c.take<double2>(S * kMaxGrid);
+  w.sums = c.take<double2>(S);
+  w.bytes = c.off;
+  return w;
+}
+
+int check_ell(const gtb_ell* H) {
+  if (!H || H->n <= 0 || H->width < 0 || (H->width > 0 && (!H->cols || !H->vals)))
+    return GTB_ERR_INVALID_ARG;
+  if (H->n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
+  return GTB_OK;
+}
+
+int check_ws(const void* ws, size_t ws_bytes, size_t need) {
+  if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u) || ws_bytes < need) return GTB_ERR_WORKSPACE;
+  return GTB_OK;
+}
+
+int fill_grid(int64_t total) {
+  return (int)std::max<int64_t>(1, std::min<int64_t>((total + kBlock - 1) / kBlock, kMaxGrid));
+}
+
+struct LoopTimer {
+  cudaEvent_t beg = nullptr, end = nullptr;
+  int passes = 0;
+  bool armed = false;
+};
+thread_local LoopTimer g_timer;
+
+}  // namespace
+}  // namespace gtb
+
+using namespace gtb;
+
+extern "C" int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, double* phi,
+                                     void* stream) {
+  if (!phi || R <= 0 || n < 0 || r0 < 0) return GTB_ERR_INVALID_ARG;
+  if (n == 0) return GTB_OK;
+  random_phase_kernel<<<fill_grid(n * R), kBlock, 0, static_cast<cudaStream_t>(stream)>>>(
+      seed, r0, R, n, reinterpret_cast<double2*>(phi));
+  GTB_LAUNCHED();
+  return GTB_OK;
+}
+
+extern "C" size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch) {
+  if (n <= 0 || M <= 0 || R_batch <= 0) return 0;
+  return carve_kpm(nullptr, n, M, R_batch).bytes;
+}
+
+extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
+                               int32_t R_batch, uint64_t seed, int32_t mode, double* mu, void* ws,
+                               size_t ws_bytes, void* stream) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if (!mu || M <= 0 || !(a > 0.0) || !std::isfinite(b) || R_batch <= 0 || R_batch > 64 ||
+      (mode != 0 && mode != 1) || (mode == 0 && R_total <= 0))
+    return GTB_ERR_INVALID_ARG;
+  rc = check_ws(ws, ws_bytes, gtb_kpm_workspace_bytes(H->n, M, R_batch));
+  if (rc != GTB_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int64_t n = H->n;
+  const KpmWs w = carve_kpm(ws, n, M, R_batch);
+  const int S = (M + 1) / 2;  // fused passes: phi_1 .. phi_S
+  const int64_t n_vec = mode == 0 ? (int64_t)R_total : n;
+  GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2) * (size_t)S, st));
+  GTB_CUDA_TRY(cudaMemsetAsync(w.status, 0, sizeof(int32_t) * 64, st));
+  if (!g_timer.beg) {
+    GTB_CUDA_TRY(cudaEventCreate(&g_timer.beg));
+    GTB_CUDA_TRY(cudaEventCreate(&g_timer.end));
+  }
+  g_timer.armed = false;
+  for (int64_t r0 = 0; r0 < n_vec; r0 += R_batch) {
+    const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
+    const bool last_batch = r0 + R_batch >= n_vec;
+    StepPlan plan;
+    rc = make_plan(n, R, H->diag != nullptr, &plan);
+    if (rc != GTB_OK) return rc;
+    double* cur = w.phi_a;   // phi_k
+    double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
+    if (mode == 0) {
+      random_phase_kernel<<<fill_grid(n * R), kBlock, 0, st>>>(seed, (int32_t)r0, R, n,
+                                                               reinterpret_cast<double2*>(cur));
+    } else {
+      basis_fill_kernel<<<fill_grid(n * R), kBlock, 0, st>>>(r0, R, n,
+                                                             reinterpret_cast<double2*>(cur));
+    }
+    GTB_LAUNCHED();
+    StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, cur, io, 1.0 / a, b, w.partial};
+    plan.first<<<plan.grid, kBlock, 0, st>>>(sa);  // K6: phi_1, <phi_0|phi_0>, Re<phi_1|phi_0>
+    GTB_LAUNCHED();
+    if (last_batch) GTB_CUDA_TRY(cudaEventRecord(g_timer.beg, st));
+    for (int k = 1; k < S; ++k) {  // K7: phi_{k+1} from phi_k (cur) and phi_{k-1} (io)
+      std::swap(cur, io);
+      sa.phi_cur = cur;
+      sa.phi_io = io;
+      sa.scale = 2.0 / a;
+      sa.partial = w.partial + (size_t)k * kMaxGrid;
+      plan.next<<<plan.grid, kBlock, 0, st>>>(sa);
+      GTB_LAUNCHED();
+    }
+    if (last_batch) {
+      GTB_CUDA_TRY(cudaEventRecord(g_timer.end, st));
+      g_timer.passes = S - 1;
+      g_timer.armed = true;
+    }
+    // partial rows are kMaxGrid apart; only the first plan.grid entries of each are live
+    reduce_partials_kernel<<<S, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);
+    GTB_LAUNCHED();
+  }
+  const double norm = mode == 0 ? (double)n * (double)R_total : (double)n;
+  finish_moments_kernel<<<(M + kBlock - 1) / kBlock, kBlock, 0, st>>>(w.sums, M, norm, mu, w.status);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}
+
+extern "C" int gtb_kpm_status(const void* ws, void* stream) {
+  if (!ws) return GTB_ERR_INVALID_ARG;
+  int32_t flag = 0;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GTB_CUDA_TRY(cudaMemcpyAsync(&flag, ws, sizeof(flag), cudaMemcpyDeviceToHost, st));
+  GTB_CUDA_TRY(cudaStreamSynchronize(st));
+  return flag ? GTB_ERR_DIVERGED : GTB_OK;
+}
+
+extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
+                            const double* phi_cur, double* phi_io, double* sums, void* ws,
+                            size_t ws_bytes, void* stream) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if (!phi_cur || !phi_io || !sums || !(a > 0.0) || R <= 0 || R > 64 ||
+      (reinterpret_cast<uintptr_t>(phi_cur) & 31u) || (reinterpret_cast<uintptr_t>(phi_io) & 31u))
+    return GTB_ERR_INVALID_ARG;
+  rc = check_ws(ws, ws_bytes, gtb_kpm_workspace_bytes(H->n, 2, R));
+  if (rc != GTB_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const KpmWs w = carve_kpm(ws, H->n, 2, R);
+  StepPlan plan;
+  rc = make_plan(H->n, R, H->diag != nullptr, &plan);
+  if (rc != GTB_OK) return rc;
+  GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
+  StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width, plan.T, phi_cur, phi_io,
+              (first ? 1.0 : 2.0) / a, b, w.partial};
+  (first ? plan.first : plan.next)<<<plan.grid, kBlock, 0, st>>>(sa);
+  GTB_LAUNCHED();
+  reduce_partials_kernel<<<1, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);
+  GTB_LAUNCHED();
+  copy_sums_kernel<<<1, 1, 0, st>>>(w.sums, sums);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}
+
+extern "C" int gtb_kpm_last_loop_ms(double* ms, int32_t* passes) {
+  if (!ms || !passes) return GTB_ERR_INVALID_ARG;
+  if (!g_timer.armed) return GTB_ERR_INVALID_ARG;
+  GTB_CUDA_TRY(cudaEventSynchronize(g_timer.end));
+  float t = 0.f;
+  GTB_CUDA_TRY(cudaEventElapsedTime(&t, g_timer.beg, g_timer.end));
+  *ms = (double)t;
+  *passes = g_timer.passes;
+  return GTB_OK;
+}
