@@ -335,8 +335,9 @@ using namespace gtb;
 
 extern "C" int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, double* phi,
                                      void* stream) {
-  if (!phi || R <= 0 || n < 0 || r0 < 0) return GTB_ERR_INVALID_ARG;
+  if (R <= 0 || n < 0 || r0 < 0) return GTB_ERR_INVALID_ARG;
   if (n == 0) return GTB_OK;
+  if (!phi) return GTB_ERR_INVALID_ARG;
   random_phase_kernel<<<fill_grid(n * R), kBlock, 0, static_cast<cudaStream_t>(stream)>>>(
       seed, r0, R, n, reinterpret_cast<double2*>(phi));
   GTB_LAUNCHED();
