@@ -253,4 +253,6 @@ def test_end_to_end_dos(key, nx, ny, kw):
     mu = gtb.kpm_moments(Hg, a, b, M, w.R, w.R, w.seed)
     got = gtb.dos(mu, a, b, _dev(E)).cpu().numpy()
     assert np.abs(got - ref).max() <= DOS_TOL * ref.max()
-    assert abs(np.trapezoid(got, E) - 1.0) < 1e-3 and got.min() > -1e-12
+    # interior points only: when fl((E_max - b)/a) lands one ulp inside |x| < 1 the end point
+    # carries the 1/sqrt(1 - x^2) weight (both sides agree on it above; it is not part of the integral)
+    assert abs(np.trapezoid(got[1:-1], E[1:-1]) - 1.0) < 1e-3 and got.min() > -1e-12
