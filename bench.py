@@ -38,6 +38,7 @@ UNIT = "atom*moment*vector updates/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
 # `ncu --set full` captures summarised under profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = {
+    "c5-pristine-5000x5000": 13.178e9,     # profiles/r01_c5_k7_full.md (10.00 GB read + 3.18 GB written)
 }
 
 
@@ -168,6 +169,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2509_06525_b200 import binding as gtb
+    from paper_2509_06525_b200 import replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
@@ -183,7 +185,7 @@ def run_ours(args):
     w = _workload(args)
     inp = W.make_inputs(w)
     n = w.n_atoms
-    seed = w.seed + 1000 * rank            # independent replica per rank
+    seed = replicas.replica_seed(w.seed, rank)      # independent replica per rank
     # host inputs in pinned memory (e2e arm) and resident copies (device arm)
     h_pos = torch.from_numpy(inp.pos).pin_memory()
     h_spec = torch.from_numpy(inp.species).pin_memory()
@@ -216,9 +218,7 @@ def run_ours(args):
         return rho
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dev)
 
     def timed(fn, steps):
         barrier()
@@ -233,10 +233,8 @@ def run_ours(args):
             loop_passes += passes
         e1.record()
         barrier()
-        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item()), gtb.launch_count() - l0, loop_ms, loop_passes
+        t = replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+        return t, gtb.launch_count() - l0, loop_ms, loop_passes
 
     def device_step():
         step(d_pos, d_spec, d_shift)
@@ -258,9 +256,9 @@ def run_ours(args):
         e2e_step()
     ms_e2e, _, _, _ = timed(e2e_step, args.steps)
 
-    units = float(n) * w.M * w.R * args.steps * world
-    value = units / (ms * 1e-3)
-    e2e = units / (ms_e2e * 1e-3)
+    units = float(n) * w.M * w.R * args.steps            # per rank
+    value = replicas.whole_job_value(units, ms)
+    e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
