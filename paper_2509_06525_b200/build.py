@@ -45,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     tmp = LIB + ".tmp"
-    cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC, "-shared", "-o", tmp, *sources()]
+    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("GTB_NVCC_EXTRA", "").split(), "-I", INCLUDE, "-I", CSRC, "-shared", "-o", tmp, *sources()]
     res = subprocess.run(cmd, cwd=HERE, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -15,6 +15,7 @@
 // accumulates <phi_n|phi_n> and Re<phi_{n+1}|phi_n> in registers -> warp shuffles -> one slot per
 // block.  H is read once per pass for all R vectors.
 #include <cmath>
+#include <cstdlib>
 
 #include "common.cuh"
 
@@ -137,7 +138,7 @@ struct StepArgs {
 // K6 / K7.  Thread e handles element e of phi viewed as an array of Vec<VW>: row = e / T, vector
 // group t = e % T, so a warp touches one contiguous 32*VW*8-byte span of phi_{n-1}/phi_{n+1}, and
 // every gather of a row's neighbour is T consecutive threads reading R*16 contiguous bytes.
-template <int VW, int LOG2T, bool kFirst, bool kDiag>
+template <int VW, int LOG2T, bool kFirst, bool kDiag, int CH>
 __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
   const int64_t n = a.n;
   const int T = LOG2T >= 0 ? (1 << LOG2T) : a.T;
@@ -158,13 +159,36 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
     Vec<VW> prev;
     if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
     const Vec<VW> own = load_gather<VW>(a.phi_cur + e * VW);
+    if (CH == 0) {
 #pragma unroll 4
-    for (int k = 0; k < width; ++k) {
-      const int64_t c = __ldg(cp + (size_t)k * n);
-      const double v = __ldg(vp + (size_t)k * n);
-      const Vec<VW> x = load_gather<VW>(xt + c * T * VW);
+      for (int k = 0; k < width; ++k) {
+        const int64_t c = __ldg(cp + (size_t)k * n);
+        const double v = __ldg(vp + (size_t)k * n);
+        const Vec<VW> x = load_gather<VW>(xt + c * T * VW);
 #pragma unroll
-      for (int q = 0; q < VW; ++q) acc.v[q] = fma(v, x.v[q], acc.v[q]);
+        for (int q = 0; q < VW; ++q) acc.v[q] = fma(v, x.v[q], acc.v[q]);
+      }
+    } else {
+      // wide rows: CH slots at a time -- all CH column/hopping loads are issued before the CH
+      // gathers that depend on them, so a thread keeps 2*CH + CH loads in flight instead of 4
+      constexpr int C = CH > 0 ? CH : 1;
+      for (int k0 = 0; k0 < width; k0 += C) {
+        int32_t c[C];
+        double v[C];
+#pragma unroll
+        for (int j = 0; j < C; ++j) {
+          const bool ok = k0 + j < width;
+          c[j] = ok ? __ldg(cp + (size_t)(k0 + j) * n) : (int32_t)row;
+          v[j] = ok ? __ldg(vp + (size_t)(k0 + j) * n) : 0.0;
+        }
+        Vec<VW> x[C];
+#pragma unroll
+        for (int j = 0; j < C; ++j) x[j] = load_gather<VW>(xt + (int64_t)c[j] * T * VW);
+#pragma unroll
+        for (int j = 0; j < C; ++j)
+#pragma unroll
+          for (int q = 0; q < VW; ++q) acc.v[q] = fma(v[j], x[j].v[q], acc.v[q]);
+      }
     }
     if (kDiag) {
       const double d = __ldg(a.diag + row);
@@ -191,6 +215,177 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
   }
   __syncthreads();
   if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+// ---- K7t: the same pass with the Hamiltonian stream staged by TMA ------------------------------
+// With wide rows (K ~ 10-20) the register path above is latency-bound: every gather waits for a
+// column index that itself comes from HBM.  Here one lane-parallel producer (warp 0) copies the
+// next tiles' ELL slots (cols, vals, diag) into a ring of shared-memory stages with
+// cp.async.bulk (TMA, completion on an mbarrier) and bulk-prefetches the tiles' phi_{n-1}/phi_n
+// lines into L2, so the consumers' dependent chain is  LDS column -> gather  only.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        " selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+      "l"(src), "r"(bytes), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+
+constexpr int kBarBytes = 128;  // mbarrier ring at the start of dynamic shared memory
+
+// stage layout (TR rows): vals [width][TR] f64 | diag [TR] f64 | cols [width][TR] i32
+__host__ __device__ inline uint32_t tile_stage_bytes(int width, int TR, bool diag) {
+  return (uint32_t)((width * TR * 12 + (diag ? TR * 8 : 0) + 127) / 128 * 128);
+}
+
+template <int LOG2T, bool kFirst, bool kDiag, int CH>
+__global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int TR = kBlock / T;  // rows per tile: one thread per 256-bit element
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int64_t n = a.n;
+  const int width = a.width;
+  const double scale = a.scale, b = a.b;
+  const uint32_t stage_bytes = tile_stage_bytes(width, TR, kDiag);
+  const uint32_t vals_off = 0, diag_off = (uint32_t)width * TR * 8;
+  const uint32_t cols_off = diag_off + (kDiag ? TR * 8 : 0);
+  const uint32_t bar0 = smem_u32(smem);
+  unsigned char* const stage0 = smem + kBarBytes;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int64_t n_tiles = (n + TR - 1) / TR;
+  const int64_t my_tiles = blockIdx.x < n_tiles ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+
+  if (tid == 0) {
+    for (int s = 0; s < nstages; ++s) mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // producer: executed by all lanes of warp 0
+  auto issue = [&](int64_t i) {
+    const int s = (int)(i % nstages);
+    const int64_t row0 = (blockIdx.x + i * gridDim.x) * TR;
+    const uint32_t rows = (uint32_t)min((int64_t)TR, n - row0);
+    const uint32_t bar = bar0 + 8 * s;
+    const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
+    if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
+    __syncwarp();
+    for (int j = lane; j < 2 * width + 3; j += 32) {
+      if (j < width) {
+        bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
+      } else if (j < 2 * width) {
+        const int k = j - width;
+        bulk_g2s(base + vals_off + (uint32_t)k * TR * 8, a.vals + (size_t)k * n + row0, rows * 8, bar);
+      } else if (j == 2 * width) {
+        if (kDiag) bulk_g2s(base + diag_off, a.diag + row0, rows * 8, bar);
+      } else if (j == 2 * width + 1) {
+        bulk_prefetch_l2(a.phi_cur + row0 * (T * VW), rows * (T * VW * 8));
+      } else {
+        if (!kFirst) bulk_prefetch_l2(a.phi_io + row0 * (T * VW), rows * (T * VW * 8));
+      }
+    }
+  };
+  if (wid == 0)
+    for (int64_t i = 0; i < min((int64_t)nstages, my_tiles); ++i) issue(i);
+
+  double s1 = 0.0, s2 = 0.0;
+  const int rl = tid >> LOG2T;             // row within the tile
+  const int t = tid & (T - 1);             // 256-bit element within the row
+  const double* xt = a.phi_cur + t * VW;
+  for (int64_t i = 0; i < my_tiles; ++i) {
+    const int s = (int)(i % nstages);
+    const int64_t row = (blockIdx.x + i * gridDim.x) * TR + rl;
+    const bool live = row < n;
+    const int64_t e = row * T + t;
+    Vec<VW> prev, own, acc;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) acc.v[q] = prev.v[q] = own.v[q] = 0.0;
+    if (live) {
+      if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
+      own = load_gather<VW>(a.phi_cur + e * VW);
+    }
+    mbar_wait(bar0 + 8 * s, (uint32_t)((i / nstages) & 1));
+    const unsigned char* st = stage0 + (size_t)s * stage_bytes;
+    const int32_t* sc = reinterpret_cast<const int32_t*>(st + cols_off) + rl;
+    const double* sv = reinterpret_cast<const double*>(st + vals_off) + rl;
+    if (live) {
+      for (int k0 = 0; k0 < width; k0 += CH) {
+        int32_t c[CH];
+        double v[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+          const bool ok = k0 + j < width;
+          c[j] = ok ? sc[(k0 + j) * TR] : (int32_t)row;
+          v[j] = ok ? sv[(k0 + j) * TR] : 0.0;
+        }
+        Vec<VW> x[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) x[j] = load_gather<VW>(xt + (int64_t)c[j] * (T * VW));
+#pragma unroll
+        for (int j = 0; j < CH; ++j)
+#pragma unroll
+          for (int q = 0; q < VW; ++q) acc.v[q] = fma(v[j], x[j].v[q], acc.v[q]);
+      }
+      if (kDiag) {
+        const double d = reinterpret_cast<const double*>(st + diag_off)[rl];
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc.v[q] = fma(d, own.v[q], acc.v[q]);
+      }
+    }
+    __syncthreads();  // every thread has read stage s: hand it back to the producer
+    if (wid == 0 && i + nstages < my_tiles) issue(i + nstages);
+    if (live) {
+      Vec<VW> y;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
+        if (!kFirst) y.v[q] -= prev.v[q];
+        s1 = fma(own.v[q], own.v[q], s1);
+        s2 = fma(y.v[q], own.v[q], s2);
+      }
+      store_stream<VW>(a.phi_io + e * VW, y);
+    }
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (tid == 0) {
 #pragma unroll
     for (int w = 1; w < kBlock / 32; ++w) {
       s1 += red[w][0];
@@ -253,34 +448,123 @@ __global__ void copy_sums_kernel(const double2* sums, double* out2) {
 
 // ---- host side ---------------------------------------------------------------------------
 using StepFn = void (*)(const StepArgs);
+using TileFn = void (*)(const StepArgs, const int);
 
 struct StepPlan {
-  StepFn first, next;
-  int vw, T;
-  int grid;
+  StepFn first = nullptr, next = nullptr;   // register path (K6/K7)
+  TileFn tfirst = nullptr, tnext = nullptr; // TMA-staged path (K7t); used when stages > 0
+  int vw = 0, T = 0;
+  int grid = 0;
+  int stages = 0;
+  size_t smem = 0;
 };
 
-template <int VW, int LOG2T>
-void pick(bool diag, StepPlan* p) {
-  p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true> : cheb_step_kernel<VW, LOG2T, true, false>;
-  p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true> : cheb_step_kernel<VW, LOG2T, false, false>;
+template <int VW, int LOG2T, int CH>
+void pick_ch(bool diag, StepPlan* p) {
+  p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true, CH> : cheb_step_kernel<VW, LOG2T, true, false, CH>;
+  p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true, CH> : cheb_step_kernel<VW, LOG2T, false, false, CH>;
 }
 
-int make_plan(int64_t n, int R, bool diag, StepPlan* p) {
-  if (R == 2) { pick<4, 0>(diag, p); p->vw = 4; p->T = 1; }
-  else if (R == 4) { pick<4, 1>(diag, p); p->vw = 4; p->T = 2; }
-  else if (R == 8) { pick<4, 2>(diag, p); p->vw = 4; p->T = 4; }
-  else if (R == 1) { pick<2, 0>(diag, p); p->vw = 2; p->T = 1; }
-  else { pick<2, -1>(diag, p); p->vw = 2; p->T = R; }
+template <int VW, int LOG2T>
+void pick(bool diag, int ch, StepPlan* p) {
+  if (ch == 0) pick_ch<VW, LOG2T, 0>(diag, p);
+  else pick_ch<VW, LOG2T, 8>(diag, p);
+}
+
+template <int LOG2T, int CH>
+void pick_tile_ch(bool diag, StepPlan* p) {
+  p->tfirst = diag ? cheb_tile_kernel<LOG2T, true, true, CH> : cheb_tile_kernel<LOG2T, true, false, CH>;
+  p->tnext = diag ? cheb_tile_kernel<LOG2T, false, true, CH> : cheb_tile_kernel<LOG2T, false, false, CH>;
+}
+
+template <int LOG2T>
+void pick_tile(bool diag, int ch, StepPlan* p) {
+  switch (ch) {
+    case 3: pick_tile_ch<LOG2T, 3>(diag, p); break;
+    case 4: pick_tile_ch<LOG2T, 4>(diag, p); break;
+    case 6: pick_tile_ch<LOG2T, 6>(diag, p); break;
+    case 8: pick_tile_ch<LOG2T, 8>(diag, p); break;
+    default: pick_tile_ch<LOG2T, 10>(diag, p); break;
+  }
+}
+
+// gathers kept in flight per thread: the chunk that pads `width` least (ties: the larger)
+int tile_chunk(int width) {
+  if (width <= 3) return 3;
+  if (width <= 4) return 4;
+  int best = 10, waste = (width + 9) / 10 * 10 - width;
+  for (int ch : {8, 6}) {
+    const int w = (width + ch - 1) / ch * ch - width;
+    if (w < waste) { best = ch; waste = w; }
+  }
+  return best;
+}
+
+int env_int(const char* name, int dflt) {
+  const char* e = getenv(name);
+  return e ? atoi(e) : dflt;
+}
+
+int make_plan(const gtb_ell* H, int R, StepPlan* p) {
+  const int64_t n = H->n;
+  const int width = H->width;
+  const bool diag = H->diag != nullptr;
+  const int ch = width <= 4 ? 0 : 8;
+  int log2t = -1;
+  if (R == 2) { pick<4, 0>(diag, ch, p); p->vw = 4; p->T = 1; log2t = 0; }
+  else if (R == 4) { pick<4, 1>(diag, ch, p); p->vw = 4; p->T = 2; log2t = 1; }
+  else if (R == 8) { pick<4, 2>(diag, ch, p); p->vw = 4; p->T = 4; log2t = 2; }
+  else if (R == 1) { pick<2, 0>(diag, ch, p); p->vw = 2; p->T = 1; }
+  else { pick<2, -1>(diag, ch, p); p->vw = 2; p->T = R; }
   int dev = 0, sms = kSmCount, per_sm = 0;
   GTB_CUDA_TRY(cudaGetDevice(&dev));
   GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  // TMA-staged path: bulk copies need 16-byte aligned sources and sizes in every slot row
+  const bool aligned = n % 4 == 0 && width >= 1 &&
+                       !(reinterpret_cast<uintptr_t>(H->cols) & 15u) &&
+                       !(reinterpret_cast<uintptr_t>(H->vals) & 15u) &&
+                       !(reinterpret_cast<uintptr_t>(H->diag) & 15u);
+  int stages = env_int("GTB_K7_TILE", (width > 4 || R >= 4) ? 1 : 0) ? env_int("GTB_K7_STAGES", 2) : 0;
+  if (log2t < 0 || !aligned) stages = 0;
+  p->stages = 0;
+  if (stages > 0) {
+    const int tch = tile_chunk(width);
+    if (log2t == 0) pick_tile<0>(diag, tch, p);
+    else if (log2t == 1) pick_tile<1>(diag, tch, p);
+    else pick_tile<2>(diag, tch, p);
+    const int TR = kBlock / p->T;
+    const size_t stage_bytes = tile_stage_bytes(width, TR, diag);
+    int max_smem = 0;
+    GTB_CUDA_TRY(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    if (stages > 8) stages = 8;
+    while (stages > 1 && kBarBytes + stages * stage_bytes > (size_t)max_smem) --stages;
+    const size_t smem = kBarBytes + stages * stage_bytes;
+    if (smem <= (size_t)max_smem) {
+      GTB_CUDA_TRY(cudaFuncSetAttribute(p->tfirst, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      GTB_CUDA_TRY(cudaFuncSetAttribute(p->tnext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kBlock, smem));
+      per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
+      const int64_t n_tiles = (n + TR - 1) / TR;
+      p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, (int64_t)sms * per_sm));
+      p->grid = std::min(p->grid, kMaxGrid);
+      p->stages = stages;
+      p->smem = smem;
+      return GTB_OK;
+    }
+  }
   GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0));
   per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
   const int64_t total = n * p->T;
   int64_t grid = std::min<int64_t>((total + kBlock - 1) / kBlock, (int64_t)sms * per_sm);
   p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(grid, kMaxGrid));
   return GTB_OK;
+}
+
+void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st) {
+  if (p.stages > 0)
+    (first ? p.tfirst : p.tnext)<<<p.grid, kBlock, p.smem, st>>>(sa, p.stages);
+  else
+    (first ? p.first : p.next)<<<p.grid, kBlock, 0, st>>>(sa);
 }
 
 struct KpmWs {
@@ -375,7 +659,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    rc = make_plan(n, R, H->diag != nullptr, &plan);
+    rc = make_plan(H, R, &plan);
     if (rc != GTB_OK) return rc;
     double* cur = w.phi_a;   // phi_k
     double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
@@ -388,7 +672,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     }
     GTB_LAUNCHED();
     StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, cur, io, 1.0 / a, b, w.partial};
-    plan.first<<<plan.grid, kBlock, 0, st>>>(sa);  // K6: phi_1, <phi_0|phi_0>, Re<phi_1|phi_0>
+    launch_step(plan, true, sa, st);  // K6: phi_1, <phi_0|phi_0>, Re<phi_1|phi_0>
     GTB_LAUNCHED();
     if (last_batch) GTB_CUDA_TRY(cudaEventRecord(g_timer.beg, st));
     for (int k = 1; k < S; ++k) {  // K7: phi_{k+1} from phi_k (cur) and phi_{k-1} (io)
@@ -397,7 +681,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
       sa.phi_io = io;
       sa.scale = 2.0 / a;
       sa.partial = w.partial + (size_t)k * kMaxGrid;
-      plan.next<<<plan.grid, kBlock, 0, st>>>(sa);
+      launch_step(plan, false, sa, st);
       GTB_LAUNCHED();
     }
     if (last_batch) {
@@ -437,12 +721,12 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const KpmWs w = carve_kpm(ws, H->n, 2, R);
   StepPlan plan;
-  rc = make_plan(H->n, R, H->diag != nullptr, &plan);
+  rc = make_plan(H, R, &plan);
   if (rc != GTB_OK) return rc;
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
   StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width, plan.T, phi_cur, phi_io,
               (first ? 1.0 : 2.0) / a, b, w.partial};
-  (first ? plan.first : plan.next)<<<plan.grid, kBlock, 0, st>>>(sa);
+  launch_step(plan, first != 0, sa, st);
   GTB_LAUNCHED();
   reduce_partials_kernel<<<1, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);
   GTB_LAUNCHED();

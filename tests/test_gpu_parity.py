@@ -207,6 +207,56 @@ def test_single_step_and_sums_match_oracle_rows():
     assert s[1] == pytest.approx((phi2 * phi1).sum(), rel=1e-12, abs=1e-9)
 
 
+# K7 has two implementations: the register path and the TMA-staged tile path.
+# GTB_K7_TILE forces one or the other, GTB_K7_STAGES the depth of the shared-memory ring.
+@pytest.mark.parametrize("key,nx,ny,kw,R", [("c2", 37, 23, {}, 8), ("c3", 33, 31, {}, 4),
+                                             ("c2b", 41, 29, {}, 2), ("c4", 48, 21, {"stripe": 6}, 8),
+                                             ("c5", 57, 43, {}, 2), ("c5", 57, 43, {}, 4)])
+@pytest.mark.parametrize("tile,stages", [(0, 0), (1, 1), (1, 2), (1, 3), (1, 5)])
+def test_both_k7_paths_match_oracle_rows(monkeypatch, key, nx, ny, kw, R, tile, stages):
+    monkeypatch.setenv("GTB_K7_TILE", str(tile))
+    monkeypatch.setenv("GTB_K7_STAGES", str(max(stages, 1)))
+    w, inp = _small(key, nx, ny, kw)
+    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
+    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
+    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
+    n = Ho.n
+    phi0 = oracle.random_phase_fill(11, 0, R, n)
+    rows = np.arange(n)
+    phi1 = oracle.kpm_step_rows(Ho, a, b, True, None, phi0, rows)
+    phi2 = oracle.kpm_step_rows(Ho, a, b, False, phi0, phi1, rows)
+    g0 = _dev(phi0)
+    g1 = torch.empty_like(g0)
+    s = gtb.kpm_step(Hg, a, b, True, g0, g1).cpu().numpy()
+    assert np.abs(g1.cpu().numpy() - phi1).max() <= 1e-14
+    assert s[0] == pytest.approx(n * R, rel=1e-14)
+    s = gtb.kpm_step(Hg, a, b, False, g1, g0).cpu().numpy()
+    assert np.abs(g0.cpu().numpy() - phi2).max() <= 1e-14
+    assert s[0] == pytest.approx((phi1 * phi1).sum(), rel=1e-13)
+    assert s[1] == pytest.approx((phi2 * phi1).sum(), rel=1e-12, abs=1e-9)
+    M = 65
+    ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+
+
+@pytest.mark.parametrize("drop", [1, 2, 3])
+def test_atom_count_not_a_multiple_of_four_takes_the_register_path(drop):
+    # bulk copies need 16-byte aligned slot rows (n % 4 == 0); any other n must still be exact
+    w, inp = _small("c2b", 23, 17, {})
+    n = inp.pos.shape[0] - drop
+    args = (inp.box, (0, 0, 0), w.cutoff, w.onsite, w.t0, w.r0, w.beta)
+    shift = inp.onsite_shift[:n]
+    Ho = oracle.build_hamiltonian(inp.pos[:n], inp.species[:n], *args, shift, method=1)
+    Hg = gtb.build_hamiltonian(_dev(inp.pos[:n]), _dev(inp.species[:n]), *args, _dev(shift))
+    assert (Hg.cols.cpu().numpy() == Ho.cols).all()
+    a, b = _scale(Ho)
+    for R in (2, 4, 8):
+        ref = oracle.kpm_moments(Ho, a, b, 48, R, 3, mode=0, algo=0)
+        got = gtb.kpm_moments(Hg, a, b, 48, R, R, 3).cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-12
+
+
 def test_divergence_is_reported():
     w, inp = _small("c5", 20, 20, {})
     Hg = _gpu_H(w, inp, with_diag=False)
