@@ -39,6 +39,8 @@ UNIT = "atom*moment*vector updates/s"
 # `ncu --set full` captures summarised under profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = {
     "c5-pristine-5000x5000": 13.178e9,     # profiles/r01_c5_k7_full.md (10.00 GB read + 3.18 GB written)
+    "c2-disordered-500x500-rc4.0": 0.6125e9,    # profiles/r01_wide_k7_full.md (504.5 MB + 108.0 MB)
+    "c3-disordered-1600x1600-rc4.0": 4.508e9,   # profiles/r01_wide_k7_full.md (3.865 GB + 643.5 MB)
 }
 
 
@@ -266,7 +268,10 @@ def run_ours(args):
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "cheb_step_kernel (K7 fused Chebyshev pass)",
+    k7_name = ("cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
+               if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
+               else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
+    roofline = {"bound": "hbm", "kernel": k7_name,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                 "traffic": NCU_TRAFFIC_BYTES.get(w.name),
