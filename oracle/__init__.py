@@ -194,3 +194,66 @@ def dos(mu, a: float, b: float, energies, kernel: int = 1, scale: float = 1.0) -
                         C.c_void_p(rho.ctypes.data))
     _check(st, "dos")
     return rho
+
+
+# ---------------------------------------------------------------- VAC conductivity (Eq. 3)
+def _p(x: np.ndarray) -> C.c_void_p:
+    return C.c_void_p(x.ctypes.data)
+
+
+def velocity_ell(H: Ell, pos, box, pbc, axis: int = 0) -> np.ndarray:
+    """vvals[k][i] = vals[k][i] * (x_j - x_i)_axis, minimum image (reading V1); V = i * vvals."""
+    pos, box, pbc = _f64(pos), _f64(box), _i32(pbc)
+    out = np.zeros((H.width, H.n))
+    hc = H._c()
+    _check(lib().gtbo_velocity_ell(C.byref(hc), _p(pos), _p(box), _p(pbc), C.c_int32(axis), _p(out)),
+           "velocity_ell")
+    return out
+
+
+def velocity_apply(H: Ell, vvals, x) -> np.ndarray:
+    """y = V x;  x is [n][R][2]."""
+    x, vvals = _f64(x), _f64(vvals)
+    y = np.zeros_like(x)
+    hc = H._c()
+    _check(lib().gtbo_velocity_apply(C.byref(hc), _p(vvals), C.c_int32(x.shape[1]), _p(x), _p(y)),
+           "velocity_apply")
+    return y
+
+
+def evolve(H: Ell, a: float, b: float, dt: float, x, return_terms: bool = False):
+    """y = exp(-i H dt) x (Chebyshev-Bessel expansion, reading V4);  x is [n][R][2]."""
+    x = _f64(x)
+    y = np.zeros_like(x)
+    terms = C.c_int32(0)
+    hc = H._c()
+    _check(lib().gtbo_evolve(C.byref(hc), C.c_double(a), C.c_double(b), C.c_double(dt),
+                             C.c_int32(x.shape[1]), _p(x), _p(y), C.byref(terms)), "evolve")
+    return (y, int(terms.value)) if return_terms else y
+
+
+def vac_moments(H: Ell, vvals, a: float, b: float, M: int, n_steps: int, dt: float, R: int = 1,
+                seed: int = 0, mode: int = 0) -> np.ndarray:
+    """C[j][n] (readings V2, V3)."""
+    vvals = _f64(vvals)
+    out = np.zeros((n_steps, M))
+    hc = H._c()
+    _check(lib().gtbo_vac_moments(C.byref(hc), _p(vvals), C.c_double(a), C.c_double(b), C.c_int32(M),
+                                  C.c_int32(n_steps), C.c_double(dt), C.c_int32(R),
+                                  C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode), _p(out)),
+           "vac_moments")
+    return out
+
+
+def vac_conductivity(Cm, a: float, b: float, energies, dt: float, kernel: int = 1,
+                     scale: float = 1.0):
+    """(rho_vv[j][g], sigma[j][g]) from C[j][n] (readings V5, V6)."""
+    Cm, energies = _f64(Cm), _f64(energies)
+    n_steps, M = Cm.shape
+    G = energies.shape[0]
+    rv, sg = np.zeros((n_steps, G)), np.zeros((n_steps, G))
+    _check(lib().gtbo_vac_conductivity(_p(Cm), C.c_int32(M), C.c_int32(n_steps), C.c_double(a),
+                                       C.c_double(b), C.c_int32(kernel), _p(energies), C.c_int32(G),
+                                       C.c_double(dt), C.c_double(scale), _p(rv), _p(sg)),
+           "vac_conductivity")
+    return rv, sg

@@ -117,6 +117,29 @@ int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
 /* g[n], n = 0..M-1 (exported so the kernel itself can be pinned).           */
 int gtbo_jackson(int32_t M, double* g);
 
+/* --- VAC conductivity (Eq. 3) -- */
+/* Units hbar = 1: times in hbar/eV, velocities in eV*Angstrom.  Readings V1-V6
+ * are listed at the top of gtbo_vac.cpp and in DESIGN.md sec. 11.
+ * V1: vvals[k][i] = vals[k][i]*(x_j - x_i)_axis (minimum image), V = i*vvals. */
+int gtbo_velocity_ell(const gtbo_ell* H, const double* pos, const double box[3],
+                      const int32_t pbc[3], int32_t axis, double* vvals /*[width][n]*/);
+/* y = V x on R interleaved vectors ([n][R][2]). */
+int gtbo_velocity_apply(const gtbo_ell* H, const double* vvals, int32_t R,
+                        const double* x, double* y);
+/* V4: y = exp(-i H dt) x by the Chebyshev-Bessel expansion; *terms = its length. */
+int gtbo_evolve(const gtbo_ell* H, double a, double b, double dt, int32_t R,
+                const double* x, double* y, int32_t* terms);
+/* V2/V3: C[j][n] = (1/(N R)) sum_r Re<U^j phi_r| T_n(H~) V |U^j V phi_r>,
+ * j = 0..n_steps-1, n = 0..M-1.  mode 0 random-phase vectors, 1 all basis vectors. */
+int gtbo_vac_moments(const gtbo_ell* H, const double* vvals, double a, double b,
+                     int32_t M, int32_t n_steps, double dt, int32_t R, uint64_t seed,
+                     int32_t mode, double* C /*[n_steps][M]*/);
+/* V5/V6: rho_vv[j][g] (optional) = reconstruction of C[j][:] as gtbo_dos;
+ * sigma[j][g] = scale * trapezoid integral of rho_vv over tau in [0, j dt]. */
+int gtbo_vac_conductivity(const double* C, int32_t M, int32_t n_steps, double a,
+                          double b, int32_t kernel, const double* energies, int32_t G,
+                          double dt, double scale, double* rho_vv, double* sigma);
+
 #ifdef __cplusplus
 }
 #endif
