@@ -169,6 +169,56 @@ int gtb_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
 /* ASYNC.  g (DEVICE [M]) = Jackson coefficients as above. */
 int gtb_jackson(int32_t M, double* g, void* stream);
 
+/* ---- VAC conductivity (Eq. 3; time step and step count :60, :68) ----
+ * sigma(E, t) = (2 e^2/Omega) int_0^t Tr[delta(E - H) Re(V V(tau))] dtau,  V(tau) = e^{iH tau} V e^{-iH tau}.
+ * The paper prints no formula for V, the propagator or the estimator; readings V1-V6 of
+ * DESIGN.md sec. 11.  Units hbar = 1: times in hbar/eV (0.1 fs = 0.1/0.6582119569), velocities
+ * in eV*Angstrom; the prefactor 2 e^2/(Omega hbar^2) N is the caller's `scale`. */
+
+/* ASYNC.  V1: V = i [H, X_axis]  =>  V_ij = i * vvals_ij,
+ *   vvals[k][i] = vals[k][i] * d,  d = x_j - x_i (axis component), j = cols[k][i];
+ *   periodic axis: d -= L*rint(d/L)   (fp64, no FMA contraction).
+ * pos DEVICE [n][3]; box, pbc HOST; vvals DEVICE [width][n] (same layout as H->vals). */
+int gtb_velocity_ell(const gtb_ell* H, const double* pos, const double box[3],
+                     const int32_t pbc[3], int32_t axis, double* vvals, void* stream);
+
+/* ASYNC.  y = V x = i * (vvals x) on R interleaved vectors; x, y DEVICE [n][R][2], x != y. */
+int gtb_velocity_apply(const gtb_ell* H, const double* vvals, int32_t R, const double* x,
+                       double* y, void* stream);
+
+/* ASYNC.  V4: phi <- exp(-i H dt) phi by the Chebyshev-Bessel expansion
+ *   e^{-i b dt} sum_m (2 - delta_m0) (-i)^m J_m(a dt) T_m(H~),  H~ = (H - b)/a,
+ * truncated after the first m > a*dt with |J_m(a dt)| < 1e-18 (*terms, HOST, may be NULL,
+ * receives the number of terms).  phi DEVICE [n][R][2], 32-byte aligned, updated in place.
+ * Workspace: gtb_evolve_workspace_bytes(n, R). */
+size_t gtb_evolve_workspace_bytes(int64_t n, int32_t R);
+int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32_t R, double* phi,
+               int32_t* terms, void* ws, size_t ws_bytes, void* stream);
+
+/* ASYNC.  V2/V3: VAC Chebyshev moments on the time grid tau_j = j*dt, j = 0..n_steps-1:
+ *   C[j][n] = (1/(N R_total)) sum_r Re < psiL_r(tau_j) | T_n(H~) V | psiR_r(tau_j) >,  n = 0..M-1,
+ *   psiL_r(tau) = U(tau) phi_r,  psiR_r(tau) = U(tau) V phi_r,  U(tau_j) = U(dt)^j,
+ * by chi_0 = V psiR, chi_1 = H~ chi_0, chi_{n+1} = 2 H~ chi_n - chi_{n-1}, C_n = Re<psiL|chi_n>:
+ * M-1 fused passes per time step (the DOS kernel with the dot products taken against psiL).
+ * mode, R_total, R_batch, seed: as gtb_kpm_moments (mode 1: / N).  C is DEVICE [n_steps][M].
+ * Workspace: gtb_vac_workspace_bytes(n, M, n_steps, R_batch); gtb_kpm_status(ws) reports
+ * non-finite results as GTB_ERR_DIVERGED. */
+size_t gtb_vac_workspace_bytes(int64_t n, int32_t M, int32_t n_steps, int32_t R_batch);
+int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, double b, int32_t M,
+                    int32_t n_steps, double dt, int32_t R_total, int32_t R_batch, uint64_t seed,
+                    int32_t mode, double* C, void* ws, size_t ws_bytes, void* stream);
+/* SYNC.  Device time of the M-1 moment passes of the LAST time step of the last
+ * gtb_vac_moments call of this thread (CUDA events on the caller's stream). */
+int gtb_vac_last_loop_ms(double* ms, int32_t* passes);
+
+/* ASYNC.  V5/V6: rho_vv[j][g] = kernel-damped reconstruction of C[j][:] at E_g exactly as
+ * gtb_dos (scale 1); sigma[0][g] = 0, sigma[j][g] = sigma[j-1][g] + scale*dt*(rho_vv[j-1][g] +
+ * rho_vv[j][g])/2 (trapezoid rule).  C, energies, rho_vv, sigma: DEVICE; rho_vv and sigma
+ * are [n_steps][G], both written. */
+int gtb_vac_conductivity(const double* C, int32_t M, int32_t n_steps, double a, double b,
+                         int32_t kernel, const double* energies, int32_t G, double dt,
+                         double scale, double* rho_vv, double* sigma, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

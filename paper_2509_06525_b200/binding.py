@@ -30,7 +30,11 @@ EXPORTS = (
     "gtb_bounds_workspace_bytes", "gtb_spectral_bounds", "gtb_random_phase_fill",
     "gtb_kpm_workspace_bytes", "gtb_kpm_moments", "gtb_kpm_status", "gtb_kpm_step",
     "gtb_kpm_last_loop_ms", "gtb_dos", "gtb_jackson",
+    "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
+    "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
 )
+
+HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
 
 
 class GtbError(RuntimeError):
@@ -74,6 +78,10 @@ def lib() -> C.CDLL:
             getattr(L, name).argtypes = [C.c_int64]
         L.gtb_kpm_workspace_bytes.restype = C.c_size_t
         L.gtb_kpm_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32]
+        L.gtb_evolve_workspace_bytes.restype = C.c_size_t
+        L.gtb_evolve_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+        L.gtb_vac_workspace_bytes.restype = C.c_size_t
+        L.gtb_vac_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         _lib = L
     return _lib
 
@@ -301,3 +309,95 @@ def jackson(M: int, device="cuda") -> torch.Tensor:
     g = torch.empty(M, dtype=torch.float64, device=device)
     _check(lib().gtb_jackson(C.c_int32(M), _ptr(g), _stream()), "jackson")
     return g
+
+
+# ---------------------------------------------------------------- VAC conductivity (Eq. 3)
+def evolve_workspace_bytes(n: int, R: int) -> int:
+    return int(lib().gtb_evolve_workspace_bytes(n, R))
+
+
+def vac_workspace_bytes(n: int, M: int, n_steps: int, R_batch: int) -> int:
+    return int(lib().gtb_vac_workspace_bytes(n, M, n_steps, R_batch))
+
+
+def velocity_ell(H: Ell, pos: torch.Tensor, box, pbc, axis: int = 0) -> torch.Tensor:
+    """vvals [width][n] with V = i * vvals on the pattern of H (reading V1)."""
+    pos = _dev(pos, torch.float64, "pos")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    out = torch.empty_like(H.vals)
+    hc = H._c()
+    st = lib().gtb_velocity_ell(C.byref(hc), _ptr(pos), C.c_void_p(box_h.ctypes.data),
+                                C.c_void_p(pbc_h.ctypes.data), C.c_int32(axis), _ptr(out), _stream())
+    _check(st, "velocity_ell")
+    return out
+
+
+def velocity_apply(H: Ell, vvals: torch.Tensor, x: torch.Tensor) -> torch.Tensor:
+    x = _dev(x, torch.float64, "x")
+    y = torch.empty_like(x)
+    hc = H._c()
+    st = lib().gtb_velocity_apply(C.byref(hc), _ptr(vvals), C.c_int32(x.shape[1]), _ptr(x), _ptr(y),
+                                  _stream())
+    _check(st, "velocity_apply")
+    return y
+
+
+def evolve(H: Ell, a: float, b: float, dt: float, phi: torch.Tensor,
+           ws: Optional[torch.Tensor] = None) -> int:
+    """phi <- exp(-i H dt) phi in place; returns the number of Chebyshev terms used."""
+    phi = _dev(phi, torch.float64, "phi")
+    R = phi.shape[1]
+    if ws is None:
+        ws = workspace(evolve_workspace_bytes(H.n, R), phi.device)
+    terms = C.c_int32(0)
+    hc = H._c()
+    st = lib().gtb_evolve(C.byref(hc), C.c_double(a), C.c_double(b), C.c_double(dt), C.c_int32(R),
+                          _ptr(phi), C.byref(terms), _ptr(ws), C.c_size_t(ws.numel()), _stream())
+    _check(st, "evolve")
+    return int(terms.value)
+
+
+def vac_moments(H: Ell, vvals: torch.Tensor, a: float, b: float, M: int, n_steps: int, dt: float,
+                R_total: int = 1, R_batch: Optional[int] = None, seed: int = 0, mode: int = 0,
+                ws: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
+                check: bool = False) -> torch.Tensor:
+    """C[j][n], j < n_steps, n < M (readings V2, V3)."""
+    dev = H.vals.device
+    if R_batch is None:
+        R_batch = R_total if mode == 0 else 8
+    if out is None:
+        out = torch.empty((n_steps, M), dtype=torch.float64, device=dev)
+    if ws is None:
+        ws = workspace(vac_workspace_bytes(H.n, M, n_steps, R_batch), dev)
+    hc = H._c()
+    st = lib().gtb_vac_moments(C.byref(hc), _ptr(vvals), C.c_double(a), C.c_double(b), C.c_int32(M),
+                               C.c_int32(n_steps), C.c_double(dt), C.c_int32(R_total),
+                               C.c_int32(R_batch), C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode),
+                               _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream())
+    _check(st, "vac_moments")
+    if check:
+        kpm_status(ws)
+    return out
+
+
+def vac_last_loop_ms():
+    ms, passes = C.c_double(0.0), C.c_int32(0)
+    _check(lib().gtb_vac_last_loop_ms(C.byref(ms), C.byref(passes)), "vac_last_loop_ms")
+    return float(ms.value), int(passes.value)
+
+
+def vac_conductivity(Cm: torch.Tensor, a: float, b: float, energies: torch.Tensor, dt: float,
+                     kernel: int = 1, scale: float = 1.0):
+    """(rho_vv[j][g], sigma[j][g]) from C[j][n] (readings V5, V6)."""
+    Cm = _dev(Cm, torch.float64, "C")
+    energies = _dev(energies, torch.float64, "energies")
+    n_steps, M = Cm.shape
+    G = energies.shape[0]
+    rv = torch.empty((n_steps, G), dtype=torch.float64, device=Cm.device)
+    sg = torch.empty_like(rv)
+    st = lib().gtb_vac_conductivity(_ptr(Cm), C.c_int32(M), C.c_int32(n_steps), C.c_double(a),
+                                    C.c_double(b), C.c_int32(kernel), _ptr(energies), C.c_int32(G),
+                                    C.c_double(dt), C.c_double(scale), _ptr(rv), _ptr(sg), _stream())
+    _check(st, "vac_conductivity")
+    return rv, sg

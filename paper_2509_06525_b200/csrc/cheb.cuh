@@ -1,0 +1,52 @@
+// Internal interface of the fused Chebyshev pass (K6/K7/K7t, defined in kpm.cu) for the other
+// translation units of libgtb_kpm.so (vac.cu).  Product code; nothing here is used by oracle/.
+#pragma once
+
+#include "common.cuh"
+
+namespace gtb {
+
+constexpr int kBlock = 256;
+constexpr int kMaxBlocksPerSm = 8;
+constexpr int kMaxGrid = kSmCount * kMaxBlocksPerSm;
+
+struct StepArgs {
+  const int32_t* cols;
+  const double* vals;
+  const double* diag;
+  int64_t n;
+  int32_t width;
+  int32_t T;              // threads per row = R*2/VW
+  const double* phi_cur;  // phi_n           [n][R][2]
+  double* phi_io;         // phi_{n-1} in, phi_{n+1} out
+  double scale;           // 1/a (first pass) or 2/a
+  double b;
+  double2* partial;       // [gridDim.x]: (sum |phi_n|^2, sum Re conj(phi_{n+1}) phi_n), or with
+  const double* dot_with; // dot_with = L:  (sum Re conj(L) phi_n, sum Re conj(L) phi_{n+1})
+};
+
+using StepFn = void (*)(const StepArgs);
+using TileFn = void (*)(const StepArgs, const int);
+
+struct StepPlan {
+  StepFn first = nullptr, next = nullptr;   // register path (K6/K7)
+  TileFn tfirst = nullptr, tnext = nullptr; // TMA-staged path (K7t); used when stages > 0
+  int vw = 0, T = 0;
+  int grid = 0;
+  int stages = 0;
+  size_t smem = 0;
+};
+
+// dot = false: the DOS pass (dot products with phi_n itself); dot = true: with StepArgs::dot_with.
+int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p);
+void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st);
+
+int check_ell(const gtb_ell* H);
+int check_ws(const void* ws, size_t ws_bytes, size_t need);
+// mode 0: random phases of (seed, r0..r0+R-1); mode 1: basis vectors e_{r0}..e_{r0+R-1}
+void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st);
+// sums[s] += sum_{k<grid} partial[s*stride + k]   for s = 0..nslots-1, fixed order
+void launch_reduce_partials(const double2* partial, int stride, int grid, double2* sums, int nslots,
+                            cudaStream_t st);
+
+}  // namespace gtb

@@ -17,14 +17,11 @@
 #include <cmath>
 #include <cstdlib>
 
-#include "common.cuh"
+#include "cheb.cuh"
 
 namespace gtb {
 namespace {
 
-constexpr int kBlock = 256;
-constexpr int kMaxBlocksPerSm = 8;
-constexpr int kMaxGrid = kSmCount * kMaxBlocksPerSm;
 constexpr uint64_t kGamma = 0x9E3779B97F4A7C15ull;
 
 // ---- counter hash (reading C3) ----------------------------------------------------------
@@ -121,24 +118,11 @@ __device__ __forceinline__ void store_stream<4>(double* p, const Vec<4>& x) {
                : "memory");
 }
 
-struct StepArgs {
-  const int32_t* cols;
-  const double* vals;
-  const double* diag;
-  int64_t n;
-  int32_t width;
-  int32_t T;              // threads per row = R*2/VW
-  const double* phi_cur;  // phi_n           [n][R][2]
-  double* phi_io;         // phi_{n-1} in, phi_{n+1} out
-  double scale;           // 1/a (first pass) or 2/a
-  double b;
-  double2* partial;       // [gridDim.x]: (sum |phi_n|^2, sum Re conj(phi_{n+1}) phi_n)
-};
 
 // K6 / K7.  Thread e handles element e of phi viewed as an array of Vec<VW>: row = e / T, vector
 // group t = e % T, so a warp touches one contiguous 32*VW*8-byte span of phi_{n-1}/phi_{n+1}, and
 // every gather of a row's neighbour is T consecutive threads reading R*16 contiguous bytes.
-template <int VW, int LOG2T, bool kFirst, bool kDiag, int CH>
+template <int VW, int LOG2T, bool kFirst, bool kDiag, int CH, bool kDotL>
 __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
   const int64_t n = a.n;
   const int T = LOG2T >= 0 ? (1 << LOG2T) : a.T;
@@ -159,6 +143,8 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
     Vec<VW> prev;
     if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
     const Vec<VW> own = load_gather<VW>(a.phi_cur + e * VW);
+    Vec<VW> with;
+    if (kDotL) with = load_stream<VW>(a.dot_with + e * VW);
     if (CH == 0) {
 #pragma unroll 4
       for (int k = 0; k < width; ++k) {
@@ -200,8 +186,8 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
     for (int q = 0; q < VW; ++q) {
       y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
       if (!kFirst) y.v[q] -= prev.v[q];
-      s1 = fma(own.v[q], own.v[q], s1);
-      s2 = fma(y.v[q], own.v[q], s2);
+      s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+      s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
     }
     store_stream<VW>(a.phi_io + e * VW, y);
   }
@@ -268,7 +254,7 @@ __host__ __device__ inline uint32_t tile_stage_bytes(int width, int TR, bool dia
   return (uint32_t)((width * TR * 12 + (diag ? TR * 8 : 0) + 127) / 128 * 128);
 }
 
-template <int LOG2T, bool kFirst, bool kDiag, int CH>
+template <int LOG2T, bool kFirst, bool kDiag, int CH, bool kDotL>
 __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
@@ -301,7 +287,7 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
     const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
     if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
     __syncwarp();
-    for (int j = lane; j < 2 * width + 3; j += 32) {
+    for (int j = lane; j < 2 * width + 4; j += 32) {
       if (j < width) {
         bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
       } else if (j < 2 * width) {
@@ -311,8 +297,10 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
         if (kDiag) bulk_g2s(base + diag_off, a.diag + row0, rows * 8, bar);
       } else if (j == 2 * width + 1) {
         bulk_prefetch_l2(a.phi_cur + row0 * (T * VW), rows * (T * VW * 8));
-      } else {
+      } else if (j == 2 * width + 2) {
         if (!kFirst) bulk_prefetch_l2(a.phi_io + row0 * (T * VW), rows * (T * VW * 8));
+      } else {
+        if (kDotL) bulk_prefetch_l2(a.dot_with + row0 * (T * VW), rows * (T * VW * 8));
       }
     }
   };
@@ -328,9 +316,9 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
     const int64_t row = (blockIdx.x + i * gridDim.x) * TR + rl;
     const bool live = row < n;
     const int64_t e = row * T + t;
-    Vec<VW> prev, own, acc;
+    Vec<VW> prev, own, acc, with;
 #pragma unroll
-    for (int q = 0; q < VW; ++q) acc.v[q] = prev.v[q] = own.v[q] = 0.0;
+    for (int q = 0; q < VW; ++q) acc.v[q] = prev.v[q] = own.v[q] = with.v[q] = 0.0;
     if (live) {
       if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
       own = load_gather<VW>(a.phi_cur + e * VW);
@@ -366,13 +354,14 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
     __syncthreads();  // every thread has read stage s: hand it back to the producer
     if (wid == 0 && i + nstages < my_tiles) issue(i + nstages);
     if (live) {
+      if (kDotL) with = load_stream<VW>(a.dot_with + e * VW);  // prefetched into L2 by the producer
       Vec<VW> y;
 #pragma unroll
       for (int q = 0; q < VW; ++q) {
         y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
         if (!kFirst) y.v[q] -= prev.v[q];
-        s1 = fma(own.v[q], own.v[q], s1);
-        s2 = fma(y.v[q], own.v[q], s2);
+        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
       }
       store_stream<VW>(a.phi_io + e * VW, y);
     }
@@ -447,45 +436,39 @@ __global__ void copy_sums_kernel(const double2* sums, double* out2) {
 }
 
 // ---- host side ---------------------------------------------------------------------------
-using StepFn = void (*)(const StepArgs);
-using TileFn = void (*)(const StepArgs, const int);
-
-struct StepPlan {
-  StepFn first = nullptr, next = nullptr;   // register path (K6/K7)
-  TileFn tfirst = nullptr, tnext = nullptr; // TMA-staged path (K7t); used when stages > 0
-  int vw = 0, T = 0;
-  int grid = 0;
-  int stages = 0;
-  size_t smem = 0;
-};
-
-template <int VW, int LOG2T, int CH>
+template <int VW, int LOG2T, int CH, bool DOT>
 void pick_ch(bool diag, StepPlan* p) {
-  p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true, CH> : cheb_step_kernel<VW, LOG2T, true, false, CH>;
-  p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true, CH> : cheb_step_kernel<VW, LOG2T, false, false, CH>;
+  p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true, CH, DOT> : cheb_step_kernel<VW, LOG2T, true, false, CH, DOT>;
+  p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true, CH, DOT> : cheb_step_kernel<VW, LOG2T, false, false, CH, DOT>;
 }
 
 template <int VW, int LOG2T>
-void pick(bool diag, int ch, StepPlan* p) {
-  if (ch == 0) pick_ch<VW, LOG2T, 0>(diag, p);
-  else pick_ch<VW, LOG2T, 8>(diag, p);
+void pick(bool diag, int ch, bool dot, StepPlan* p) {
+  if (ch == 0) { if (dot) pick_ch<VW, LOG2T, 0, true>(diag, p); else pick_ch<VW, LOG2T, 0, false>(diag, p); }
+  else { if (dot) pick_ch<VW, LOG2T, 8, true>(diag, p); else pick_ch<VW, LOG2T, 8, false>(diag, p); }
 }
 
-template <int LOG2T, int CH>
+template <int LOG2T, int CH, bool DOT>
 void pick_tile_ch(bool diag, StepPlan* p) {
-  p->tfirst = diag ? cheb_tile_kernel<LOG2T, true, true, CH> : cheb_tile_kernel<LOG2T, true, false, CH>;
-  p->tnext = diag ? cheb_tile_kernel<LOG2T, false, true, CH> : cheb_tile_kernel<LOG2T, false, false, CH>;
+  p->tfirst = diag ? cheb_tile_kernel<LOG2T, true, true, CH, DOT> : cheb_tile_kernel<LOG2T, true, false, CH, DOT>;
+  p->tnext = diag ? cheb_tile_kernel<LOG2T, false, true, CH, DOT> : cheb_tile_kernel<LOG2T, false, false, CH, DOT>;
+}
+
+template <int LOG2T, bool DOT>
+void pick_tile_dot(bool diag, int ch, StepPlan* p) {
+  switch (ch) {
+    case 3: pick_tile_ch<LOG2T, 3, DOT>(diag, p); break;
+    case 4: pick_tile_ch<LOG2T, 4, DOT>(diag, p); break;
+    case 6: pick_tile_ch<LOG2T, 6, DOT>(diag, p); break;
+    case 8: pick_tile_ch<LOG2T, 8, DOT>(diag, p); break;
+    default: pick_tile_ch<LOG2T, 10, DOT>(diag, p); break;
+  }
 }
 
 template <int LOG2T>
-void pick_tile(bool diag, int ch, StepPlan* p) {
-  switch (ch) {
-    case 3: pick_tile_ch<LOG2T, 3>(diag, p); break;
-    case 4: pick_tile_ch<LOG2T, 4>(diag, p); break;
-    case 6: pick_tile_ch<LOG2T, 6>(diag, p); break;
-    case 8: pick_tile_ch<LOG2T, 8>(diag, p); break;
-    default: pick_tile_ch<LOG2T, 10>(diag, p); break;
-  }
+void pick_tile(bool diag, int ch, bool dot, StepPlan* p) {
+  if (dot) pick_tile_dot<LOG2T, true>(diag, ch, p);
+  else pick_tile_dot<LOG2T, false>(diag, ch, p);
 }
 
 // gathers kept in flight per thread: the chunk that pads `width` least (ties: the larger)
@@ -505,17 +488,19 @@ int env_int(const char* name, int dflt) {
   return e ? atoi(e) : dflt;
 }
 
-int make_plan(const gtb_ell* H, int R, StepPlan* p) {
+}  // namespace
+
+int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   const int64_t n = H->n;
   const int width = H->width;
   const bool diag = H->diag != nullptr;
   const int ch = width <= 4 ? 0 : 8;
   int log2t = -1;
-  if (R == 2) { pick<4, 0>(diag, ch, p); p->vw = 4; p->T = 1; log2t = 0; }
-  else if (R == 4) { pick<4, 1>(diag, ch, p); p->vw = 4; p->T = 2; log2t = 1; }
-  else if (R == 8) { pick<4, 2>(diag, ch, p); p->vw = 4; p->T = 4; log2t = 2; }
-  else if (R == 1) { pick<2, 0>(diag, ch, p); p->vw = 2; p->T = 1; }
-  else { pick<2, -1>(diag, ch, p); p->vw = 2; p->T = R; }
+  if (R == 2) { pick<4, 0>(diag, ch, dot, p); p->vw = 4; p->T = 1; log2t = 0; }
+  else if (R == 4) { pick<4, 1>(diag, ch, dot, p); p->vw = 4; p->T = 2; log2t = 1; }
+  else if (R == 8) { pick<4, 2>(diag, ch, dot, p); p->vw = 4; p->T = 4; log2t = 2; }
+  else if (R == 1) { pick<2, 0>(diag, ch, dot, p); p->vw = 2; p->T = 1; }
+  else { pick<2, -1>(diag, ch, dot, p); p->vw = 2; p->T = R; }
   int dev = 0, sms = kSmCount, per_sm = 0;
   GTB_CUDA_TRY(cudaGetDevice(&dev));
   GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -529,9 +514,9 @@ int make_plan(const gtb_ell* H, int R, StepPlan* p) {
   p->stages = 0;
   if (stages > 0) {
     const int tch = tile_chunk(width);
-    if (log2t == 0) pick_tile<0>(diag, tch, p);
-    else if (log2t == 1) pick_tile<1>(diag, tch, p);
-    else pick_tile<2>(diag, tch, p);
+    if (log2t == 0) pick_tile<0>(diag, tch, dot, p);
+    else if (log2t == 1) pick_tile<1>(diag, tch, dot, p);
+    else pick_tile<2>(diag, tch, dot, p);
     const int TR = kBlock / p->T;
     const size_t stage_bytes = tile_stage_bytes(width, TR, diag);
     int max_smem = 0;
@@ -567,6 +552,33 @@ void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t
     (first ? p.first : p.next)<<<p.grid, kBlock, 0, st>>>(sa);
 }
 
+void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st) {
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n * R + kBlock - 1) / kBlock, kMaxGrid));
+  if (mode == 0)
+    random_phase_kernel<<<grid, kBlock, 0, st>>>(seed, (int32_t)r0, R, n, reinterpret_cast<double2*>(phi));
+  else
+    basis_fill_kernel<<<grid, kBlock, 0, st>>>(r0, R, n, reinterpret_cast<double2*>(phi));
+}
+
+void launch_reduce_partials(const double2* partial, int stride, int grid, double2* sums, int nslots,
+                            cudaStream_t st) {
+  reduce_partials_kernel<<<nslots, 128, 0, st>>>(partial, stride, grid, sums);
+}
+
+int check_ell(const gtb_ell* H) {
+  if (!H || H->n <= 0 || H->width < 0 || (H->width > 0 && (!H->cols || !H->vals)))
+    return GTB_ERR_INVALID_ARG;
+  if (H->n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
+  return GTB_OK;
+}
+
+int check_ws(const void* ws, size_t ws_bytes, size_t need) {
+  if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u) || ws_bytes < need) return GTB_ERR_WORKSPACE;
+  return GTB_OK;
+}
+
+namespace {
+
 struct KpmWs {
   double* phi_a;
   double* phi_b;
@@ -587,18 +599,6 @@ KpmWs carve_kpm(void* ws, int64_t n, int32_t M, int32_t R) {
   w.sums = c.take<double2>(S);
   w.bytes = c.off;
   return w;
-}
-
-int check_ell(const gtb_ell* H) {
-  if (!H || H->n <= 0 || H->width < 0 || (H->width > 0 && (!H->cols || !H->vals)))
-    return GTB_ERR_INVALID_ARG;
-  if (H->n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
-  return GTB_OK;
-}
-
-int check_ws(const void* ws, size_t ws_bytes, size_t need) {
-  if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u) || ws_bytes < need) return GTB_ERR_WORKSPACE;
-  return GTB_OK;
 }
 
 int fill_grid(int64_t total) {
@@ -659,7 +659,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    rc = make_plan(H, R, &plan);
+    rc = make_plan(H, R, false, &plan);
     if (rc != GTB_OK) return rc;
     double* cur = w.phi_a;   // phi_k
     double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
@@ -721,7 +721,7 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const KpmWs w = carve_kpm(ws, H->n, 2, R);
   StepPlan plan;
-  rc = make_plan(H, R, &plan);
+  rc = make_plan(H, R, false, &plan);
   if (rc != GTB_OK) return rc;
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
   StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width, plan.T, phi_cur, phi_io,
