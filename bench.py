@@ -34,6 +34,7 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
+VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in hbar/eV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
 # `ncu --set full` captures summarised under profiles/ (None until a capture exists).
@@ -123,6 +124,29 @@ def _oracle_step(w, inp, energies_of):
     return time.perf_counter() - t0, rho
 
 
+def _oracle_vac_step(w, inp, n_steps, dt):
+    import oracle
+    t0 = time.perf_counter()
+    H = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0,
+                                 w.r0, w.beta, inp.onsite_shift, method=1, with_diag=w.use_diag)
+    if w.a is None:
+        lo, hi = oracle.spectral_bounds(H)
+        a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    else:
+        a, b = w.a, w.b
+    vv = oracle.velocity_ell(H, inp.pos, inp.box, inp.pbc, 0)
+    Cm = oracle.vac_moments(H, vv, a, b, w.M, n_steps, dt, R=w.R, seed=w.seed, mode=0)
+    _, sigma = oracle.vac_conductivity(Cm, a, b, W.energy_grid(w, a, b), dt)
+    return time.perf_counter() - t0, sigma
+
+
+def _cpu_sample_vac(w: W.Workload, n_steps: int):
+    """Bounded VAC sample for the oracle: <= 40 000 atoms, M and the step count cut so that one
+    run is roughly 10-30 s (the oracle's VAC loop is serial over vectors)."""
+    nx, ny = min(w.nx, 100), min(w.ny, 100)
+    return w.scaled(nx, ny, M=min(w.M, 64)), min(n_steps, 4)
+
+
 def _cpu_sample(w: W.Workload) -> W.Workload:
     """Bounded sample of the workload for the oracle: same construction, 10^6 atoms at most,
     moments cut so that one pass is roughly 10-30 s of CPU work."""
@@ -147,18 +171,24 @@ def run_reference(args):
     if rank != 0:
         return
     w = _workload(args)
-    s = _cpu_sample(w)
-    inp = W.make_inputs(s)
-    for _ in range(args.warmup):
-        pass   # the oracle has no warm-up state; the sample is sized so K steps fit in minutes
-    times = [_oracle_step(s, inp, W.energy_grid)[0] for _ in range(args.steps)]
-    t = float(np.mean(times))
-    value = s.n_atoms * s.M * s.R / t
-    sample = f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos"
+    if args.quantity == "vac":
+        s, ns = _cpu_sample_vac(w, args.time_steps)
+        inp = W.make_inputs(s)
+        times = [_oracle_vac_step(s, inp, ns, VAC_DT)[0] for _ in range(args.steps)]
+        t = float(np.mean(times))
+        value = s.n_atoms * s.M * s.R * ns / t
+        sample = f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, time steps={ns}, build+velocity+vac_moments+conductivity"
+    else:
+        s = _cpu_sample(w)
+        inp = W.make_inputs(s)
+        times = [_oracle_step(s, inp, W.energy_grid)[0] for _ in range(args.steps)]
+        t = float(np.mean(times))
+        value = s.n_atoms * s.M * s.R / t
+        sample = f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": w.name, "sample": sample},
+            "data": "synthetic", "config": {"workload": w.name, "quantity": args.quantity, "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": _cores(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -304,6 +334,133 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_vac(args):
+    """Same contract as run_ours for the VAC conductivity (Eq. 3): a step = build_hamiltonian ->
+    velocity_ell -> vac_moments (n_steps time points, M moments each: M-1 fused passes per point
+    plus two Chebyshev-Bessel propagations) -> vac_conductivity.  units = N*M*R*n_steps."""
+    import torch
+    import torch.distributed as dist
+    from paper_2509_06525_b200 import binding as gtb
+    from paper_2509_06525_b200 import replicas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    gtb.lib()
+    w = _workload(args)
+    T = args.time_steps
+    inp = W.make_inputs(w)
+    n = w.n_atoms
+    seed = replicas.replica_seed(w.seed, rank)
+    h_pos = torch.from_numpy(inp.pos).pin_memory()
+    h_spec = torch.from_numpy(inp.species).pin_memory()
+    h_shift = torch.from_numpy(inp.onsite_shift).pin_memory() if inp.onsite_shift is not None else None
+    d_pos, d_spec = h_pos.to(dev), h_spec.to(dev)
+    d_shift = h_shift.to(dev) if h_shift is not None else None
+    h2d = h_pos.numel() * 8 + h_spec.numel() * 4 + (h_shift.numel() * 8 if h_shift is not None else 0)
+    ws_build = gtb.workspace(gtb.build_workspace_bytes(n), dev)
+    ws_vac = gtb.workspace(gtb.vac_workspace_bytes(n, w.M, T, w.R), dev)
+    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n), dev)
+    Cm = torch.empty((T, w.M), dtype=torch.float64, device=dev)
+    h_sigma = torch.empty((T, w.n_energies), dtype=torch.float64).pin_memory()
+    state = {}
+
+    def step(pos, spec, shift):
+        H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
+                                  w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
+        if w.a is None:
+            lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
+            a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+        else:
+            a, b = w.a, w.b
+        vv = gtb.velocity_ell(H, pos, inp.box, inp.pbc, 0)
+        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, ws=ws_vac, out=Cm)
+        if "E" not in state:
+            state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
+        _, sigma = gtb.vac_conductivity(Cm, a, b, state["E"], VAC_DT)
+        state["H"] = H
+        return sigma
+
+    def timed(fn, steps):
+        replicas.barrier(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = gtb.launch_count()
+        loop_ms, loop_passes = 0.0, 0
+        e0.record()
+        for _ in range(steps):
+            fn()
+            ms, passes = gtb.vac_last_loop_ms()
+            loop_ms += ms
+            loop_passes += passes
+        e1.record()
+        replicas.barrier(dev)
+        return replicas.max_over_ranks(e0.elapsed_time(e1), dev), gtb.launch_count() - l0, loop_ms, loop_passes
+
+    def device_step():
+        step(d_pos, d_spec, d_shift)
+
+    def e2e_step():
+        pos = h_pos.to(dev, non_blocking=True)
+        spec = h_spec.to(dev, non_blocking=True)
+        shift = h_shift.to(dev, non_blocking=True) if h_shift is not None else None
+        h_sigma.copy_(step(pos, spec, shift), non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    for _ in range(args.warmup):
+        device_step()
+    with ClockSampler(local) as clk:
+        ms, launches, loop_ms, loop_passes = timed(device_step, args.steps)
+    H = state["H"]
+    e2e_step()
+    ms_e2e, _, _, _ = timed(e2e_step, args.steps)
+    units = float(n) * w.M * w.R * T * args.steps
+    per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R) + 16 * w.R
+    bytes_per_launch = float(n) * per_atom
+    k_ms = loop_ms / max(loop_passes, 1)
+    peak, peak_src = _peaks()
+    achieved = bytes_per_launch / (k_ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": replicas.whole_job_value(units, ms), "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (complex128 vectors)", "data": "synthetic",
+            "config": {"workload": w.name, "quantity": "vac (Eq. 3)", "atoms": n, "ell_width": H.width,
+                       "moments": w.M, "vectors": w.R, "time_steps": T, "dt_fs": 0.1,
+                       "energies": w.n_energies, "passes_per_step": T * (w.M - 1),
+                       "l2": "inputs larger than L2 (working set %.1f GB)" % (
+                           (4 * n * w.R * 16 + 1.67 * H.nbytes()) / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "seconds_per_conductivity": ms / args.steps * 1e-3,
+            "e2e": {"value": replicas.whole_job_value(units, ms_e2e), "unit": UNIT,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": h_sigma.numel() * 8,
+                    "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "kernel": "fused Chebyshev pass, dot products against the evolved bra "
+                                                   "(cheb_tile_kernel / cheb_step_kernel, kDotL variant)",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "peak_source": peak_src, "traffic": None,
+                         "algorithmic_bytes_per_launch": bytes_per_launch,
+                         "bytes_per_atom_pass": per_atom, "ms_per_launch": k_ms,
+                         "launches_timed": loop_passes,
+                         "share_of_step": k_ms * T * (w.M - 1) * args.steps / ms},
+            "clocks": clk.summary()}
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            s, ns = _cpu_sample_vac(w, T)
+            t, _ = _oracle_vac_step(s, W.make_inputs(s), ns, VAC_DT)
+            line["cpu_baseline"] = {
+                "value": s.n_atoms * s.M * s.R * ns / t, "unit": UNIT, "cores": _cores(), "kind": "oracle",
+                "sample": f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, time steps={ns}, {t:.1f} s"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     p = argparse.ArgumentParser()
     p.add_argument("--gpus", type=int, default=1)
@@ -315,9 +472,16 @@ def main():
     p.add_argument("--ny", type=int, default=0)
     p.add_argument("--moments", type=int, default=0, help="override M (debugging)")
     p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--quantity", default="dos", choices=["dos", "vac"],
+                   help="dos: the headline path (Eq. 4); vac: the VAC conductivity (Eq. 3, NEXT-1)")
+    p.add_argument("--time-steps", type=int, default=24, help="vac: points of the time grid (dt = 0.1 fs)")
     args = p.parse_args()
+    if args.quantity == "vac" and not args.moments:
+        args.moments = 512
     if args.impl == "reference":
         run_reference(args)
+    elif args.quantity == "vac":
+        run_vac(args)
     else:
         run_ours(args)
 
