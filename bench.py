@@ -45,6 +45,13 @@ NCU_TRAFFIC_BYTES = {
 }
 
 
+# the same for the bra-dot pass of the VAC path (profiles/r01_vac_c2.md)
+NCU_TRAFFIC_VAC_BYTES = {
+    "c2-disordered-500x500-rc4.0": 0.7451e9,    # 632.9 MB read + 112.2 MB written
+    "c5-pristine-5000x5000": 16.383e9,          # 13.20 GB read + 3.18 GB written
+}
+
+
 def _peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -141,9 +148,9 @@ def _oracle_vac_step(w, inp, n_steps, dt):
 
 
 def _cpu_sample_vac(w: W.Workload, n_steps: int):
-    """Bounded VAC sample for the oracle: <= 40 000 atoms, M and the step count cut so that one
+    """Bounded VAC sample for the oracle: <= 160 000 atoms, M and the step count cut so that one
     run is roughly 10-30 s (the oracle's VAC loop is serial over vectors)."""
-    nx, ny = min(w.nx, 100), min(w.ny, 100)
+    nx, ny = min(w.nx, 200), min(w.ny, 200)
     return w.scaled(nx, ny, M=min(w.M, 64)), min(n_steps, 4)
 
 
@@ -443,7 +450,7 @@ def run_vac(args):
             "roofline": {"bound": "hbm", "kernel": "fused Chebyshev pass, dot products against the evolved bra "
                                                    "(cheb_tile_kernel / cheb_step_kernel, kDotL variant)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "peak_source": peak_src, "traffic": None,
+                         "peak_source": peak_src, "traffic": NCU_TRAFFIC_VAC_BYTES.get(w.name),
                          "algorithmic_bytes_per_launch": bytes_per_launch,
                          "bytes_per_atom_pass": per_atom, "ms_per_launch": k_ms,
                          "launches_timed": loop_passes,
