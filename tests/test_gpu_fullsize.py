@@ -162,3 +162,38 @@ def test_c5_hundred_million_atoms_full_size():
         exact = sum(c * tr[k] for k, c in enumerate(coef) if c != 0.0)
         assert abs(mu[n_] - exact) <= bound, (n_, mu[n_], exact)
     assert np.abs(mu[1::2]).max() <= bound
+
+
+# ------------------------------------------------------------------ VAC path (Eq. 3) at full size
+def test_c2_vac_moments_full_size_against_oracle():
+    """10^6 atoms, K = 20, R = 8 (the launch configuration `bench.py --quantity vac` times): velocity
+    values in full, and a short moment run (M = 12, 2 time points) against the oracle's."""
+    w, Ho, Hg = _build_both("c2")
+    inp = W.make_inputs(w)
+    a, b = _scale(w, Ho)
+    vo = oracle.velocity_ell(Ho, inp.pos, inp.box, inp.pbc, 0)
+    vg = gtb.velocity_ell(Hg, _dev(inp.pos), inp.box, inp.pbc, 0)
+    assert np.abs(vg.cpu().numpy() - vo).max() <= ULP4 * np.abs(vo).max()
+    dt = 0.1 / gtb.HBAR_EV_FS
+    M, T = 12, 2
+    ref = oracle.vac_moments(Ho, vo, a, b, M, T, dt, R=w.R, seed=w.seed, mode=0)
+    got = gtb.vac_moments(Hg, vg, a, b, M, T, dt, w.R, w.R, w.seed, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-9 * ref[0, 0]
+    assert np.abs(got - ref).max() <= 1e-11 * ref[0, 0]
+
+
+def test_c5_vac_properties_at_hundred_million_atoms():
+    """Properties that hold at any size for pristine nearest-neighbour graphene: C_0(0) =
+    Tr V^2 / N = 1.5 t^2 a_cc^2 (pin P17) within the stochastic bound, odd moments ~ 0, and the
+    autocorrelation decays from tau = 0."""
+    w, Ho, Hg = _build_both("c5")
+    inp = W.make_inputs(w)
+    vg = gtb.velocity_ell(Hg, _dev(inp.pos), inp.box, inp.pbc, 0)
+    dt = 0.1 / gtb.HBAR_EV_FS
+    M, T = 6, 3
+    C = gtb.vac_moments(Hg, vg, w.a, w.b, M, T, dt, w.R, w.R, w.seed, check=True).cpu().numpy()
+    c00 = 1.5 * 2.7**2 * 1.42**2
+    bound = 6.0 * c00 / np.sqrt(float(Hg.n) * w.R)
+    assert abs(C[0, 0] - c00) <= bound
+    assert np.abs(C[:, 1::2]).max() <= bound
+    assert C[2, 0] < C[1, 0] < C[0, 0]
