@@ -384,6 +384,232 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
   }
 }
 
+// ---- K7s: two Chebyshev steps per HBM sweep (temporal blocking through L2) -----------------------
+// One pass of K7 moves 12K + 48R bytes per atom through HBM for one step.  Here one launch advances
+// every row by TWO steps: rows are cut into chunks of `chunk_rows`; task (j, l) = step l (0 or 1)
+// on chunk j, one WARP per task; tasks are ordered by the key j + skew*l and dealt round-robin to
+// the resident warps, so step 1 of a chunk runs shortly after step 0 of the chunks around it, while
+// their phi_{n+1} (just written), phi_n and H rows are still in the 126 MB L2.  HBM then sees
+// 12K + 32R read + 32R written per atom for two steps instead of 2*(12K + 48R)  (ncu: 17.2 GB
+// instead of 26.4 GB per two steps at config 5).
+// Dependencies: step 1 on chunk j gathers phi_{n+1} from the rows within `halo` (the largest ring
+// distance |col - row| of H) of its own, and overwrites the phi_n rows that step 0 of those rows
+// gathers; so it waits until step 0 has finished on every 1024-row group that overlaps that range
+// (group counters: release increments, acquire polls).  The task order is a topological order of
+// that relation (skew > halo in chunks; the first chunks, whose left neighbours wrap around the
+// ring, run step 1 last), step-0 tasks never wait, every warp works through its tasks in increasing
+// order and all warps are resident (grid = SMs x occupancy): no deadlock.  A spin limit turns any
+// violation into an error flag instead of a hang.  Step 1 reads phi_{n+1} with plain loads, not .nc.
+constexpr int kGroupRows = 1024;
+
+struct SweepArgs {
+  StepArgs s;            // phi_cur = phi_n, phi_io = phi_{n-1}: roles swap for step 1
+  int32_t chunk_rows;    // divides kGroupRows, multiple of 32
+  int32_t n_chunks;
+  const int32_t* halo_rows;  // device: largest ring distance |col - row| of H
+  int32_t slack;         // skew = halo chunks + 1 + slack
+  int32_t* group_done;   // [ceil(n / kGroupRows)], zeroed before the launch: step-0 chunks finished
+  int32_t* error;        // set to 2 when a wait exceeds the spin limit
+  double2* partial0;     // [n_chunks] warp sums of step 0
+  double2* partial1;     // [n_chunks] warp sums of step 1
+};
+
+__device__ __forceinline__ int32_t ld_acquire(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.global.acquire.gpu.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ Vec<4> load_coherent(const double* p) {
+  Vec<4> r;
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3])
+               : "l"(p)
+               : "memory");
+  return r;
+}
+
+// rows [row0, row1) of one step by one warp; kCoherent: phi_n was written earlier in this launch
+template <int LOG2T, bool kDiag, bool kCoherent>
+__device__ __forceinline__ void sweep_rows(const StepArgs& a, const double* __restrict__ cur,
+                                           double* __restrict__ io, int64_t row0, int64_t row1,
+                                           int lane, double& s1, double& s2) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  const int64_t n = a.n;
+  const int width = a.width;
+  const double scale = a.scale, b = a.b;
+  const int64_t e_end = row1 * T;
+  for (int64_t e = row0 * T + lane; e < e_end; e += 32) {
+    const int64_t row = e >> LOG2T;
+    const int64_t t = e - row * T;
+    const double* xt = cur + t * VW;
+    const int32_t* cp = a.cols + row;
+    const double* vp = a.vals + row;
+    const Vec<VW> prev = load_stream<VW>(io + e * VW);
+    const Vec<VW> own = kCoherent ? load_coherent(cur + e * VW) : load_gather<VW>(cur + e * VW);
+    Vec<VW> acc;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) acc.v[q] = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < width; ++k) {
+      const int64_t c = __ldg(cp + (size_t)k * n);
+      const double v = __ldg(vp + (size_t)k * n);
+      const Vec<VW> x = kCoherent ? load_coherent(xt + c * T * VW) : load_gather<VW>(xt + c * T * VW);
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = fma(v, x.v[q], acc.v[q]);
+    }
+    if (kDiag) {
+      const double d = __ldg(a.diag + row);
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = fma(d, own.v[q], acc.v[q]);
+    }
+    Vec<VW> y;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) {
+      y.v[q] = (acc.v[q] - b * own.v[q]) * scale - prev.v[q];
+      s1 = fma(own.v[q], own.v[q], s1);
+      s2 = fma(y.v[q], own.v[q], s2);
+    }
+    store_stream<VW>(io + e * VW, y);
+  }
+}
+
+constexpr int kSpinLimit = 1 << 21;  // x 200 ns: ~0.4 s
+
+template <int LOG2T, bool kDiag>
+__global__ void __launch_bounds__(kBlock, 4) cheb_sweep_kernel(const SweepArgs a) {
+  const int64_t n = a.s.n;
+  const int nc = a.n_chunks, cr = a.chunk_rows;
+  const int lane = threadIdx.x & 31;
+  const int64_t halo = *a.halo_rows;
+  const int ng = (int)((n + kGroupRows - 1) / kGroupRows);
+  const int h = (int)min((int64_t)nc, (halo + cr - 1) / cr);   // halo in chunks
+  const bool whole_ring = 2 * (halo + cr) + kGroupRows >= n;   // the wait range covers the ring
+  const int seam = whole_ring ? nc : h;                        // chunks whose step 1 runs last
+  const int skew = h + 1 + a.slack;
+  // task list: keys t = 0 .. nc-1+skew, two slots per key: (j = t, l = 0) and (j = t - skew, l = 1)
+  // for j >= seam; then (j, 1) for j = 0 .. seam-1.
+  const int64_t main_slots = 2 * ((int64_t)nc + skew);
+  const int64_t total = main_slots + seam;
+  // an odd number of workers, so that a warp alternates between step-0 and step-1 slots (with an
+  // even stride half of the warps would only ever see step-1 slots and wait on the other half)
+  const int64_t W = ((int64_t)gridDim.x * (kBlock / 32) - 1) | 1;
+  bool abort = false;
+  const int64_t me = (int64_t)blockIdx.x * (kBlock / 32) + (threadIdx.x >> 5);
+  for (int64_t task = me; task < total && !abort && me < W; task += W) {
+    int j, l;
+    if (task < main_slots) {
+      l = (int)(task & 1);
+      j = (int)(task >> 1) - (l ? skew : 0);
+      if (j < (l ? seam : 0) || j >= nc) continue;
+    } else {
+      l = 1;
+      j = (int)(task - main_slots);
+    }
+    const int64_t row0 = (int64_t)j * cr, row1 = min(n, row0 + cr);
+    if (l == 1) {  // wait for step 0 on every group overlapping [row0 - halo, row1 + halo) (ring)
+      int g0 = 0, cnt = ng;
+      if (!whole_ring) {
+        const int64_t lo = row0 - halo, hi = row1 + halo - 1;   // may leave [0, n): wraps
+        g0 = (int)((lo + n) % n / kGroupRows);
+        const int g1 = (int)(hi % n / kGroupRows);
+        cnt = g1 >= g0 && hi - lo < n - kGroupRows ? g1 - g0 + 1 : g1 + ng - g0 + 1;
+        if (cnt > ng) cnt = ng;
+      }
+      int spins = 0;
+      for (;;) {
+        bool ok = true;
+        for (int q = lane; q < cnt; q += 32) {
+          int g = g0 + q;
+          if (g >= ng) g -= ng;
+          const int64_t grows = min((int64_t)kGroupRows, n - (int64_t)g * kGroupRows);
+          if (ld_acquire(a.group_done + g) < (int)((grows + cr - 1) / cr)) ok = false;
+        }
+        if (__all_sync(0xffffffffu, ok)) break;
+        __nanosleep(200);
+        if (++spins > kSpinLimit || ld_acquire(a.error) != 0) {
+          if (lane == 0) atomicExch(a.error, 2);
+          abort = true;
+          break;
+        }
+      }
+      if (abort) break;
+    }
+    double s1 = 0.0, s2 = 0.0;
+    if (l == 0)
+      sweep_rows<LOG2T, kDiag, false>(a.s, a.s.phi_cur, a.s.phi_io, row0, row1, lane, s1, s2);
+    else
+      sweep_rows<LOG2T, kDiag, true>(a.s, a.s.phi_io, const_cast<double*>(a.s.phi_cur), row0, row1,
+                                     lane, s1, s2);
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    __syncwarp();  // orders the lanes' phi stores before lane 0's fence below
+    if (lane == 0) {
+      (l ? a.partial1 : a.partial0)[j] = make_double2(s1, s2);
+      if (l == 0) {
+        __threadfence();  // cumulative: the warp's stores are visible device-wide before the count
+        atomicAdd(a.group_done + row0 / kGroupRows, 1);
+      }
+    }
+  }
+}
+
+// largest ring distance min(|c - i|, n - |c - i|) over the entries of H -> *out (zeroed before)
+__global__ void __launch_bounds__(kBlock) halo_kernel(const int32_t* __restrict__ cols, int64_t n,
+                                                      int32_t width, int32_t* out) {
+  const int64_t total = n * width;
+  int m = 0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t i = e % n;
+    int64_t d = (int64_t)cols[e] - i;
+    d = d < 0 ? -d : d;
+    d = min(d, n - d);
+    m = max(m, (int)d);
+  }
+  m = warp_max_i(m);
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
+// K8s: the chunk sums of one sweep -> sums[0], sums[1], fixed order, two stages
+constexpr int kSegs = 64;
+__global__ void __launch_bounds__(kBlock) reduce_chunks_kernel(const double2* __restrict__ p0,
+                                                               const double2* __restrict__ p1,
+                                                               int n_chunks, double2* tmp) {
+  const double2* p = blockIdx.y ? p1 : p0;
+  const int per = (n_chunks + kSegs - 1) / kSegs;
+  const int beg = blockIdx.x * per, end = min(n_chunks, beg + per);
+  double s1 = 0.0, s2 = 0.0;
+  for (int k = beg + threadIdx.x; k < end; k += kBlock) {
+    s1 += p[k].x;
+    s2 += p[k].y;
+  }
+  __shared__ double red[kBlock][2];
+  red[threadIdx.x][0] = s1;
+  red[threadIdx.x][1] = s2;
+  __syncthreads();
+  for (int o = kBlock / 2; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      red[threadIdx.x][0] += red[threadIdx.x + o][0];
+      red[threadIdx.x][1] += red[threadIdx.x + o][1];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) tmp[blockIdx.y * kSegs + blockIdx.x] = make_double2(red[0][0], red[0][1]);
+}
+__global__ void reduce_segs_kernel(const double2* __restrict__ tmp, double2* sums) {
+  const double2* t = tmp + threadIdx.x * kSegs;  // thread 0: step 0, thread 1: step 1
+  double s1 = 0.0, s2 = 0.0;
+  for (int k = 0; k < kSegs; ++k) {
+    s1 += t[k].x;
+    s2 += t[k].y;
+  }
+  double2 acc = sums[threadIdx.x];
+  acc.x += s1;
+  acc.y += s2;
+  sums[threadIdx.x] = acc;
+}
+
 // K8a: sums[step] += sum over blocks of partial[step][block], in a fixed order
 __global__ void __launch_bounds__(128) reduce_partials_kernel(const double2* __restrict__ partial,
                                                               int stride, int grid, double2* sums) {
@@ -584,9 +810,15 @@ struct KpmWs {
   double* phi_b;
   double2* partial;  // [S][kMaxGrid]
   double2* sums;     // [S]
-  int32_t* status;   // [0] = non-finite flag
+  int32_t* status;   // [0] = non-finite flag, [1] = sweep error, [2] = halo of H in rows
+  int32_t* sync;     // [n/kGroupRows + 1]: step-0 chunks finished per row group   (K7s)
+  double2* cpartial; // [2][n/kMinChunk + 1] chunk sums of one sweep            (K7s)
+  double2* ctmp;     // [2][kSegs]
+  size_t chunk_cap;
   size_t bytes;
 };
+
+constexpr int kMinChunk = 64;  // smallest chunk_rows the workspace is sized for
 
 KpmWs carve_kpm(void* ws, int64_t n, int32_t M, int32_t R) {
   const size_t S = (size_t)(M + 1) / 2;
@@ -597,12 +829,23 @@ KpmWs carve_kpm(void* ws, int64_t n, int32_t M, int32_t R) {
   w.phi_b = c.take<double>((size_t)n * R * 2);
   w.partial = c.take<double2>(S * kMaxGrid);
   w.sums = c.take<double2>(S);
+  w.chunk_cap = (size_t)n / kMinChunk + 1;
+  w.sync = c.take<int32_t>((size_t)n / kGroupRows + 1);
+  w.cpartial = c.take<double2>(2 * w.chunk_cap);
+  w.ctmp = c.take<double2>(2 * kSegs);
   w.bytes = c.off;
   return w;
 }
 
 int fill_grid(int64_t total) {
   return (int)std::max<int64_t>(1, std::min<int64_t>((total + kBlock - 1) / kBlock, kMaxGrid));
+}
+
+using SweepFn = void (*)(const SweepArgs);
+SweepFn sweep_fn(int T, bool diag) {
+  if (T == 1) return diag ? cheb_sweep_kernel<0, true> : cheb_sweep_kernel<0, false>;
+  if (T == 2) return diag ? cheb_sweep_kernel<1, true> : cheb_sweep_kernel<1, false>;
+  return diag ? cheb_sweep_kernel<2, true> : cheb_sweep_kernel<2, false>;
 }
 
 struct LoopTimer {
@@ -661,6 +904,29 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     StepPlan plan;
     rc = make_plan(H, R, false, &plan);
     if (rc != GTB_OK) return rc;
+    // K7s (two steps per HBM sweep): opt-in (GTB_K7_SWEEP=1).  It moves 35 % fewer HBM bytes but
+    // measures 2.60 ms per step at config 5 against K7's 2.20 ms, so K7 stays.
+    int chunk_rows = env_int("GTB_K7_CHUNK", 128);
+    if (chunk_rows != 64 && chunk_rows != 128 && chunk_rows != 256 && chunk_rows != 512 &&
+        chunk_rows != 1024)
+      chunk_rows = 128;
+    const int n_chunks = (int)((n + chunk_rows - 1) / chunk_rows);
+    const bool sweep = env_int("GTB_K7_SWEEP", 0) != 0 && H->width >= 1 && H->width <= 4 &&
+                       (R == 2 || R == 4 || R == 8) && n >= 2 * kGroupRows;
+    int sweep_grid = 0, sweep_slack = 0;
+    if (sweep) {
+      int dev = 0, sms = kSmCount, per_sm = 0;
+      GTB_CUDA_TRY(cudaGetDevice(&dev));
+      GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+          &per_sm, sweep_fn(plan.T, H->diag != nullptr), kBlock, 0));
+      per_sm = std::max(1, std::min(per_sm, env_int("GTB_K7_SWEEP_BPS", kMaxBlocksPerSm)));
+      sweep_grid = sms * per_sm;
+      sweep_slack = env_int("GTB_K7_SLACK", sweep_grid * (kBlock / 32) / 2);  // chunks: one round of all warps
+      GTB_CUDA_TRY(cudaMemsetAsync(w.status + 2, 0, sizeof(int32_t), st));
+      halo_kernel<<<fill_grid(n * H->width), kBlock, 0, st>>>(H->cols, n, H->width, w.status + 2);
+      GTB_LAUNCHED();
+    }
     double* cur = w.phi_a;   // phi_k
     double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
     if (mode == 0) {
@@ -675,7 +941,37 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     launch_step(plan, true, sa, st);  // K6: phi_1, <phi_0|phi_0>, Re<phi_1|phi_0>
     GTB_LAUNCHED();
     if (last_batch) GTB_CUDA_TRY(cudaEventRecord(g_timer.beg, st));
-    for (int k = 1; k < S; ++k) {  // K7: phi_{k+1} from phi_k (cur) and phi_{k-1} (io)
+    int k = 1;
+    if (sweep) {  // K7s: two steps per launch while at least two remain
+      SweepFn fn = sweep_fn(plan.T, H->diag != nullptr);
+      SweepArgs wa;
+      wa.s = sa;
+      wa.s.scale = 2.0 / a;
+      wa.chunk_rows = chunk_rows;
+      wa.n_chunks = n_chunks;
+      wa.halo_rows = w.status + 2;
+      wa.slack = sweep_slack;
+      wa.group_done = w.sync;
+      wa.error = w.status + 1;
+      wa.partial0 = w.cpartial;
+      wa.partial1 = w.cpartial + w.chunk_cap;
+      for (; k + 1 < S; k += 2) {  // phi_{k+1}, phi_{k+2} from phi_k (cur after the swap), phi_{k-1}
+        std::swap(cur, io);
+        wa.s.phi_cur = cur;
+        wa.s.phi_io = io;
+        GTB_CUDA_TRY(cudaMemsetAsync(w.sync, 0, sizeof(int32_t) * ((size_t)n / kGroupRows + 1), st));
+        fn<<<sweep_grid, kBlock, 0, st>>>(wa);
+        GTB_LAUNCHED();
+        reduce_chunks_kernel<<<dim3(kSegs, 2), kBlock, 0, st>>>(wa.partial0, wa.partial1, n_chunks,
+                                                                w.ctmp);
+        GTB_LAUNCHED();
+        reduce_segs_kernel<<<1, 2, 0, st>>>(w.ctmp, w.sums + k);
+        GTB_LAUNCHED();
+        std::swap(cur, io);  // the sweep leaves phi_{k+2} in `cur`'s buffer and phi_{k+1} in `io`'s
+      }
+    }
+    const int k_single = k;
+    for (; k < S; ++k) {  // K7: phi_{k+1} from phi_k (cur) and phi_{k-1} (io)
       std::swap(cur, io);
       sa.phi_cur = cur;
       sa.phi_io = io;
@@ -690,8 +986,13 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
       g_timer.armed = true;
     }
     // partial rows are kMaxGrid apart; only the first plan.grid entries of each are live
-    reduce_partials_kernel<<<S, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);
+    reduce_partials_kernel<<<1, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);
     GTB_LAUNCHED();
+    if (k_single < S) {
+      reduce_partials_kernel<<<S - k_single, 128, 0, st>>>(w.partial + (size_t)k_single * kMaxGrid,
+                                                           kMaxGrid, plan.grid, w.sums + k_single);
+      GTB_LAUNCHED();
+    }
   }
   const double norm = mode == 0 ? (double)n * (double)R_total : (double)n;
   finish_moments_kernel<<<(M + kBlock - 1) / kBlock, kBlock, 0, st>>>(w.sums, M, norm, mu, w.status);
@@ -701,11 +1002,15 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
 
 extern "C" int gtb_kpm_status(const void* ws, void* stream) {
   if (!ws) return GTB_ERR_INVALID_ARG;
-  int32_t flag = 0;
+  int32_t flag[2] = {0, 0};
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  GTB_CUDA_TRY(cudaMemcpyAsync(&flag, ws, sizeof(flag), cudaMemcpyDeviceToHost, st));
+  GTB_CUDA_TRY(cudaMemcpyAsync(flag, ws, sizeof(flag), cudaMemcpyDeviceToHost, st));
   GTB_CUDA_TRY(cudaStreamSynchronize(st));
-  return flag ? GTB_ERR_DIVERGED : GTB_OK;
+  if (flag[1]) {  // a K7s dependency wait ran into its spin limit: the result is not valid
+    note_cuda_error(cudaErrorLaunchTimeout, "cheb_sweep_kernel dependency wait");
+    return GTB_ERR_CUDA;
+  }
+  return flag[0] ? GTB_ERR_DIVERGED : GTB_OK;
 }
 
 extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,

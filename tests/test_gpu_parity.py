@@ -240,6 +240,31 @@ def test_both_k7_paths_match_oracle_rows(monkeypatch, key, nx, ny, kw, R, tile, 
     assert np.abs(got - ref).max() <= 1e-12
 
 
+# K7s: two steps per launch through L2 (temporal blocking).  Forced on here (by default it is
+# taken only when the working set exceeds L2); chunk size, slack and lattice shapes chosen so that
+# the halo spans one chunk, several chunks, and the whole ring (ny = 2: the y-neighbour is n/2 away).
+@pytest.mark.parametrize("key,nx,ny,kw,R", [("c5", 57, 43, {}, 2), ("c1", 24, 24, {}, 4),
+                                             ("c4", 48, 21, {"stripe": 6}, 8), ("c5", 300, 2, {}, 2),
+                                             ("c5", 256, 3, {}, 4)])
+@pytest.mark.parametrize("chunk,slack", [(64, 0), (128, 2368), (256, 7), (512, 592), (1024, 3)])
+@pytest.mark.parametrize("M", [64, 65])
+def test_two_step_sweep_matches_oracle(monkeypatch, key, nx, ny, kw, R, chunk, slack, M):
+    monkeypatch.setenv("GTB_K7_SWEEP", "1")
+    monkeypatch.setenv("GTB_K7_CHUNK", str(chunk))
+    monkeypatch.setenv("GTB_K7_SLACK", str(slack))
+    w, inp = _small(key, nx, ny, kw)
+    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
+    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
+    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
+    ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
+    ws = gtb.workspace(gtb.kpm_workspace_bytes(Ho.n, M, R))
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5, ws=ws, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+    monkeypatch.setenv("GTB_K7_SWEEP", "0")
+    one = gtb.kpm_moments(Hg, a, b, M, R, R, 5, ws=ws, check=True).cpu().numpy()
+    assert np.abs(got - one).max() <= 1e-13          # same vectors, another summation order
+
+
 @pytest.mark.parametrize("drop", [1, 2, 3])
 def test_atom_count_not_a_multiple_of_four_takes_the_register_path(drop):
     # bulk copies need 16-byte aligned slot rows (n % 4 == 0); any other n must still be exact
