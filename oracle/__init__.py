@@ -257,3 +257,29 @@ def vac_conductivity(Cm, a: float, b: float, energies, dt: float, kernel: int = 
                                        C.c_double(dt), C.c_double(scale), _p(rv), _p(sg)),
            "vac_conductivity")
     return rv, sg
+
+
+# ---------------------------------------------------------------- Slater-Koster s,p blocks (NEXT-2)
+class _SkModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite_s", C.c_void_p), ("onsite_p", C.c_void_p),
+                ("sk", C.c_void_p), ("r0", C.c_double), ("beta", C.c_double),
+                ("onsite_shift", C.c_void_p)]
+
+
+def sk_hamiltonian(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, sk, r0: float = 1.0,
+                   beta: float = 0.0, onsite_shift=None, with_diag: bool = True) -> Ell:
+    """Scalar ELL over the 4n orbitals (s, px, py, pz per atom) from the neighbour lists of `nbr`."""
+    pos, species, box, pbc = _f64(pos), _i32(species), _f64(box), _i32(pbc)
+    es, ep, sk = _f64(onsite_s).reshape(-1), _f64(onsite_p).reshape(-1), _f64(sk).reshape(-1)
+    ns = es.shape[0]
+    assert sk.shape[0] == ns * ns * 4
+    shift = _f64(onsite_shift) if onsite_shift is not None else None
+    n, K = nbr.n, nbr.width
+    H = Ell(4 * n, 4 * K, np.zeros((4 * K, 4 * n), dtype=np.int32), np.zeros((4 * K, 4 * n)),
+            np.zeros(4 * n) if with_diag else None)
+    model = _SkModel(ns, es.ctypes.data, ep.ctypes.data, sk.ctypes.data, r0, beta,
+                     shift.ctypes.data if shift is not None else None)
+    nc, hc = nbr._c(), H._c()
+    _check(lib().gtbo_sk_hamiltonian(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
+                                     C.byref(model), C.byref(hc)), "sk_hamiltonian")
+    return H

@@ -140,6 +140,23 @@ int gtbo_vac_conductivity(const double* C, int32_t M, int32_t n_steps, double a,
                           double b, int32_t kernel, const double* energies, int32_t G,
                           double dt, double scale, double* rho_vv, double* sigma);
 
+/* --- multi-orbital Slater-Koster blocks (NEXT-2) ----- */
+/* s,p_x,p_y,p_z on every atom; the table is written out at the top of gtbo_sk.cpp. */
+typedef struct gtbo_sk_model {
+  int32_t n_species;
+  const double* onsite_s;     /* [n_species] eV */
+  const double* onsite_p;     /* [n_species] eV */
+  const double* sk;           /* [n_species][n_species][4]: ss_sigma, sp_sigma, pp_sigma, pp_pi (eV) */
+  double r0;
+  double beta;                /* every V scaled by exp(-beta (r/r0 - 1)); 0 -> no scaling */
+  const double* onsite_shift; /* [n] or NULL */
+} gtbo_sk_model;
+/* nbr: any ELL over the n atoms whose cols are the neighbour lists (vals unused).
+ * H: caller-allocated scalar ELL over 4n orbitals, width 4*nbr->width, diag [4n] or NULL. */
+int gtbo_sk_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* species,
+                        const double box[3], const int32_t pbc[3],
+                        const gtbo_sk_model* model, gtbo_ell* H);
+
 #ifdef __cplusplus
 }
 #endif
