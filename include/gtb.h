@@ -219,6 +219,34 @@ int gtb_vac_conductivity(const double* C, int32_t M, int32_t n_steps, double a, 
                          int32_t kernel, const double* energies, int32_t G, double dt,
                          double scale, double* rho_vv, double* sigma, void* stream);
 
+/* ---- multi-orbital Slater-Koster blocks (reading S1) ----
+ * The paper's H consists of onsite blocks H_ii and hopping blocks H_ij^{lm,l'm'} from Slater-Koster
+ * parameters and the bond direction.  This call assembles the s, p_x, p_y, p_z case: with
+ * (l, m, n) = (x_j - x_i)/r (minimum image) and every V scaled by exp(-beta (r/r0 - 1)),
+ *   E_ss = V_ss_sigma;  E_{s,pa} = a V_sp_sigma;  E_{pa,s} = -a V_sp_sigma;
+ *   E_{pa,pb} = a b V_pp_sigma + (delta_ab - a b) V_pp_pi;   onsite eps_s, eps_p (+ onsite_shift[i]).
+ * The result is a scalar ELL matrix over the 4n orbitals (orbital index 4 i + mu, mu = s, x, y, z) in
+ * the layout of this header: row (i, mu), slot 4 k + nu holds column 4 j + nu and E_{mu nu}, j = the
+ * k-th neighbour of atom i; padding slots (j = i) hold the row's own index and +0.  It is accepted
+ * by gtb_kpm_moments, gtb_velocity_ell (with positions repeated per orbital) and the rest unchanged. */
+typedef struct gtb_sk_model {
+  int32_t n_species;          /* 1..GTB_MAX_SPECIES                                          */
+  const double* onsite_s;     /* HOST [n_species] eV                                         */
+  const double* onsite_p;     /* HOST [n_species] eV                                         */
+  const double* sk;           /* HOST [n_species][n_species][4]: ss_sigma, sp_sigma, pp_sigma, pp_pi */
+  double r0;
+  double beta;
+  const double* onsite_shift; /* DEVICE [n] or NULL                                          */
+} gtb_sk_model;
+
+/* ASYNC.  nbr: any ELL matrix over the n atoms whose cols are the neighbour lists (vals unused),
+ * e.g. the output of gtb_build_hamiltonian.  H: caller-allocated, H->n = 4 n, H->width =
+ * 4 nbr->width, H->diag [4 n] or NULL.  pos, species: DEVICE.  *status (DEVICE int32) is set
+ * non-zero if a species index is out of range. */
+int gtb_sk_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* species,
+                       const double box[3], const int32_t pbc[3], const gtb_sk_model* model,
+                       gtb_ell* H, int32_t* status, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -32,6 +32,7 @@ EXPORTS = (
     "gtb_kpm_last_loop_ms", "gtb_dos", "gtb_jackson",
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
+    "gtb_sk_hamiltonian",
 )
 
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
@@ -401,3 +402,41 @@ def vac_conductivity(Cm: torch.Tensor, a: float, b: float, energies: torch.Tenso
                                     C.c_double(dt), C.c_double(scale), _ptr(rv), _ptr(sg), _stream())
     _check(st, "vac_conductivity")
     return rv, sg
+
+
+# ---------------------------------------------------------------- Slater-Koster s,p blocks (NEXT-2)
+class _SkModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite_s", C.c_void_p), ("onsite_p", C.c_void_p),
+                ("sk", C.c_void_p), ("r0", C.c_double), ("beta", C.c_double),
+                ("onsite_shift", C.c_void_p)]
+
+
+def sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, onsite_s, onsite_p,
+                   sk, r0: float = 1.0, beta: float = 0.0, onsite_shift: Optional[torch.Tensor] = None,
+                   with_diag: bool = True) -> Ell:
+    """Scalar ELL over the 4n orbitals (s, px, py, pz per atom) from the neighbour lists of `nbr`."""
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    es = np.ascontiguousarray(onsite_s, dtype=np.float64).reshape(-1)
+    ep = np.ascontiguousarray(onsite_p, dtype=np.float64).reshape(-1)
+    ns = es.shape[0]
+    sk_h = _host_f64(sk, ns * ns * 4)
+    if onsite_shift is not None:
+        onsite_shift = _dev(onsite_shift, torch.float64, "onsite_shift")
+    n, K, dev = nbr.n, nbr.width, pos.device
+    H = Ell(4 * n, 4 * K, torch.empty((4 * K, 4 * n), dtype=torch.int32, device=dev),
+            torch.empty((4 * K, 4 * n), dtype=torch.float64, device=dev),
+            torch.empty(4 * n, dtype=torch.float64, device=dev) if with_diag else None)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    model = _SkModel(ns, es.ctypes.data, ep.ctypes.data, sk_h.ctypes.data, r0, beta,
+                     onsite_shift.data_ptr() if onsite_shift is not None else None)
+    nc, hc = nbr._c(), H._c()
+    st = lib().gtb_sk_hamiltonian(C.byref(nc), _ptr(pos), _ptr(species), C.c_void_p(box_h.ctypes.data),
+                                  C.c_void_p(pbc_h.ctypes.data), C.byref(model), C.byref(hc),
+                                  _ptr(status), _stream())
+    _check(st, "sk_hamiltonian")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "sk_hamiltonian", "species index out of range")
+    return H
