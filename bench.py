@@ -34,6 +34,7 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
+ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom) or "sp" (s, px, py, pz)
 VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in hbar/eV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
@@ -121,7 +122,12 @@ def _oracle_step(w, inp, energies_of):
     t0 = time.perf_counter()
     H = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0,
                                  w.r0, w.beta, inp.onsite_shift, method=1, with_diag=w.use_diag)
-    if w.a is None:
+    if ORBITALS == "sp":
+        ns = len(w.onsite)
+        H = oracle.sk_hamiltonian(H, inp.pos, inp.species, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
+                                  W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
+                                  onsite_shift=inp.onsite_shift)
+    if w.a is None or ORBITALS == "sp":
         lo, hi = oracle.spectral_bounds(H)
         a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
     else:
@@ -161,6 +167,8 @@ def _cpu_sample(w: W.Workload) -> W.Workload:
     n = 4 * nx * ny
     width_guess = {1.95: 3, 2.65: 10, 4.0: 20}.get(w.cutoff, 10)
     budget = 4e9 * 8 / (width_guess + 5)     # updates that take ~20 s at ~2e8 upd/s for width 3
+    if ORBITALS == "sp":
+        budget /= 16                         # 4x the rows, 4x the width
     M = int(max(16, min(w.M, budget / (n * w.R))))
     return w.scaled(nx, ny, M=M)
 
@@ -190,8 +198,9 @@ def run_reference(args):
         inp = W.make_inputs(s)
         times = [_oracle_step(s, inp, W.energy_grid)[0] for _ in range(args.steps)]
         t = float(np.mean(times))
-        value = s.n_atoms * s.M * s.R / t
-        sample = f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos"
+        orb = 4 if ORBITALS == "sp" else 1
+        value = orb * s.n_atoms * s.M * s.R / t
+        sample = f"{s.name}: N={s.n_atoms} x {orb} orbitals, M={s.M}, R={s.R}, build+moments(direct)+dos"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -235,8 +244,9 @@ def run_ours(args):
 
     ws_build = gtb.workspace(gtb.build_workspace_bytes(n), dev)
     width = gtb.neighbor_width(d_pos, inp.box, inp.pbc, w.cutoff, ws=ws_build)
-    ws_kpm = gtb.workspace(gtb.kpm_workspace_bytes(n, w.M, w.R), dev)
-    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n), dev)
+    n_orb = 4 * n if ORBITALS == "sp" else n          # rows of H: the unit of the metric
+    ws_kpm = gtb.workspace(gtb.kpm_workspace_bytes(n_orb, w.M, w.R), dev)
+    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n_orb), dev)
     mu = torch.empty(w.M, dtype=torch.float64, device=dev)
     h_rho = torch.empty(w.n_energies, dtype=torch.float64).pin_memory()
     state = {}
@@ -244,7 +254,12 @@ def run_ours(args):
     def step(pos, spec, shift):
         H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
                                   w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
-        if w.a is None:
+        if ORBITALS == "sp":   # Slater-Koster s,p blocks on the neighbour lists just built
+            ns = len(w.onsite)
+            H = gtb.sk_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
+                                   W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
+                                   onsite_shift=shift)
+        if w.a is None or ORBITALS == "sp":
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
@@ -295,13 +310,13 @@ def run_ours(args):
         e2e_step()
     ms_e2e, _, _, _ = timed(e2e_step, args.steps)
 
-    units = float(n) * w.M * w.R * args.steps            # per rank
+    units = float(n_orb) * w.M * w.R * args.steps        # per rank
     value = replicas.whole_job_value(units, ms)
     e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
-    bytes_per_launch = float(n) * per_atom
+    bytes_per_launch = float(n_orb) * per_atom
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
@@ -319,13 +334,14 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128 vectors)",
             "data": "synthetic",
-            "config": {"workload": w.name, "atoms": n, "ell_width": H.width, "moments": w.M,
+            "config": {"workload": w.name, "atoms": n, "orbitals_per_atom": n_orb // n,
+                       "ell_width": H.width, "moments": w.M,
                        "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (
-                           (2 * n * w.R * 16 + H.nbytes()) / 1e9),
+                           (2 * n_orb * w.R * 16 + H.nbytes()) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "seconds_per_full_dos": ms / args.steps * 1e-3,
-            "recursion_updates_per_s": float(n) * w.M * w.R / ((loop_ms / args.steps + k7_ms) * 1e-3),
+            "recursion_updates_per_s": float(n_orb) * w.M * w.R / ((loop_ms / args.steps + k7_ms) * 1e-3),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": h_rho.numel() * 8, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": launches, "roofline": roofline, "clocks": clk.summary()}
@@ -333,9 +349,10 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             s = _cpu_sample(w)
             t, _ = _oracle_step(s, W.make_inputs(s), W.energy_grid)
+            orb = 4 if ORBITALS == "sp" else 1
             line["cpu_baseline"] = {
-                "value": s.n_atoms * s.M * s.R / t, "unit": UNIT, "cores": _cores(), "kind": "oracle",
-                "sample": f"{s.name}: N={s.n_atoms}, M={s.M}, R={s.R}, build+moments(direct)+dos, {t:.1f} s"}
+                "value": orb * s.n_atoms * s.M * s.R / t, "unit": UNIT, "cores": _cores(), "kind": "oracle",
+                "sample": f"{s.name}: N={s.n_atoms} x {orb} orbitals, M={s.M}, R={s.R}, build+moments(direct)+dos, {t:.1f} s"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -482,7 +499,13 @@ def main():
     p.add_argument("--quantity", default="dos", choices=["dos", "vac"],
                    help="dos: the headline path (Eq. 4); vac: the VAC conductivity (Eq. 3, NEXT-1)")
     p.add_argument("--time-steps", type=int, default=24, help="vac: points of the time grid (dt = 0.1 fs)")
+    p.add_argument("--orbitals", default="pz", choices=["pz", "sp"],
+                   help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
+    global ORBITALS
+    ORBITALS = args.orbitals
+    if args.orbitals == "sp" and args.quantity == "vac":
+        raise SystemExit("bench.py: --orbitals sp is wired for --quantity dos only")
     if args.quantity == "vac" and not args.moments:
         args.moments = 512
     if args.impl == "reference":

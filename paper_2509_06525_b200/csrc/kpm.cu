@@ -254,11 +254,16 @@ __host__ __device__ inline uint32_t tile_stage_bytes(int width, int TR, bool dia
   return (uint32_t)((width * TR * 12 + (diag ? TR * 8 : 0) + 127) / 128 * 128);
 }
 
+#ifndef GTB_TILE_BLOCK
+#define GTB_TILE_BLOCK 256
+#endif
+constexpr int kTileBlock = GTB_TILE_BLOCK;  // threads per CTA of K7t
+
 template <int LOG2T, bool kFirst, bool kDiag, int CH, bool kDotL>
-__global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
+__global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
-  constexpr int TR = kBlock / T;  // rows per tile: one thread per 256-bit element
+  constexpr int TR = kTileBlock / T;  // rows per tile: one thread per 256-bit element
   extern __shared__ __align__(128) unsigned char smem[];
   const int64_t n = a.n;
   const int width = a.width;
@@ -366,7 +371,7 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
       store_stream<VW>(a.phi_io + e * VW, y);
     }
   }
-  __shared__ double red[kBlock / 32][2];
+  __shared__ double red[kTileBlock / 32][2];
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
   if (lane == 0) {
@@ -376,7 +381,7 @@ __global__ void __launch_bounds__(kBlock) cheb_tile_kernel(const StepArgs a, con
   __syncthreads();
   if (tid == 0) {
 #pragma unroll
-    for (int w = 1; w < kBlock / 32; ++w) {
+    for (int w = 1; w < kTileBlock / 32; ++w) {
       s1 += red[w][0];
       s2 += red[w][1];
     }
@@ -743,7 +748,7 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
     if (log2t == 0) pick_tile<0>(diag, tch, dot, p);
     else if (log2t == 1) pick_tile<1>(diag, tch, dot, p);
     else pick_tile<2>(diag, tch, dot, p);
-    const int TR = kBlock / p->T;
+    const int TR = kTileBlock / p->T;
     const size_t stage_bytes = tile_stage_bytes(width, TR, diag);
     int max_smem = 0;
     GTB_CUDA_TRY(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
@@ -753,8 +758,8 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
     if (smem <= (size_t)max_smem) {
       GTB_CUDA_TRY(cudaFuncSetAttribute(p->tfirst, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       GTB_CUDA_TRY(cudaFuncSetAttribute(p->tnext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kBlock, smem));
-      per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
+      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kTileBlock, smem));
+      per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm * kBlock / kTileBlock));
       const int64_t n_tiles = (n + TR - 1) / TR;
       p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, (int64_t)sms * per_sm));
       p->grid = std::min(p->grid, kMaxGrid);
@@ -773,7 +778,7 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
 
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st) {
   if (p.stages > 0)
-    (first ? p.tfirst : p.tnext)<<<p.grid, kBlock, p.smem, st>>>(sa, p.stages);
+    (first ? p.tfirst : p.tnext)<<<p.grid, kTileBlock, p.smem, st>>>(sa, p.stages);
   else
     (first ? p.first : p.next)<<<p.grid, kBlock, 0, st>>>(sa);
 }

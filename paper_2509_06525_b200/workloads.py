@@ -153,3 +153,20 @@ def energy_grid(w: Workload, a: float, b: float) -> np.ndarray:
 def algorithmic_bytes_per_atom_pass(width: int, has_diag: bool, R: int) -> int:
     """B = 12 K + 8 [diag] + 48 R bytes per atom per recursion pass."""
     return 12 * width + (8 if has_diag else 0) + 48 * R
+
+
+# ---- synthetic Slater-Koster s,p parameters for the multi-orbital runs (bench.py --orbitals sp) ----
+# graphene-like two-centre integrals (eV): ss_sigma, sp_sigma, pp_sigma, pp_pi, scaled per species pair
+# (species 0 = C, 1 = B, 2 = N as in config 4); inputs only, no method arithmetic.
+SK_CC = (-6.769, 5.580, 5.037, -3.033)
+SK_ONSITE_S = (-8.868, -6.0, -11.0)
+SK_ONSITE_P = (0.0, 2.3, -2.3)
+_SK_PAIR_SCALE = {(0, 0): 1.0, (1, 2): 0.96, (0, 1): 0.93, (0, 2): 1.04, (1, 1): 0.5, (2, 2): 0.5}
+
+
+def sk_table(n_species: int) -> np.ndarray:
+    t = np.zeros((n_species, n_species, 4))
+    for (a, b), f in _SK_PAIR_SCALE.items():
+        if a < n_species and b < n_species:
+            t[a, b] = t[b, a] = f * np.array(SK_CC)
+    return t
