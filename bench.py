@@ -264,7 +264,8 @@ def run_ours(args):
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, ws=ws_kpm, mu=mu)
+        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode=gtb.MODE_ORB4 if ORBITALS == "sp" else 0,
+                        ws=ws_kpm, mu=mu)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         rho = gtb.dos(mu, a, b, state["E"])
@@ -315,12 +316,16 @@ def run_ours(args):
     e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
+    orb4 = ORBITALS == "sp" and os.environ.get("GTB_K7_ORB4", "1") != "0" and w.R in (2, 4, 8)
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
+    if orb4:   # per orbital row: K blocks of (4 B column + 128 B values) shared by 4 rows, + diag + vectors
+        per_atom = (H.width // 4) * 132 // 4 + (8 if H.diag is not None else 0) + 48 * w.R
     bytes_per_launch = float(n_orb) * per_atom
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
-    k7_name = ("cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
+    k7_name = ("cheb_orb4_kernel (K7b: fused Chebyshev pass on 4x4 orbital blocks)" if orb4 else
+               "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
                if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
                else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
     roofline = {"bound": "hbm", "kernel": k7_name,

@@ -57,6 +57,7 @@ enum {
   GTB_ERR_INDEX_RANGE = -7    /* n too large for int32 indices                     */
 };
 
+#define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
 
@@ -131,6 +132,10 @@ int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, doubl
  *         R_batch at a time (each pass of H serves R_batch vectors).
  * mode 1: exact trace over all n basis vectors e_i (R_total and seed ignored),
  *         R_batch of them per pass.
+ * mode | GTB_MODE_ORB4: the caller promises that H is the orbital-blocked matrix written by
+ *         gtb_sk_hamiltonian (4 orbitals per atom); the fused pass then works on whole 4x4
+ *         blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
+ *         when R_batch is not 2, 4 or 8.  A matrix without that structure gives wrong results.
  * R_batch: 1..64.  R_batch in {2,4,8} takes the 256-bit vector path.
  * ASYNC.  mu is DEVICE [M].  Workspace: gtb_kpm_workspace_bytes(n, M, R_batch). */
 size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch);

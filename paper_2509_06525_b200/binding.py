@@ -35,6 +35,7 @@ EXPORTS = (
     "gtb_sk_hamiltonian",
 )
 
+MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
 
 
@@ -250,7 +251,7 @@ def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
                 check: bool = False) -> torch.Tensor:
     dev = H.vals.device if H.width else H.diag.device
     if R_batch is None:
-        R_batch = R_total if mode == 0 else 8
+        R_batch = R_total if (mode & 1) == 0 else 8
     if mu is None:
         mu = torch.empty(M, dtype=torch.float64, device=dev)
     if ws is None:

@@ -389,6 +389,95 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
   }
 }
 
+// ---- K7b: the fused pass on an orbital-blocked matrix (4 orbitals per atom) --------------------
+// gtb_sk_hamiltonian's scalar ELL is block-structured: rows 4i..4i+3 (atom i) hold, in slots
+// 4k..4k+3, the 4x4 block of the pair (i, j_k), column 4 j_k + nu in slot 4k + nu; for fixed nu the
+// four entries mu = 0..3 are contiguous (32 bytes).  The scalar kernels ignore that: each orbital
+// row gathers the neighbour's four orbitals again (16 gathers per block) and reads 16 column
+// indices.  Here one thread owns (atom i, one 256-bit element of the R vectors) for all four
+// orbitals: per neighbour it reads ONE column index, the block as four 256-bit loads and the
+// neighbour's four orbital elements as four gathers, and does the 4x4xVW FMAs in registers:
+// a quarter of the L1 wavefronts and 144 instead of 192 bytes of H per block from HBM.
+// Same arithmetic per element as K7 (slot order, then diagonal), so the vectors agree bit for bit.
+template <int LOG2T, bool kFirst, bool kDiag>
+__global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  const int64_t N = a.n;             // orbital rows
+  const int64_t n_atoms = N >> 2;
+  const int K = a.width >> 2;        // neighbour slots per atom
+  const int64_t total = n_atoms * T;
+  const double scale = a.scale, b = a.b;
+  constexpr int64_t kOrb = (int64_t)T * VW;  // doubles per orbital row of phi
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t i = e >> LOG2T;
+    const int64_t t = e - i * T;
+    const double* xt = a.phi_cur + t * VW;
+    const int32_t* cp = a.cols + 4 * i;
+    const double* vp = a.vals + 4 * i;
+    Vec<VW> acc[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    int64_t j = K > 0 ? (int64_t)(__ldg(cp) >> 2) : 0;
+    for (int k = 0; k < K; ++k) {
+      const int64_t jn = k + 1 < K ? (int64_t)(__ldg(cp + (size_t)(4 * (k + 1)) * N) >> 2) : 0;
+      Vec<VW> B[4], x[4];
+#pragma unroll
+      for (int nu = 0; nu < 4; ++nu) B[nu] = load_stream<VW>(vp + (size_t)(4 * k + nu) * N);
+#pragma unroll
+      for (int nu = 0; nu < 4; ++nu) x[nu] = load_gather<VW>(xt + (4 * j + nu) * kOrb);
+#pragma unroll
+      for (int nu = 0; nu < 4; ++nu)   // slot order 4k + nu, as the scalar kernels
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+          for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(B[nu].v[mu], x[nu].v[q], acc[mu].v[q]);
+      j = jn;
+    }
+    Vec<VW> dg;
+    if (kDiag) dg = load_stream<VW>(a.diag + 4 * i);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      const int64_t at = (4 * i + mu) * kOrb + t * VW;
+      const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
+      Vec<VW> prev;
+      if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+      Vec<VW> y;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        double h = acc[mu].v[q];
+        if (kDiag) h = fma(dg.v[mu], own.v[q], h);
+        y.v[q] = (h - b * own.v[q]) * scale;
+        if (!kFirst) y.v[q] -= prev.v[q];
+        s1 = fma(own.v[q], own.v[q], s1);
+        s2 = fma(y.v[q], own.v[q], s2);
+      }
+      store_stream<VW>(a.phi_io + at, y);
+    }
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
 // ---- K7s: two Chebyshev steps per HBM sweep (temporal blocking through L2) -----------------------
 // One pass of K7 moves 12K + 48R bytes per atom through HBM for one step.  Here one launch advances
 // every row by TWO steps: rows are cut into chunks of `chunk_rows`; task (j, l) = step l (0 or 1)
@@ -721,6 +810,33 @@ int env_int(const char* name, int dflt) {
 
 }  // namespace
 
+template <int LOG2T>
+void pick_orb4(bool diag, StepPlan* p) {
+  p->first = diag ? cheb_orb4_kernel<LOG2T, true, true> : cheb_orb4_kernel<LOG2T, true, false>;
+  p->next = diag ? cheb_orb4_kernel<LOG2T, false, true> : cheb_orb4_kernel<LOG2T, false, false>;
+}
+
+// K7b plan: one thread per (atom, 256-bit element); falls back (returns false) when H or R does not fit
+bool make_plan_orb4(const gtb_ell* H, int R, StepPlan* p) {
+  if (H->n % 4 || H->width % 4 || H->width == 0 || (R != 2 && R != 4 && R != 8) ||
+      (reinterpret_cast<uintptr_t>(H->vals) & 31u) || (reinterpret_cast<uintptr_t>(H->diag) & 31u))
+    return false;
+  if (R == 2) { pick_orb4<0>(H->diag != nullptr, p); p->T = 1; }
+  else if (R == 4) { pick_orb4<1>(H->diag != nullptr, p); p->T = 2; }
+  else { pick_orb4<2>(H->diag != nullptr, p); p->T = 4; }
+  p->vw = 4;
+  p->stages = 0;
+  int dev = 0, sms = kSmCount, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0) != cudaSuccess)
+    return false;
+  per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
+  const int64_t total = H->n / 4 * p->T;
+  p->grid = (int)std::max<int64_t>(1, std::min<int64_t>((total + kBlock - 1) / kBlock, (int64_t)sms * per_sm));
+  return true;
+}
+
 int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   const int64_t n = H->n;
   const int width = H->width;
@@ -882,10 +998,13 @@ extern "C" size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch)
 }
 
 extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
-                               int32_t R_batch, uint64_t seed, int32_t mode, double* mu, void* ws,
+                               int32_t R_batch, uint64_t seed, int32_t mode_flags, double* mu, void* ws,
                                size_t ws_bytes, void* stream) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
+  if (mode_flags & ~(1 | GTB_MODE_ORB4)) return GTB_ERR_INVALID_ARG;
+  const int32_t mode = mode_flags & 1;
+  const bool orb4 = (mode_flags & GTB_MODE_ORB4) != 0;
   if (!mu || M <= 0 || !(a > 0.0) || !std::isfinite(b) || R_batch <= 0 || R_batch > 64 ||
       (mode != 0 && mode != 1) || (mode == 0 && R_total <= 0))
     return GTB_ERR_INVALID_ARG;
@@ -907,8 +1026,11 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    rc = make_plan(H, R, false, &plan);
-    if (rc != GTB_OK) return rc;
+    const bool blocked = orb4 && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb4(H, R, &plan);
+    if (!blocked) {
+      rc = make_plan(H, R, false, &plan);
+      if (rc != GTB_OK) return rc;
+    }
     // K7s (two steps per HBM sweep): opt-in (GTB_K7_SWEEP=1).  It moves 35 % fewer HBM bytes but
     // measures 2.60 ms per step at config 5 against K7's 2.20 ms, so K7 stays.
     int chunk_rows = env_int("GTB_K7_CHUNK", 128);
@@ -916,7 +1038,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
         chunk_rows != 1024)
       chunk_rows = 128;
     const int n_chunks = (int)((n + chunk_rows - 1) / chunk_rows);
-    const bool sweep = env_int("GTB_K7_SWEEP", 0) != 0 && H->width >= 1 && H->width <= 4 &&
+    const bool sweep = !blocked && env_int("GTB_K7_SWEEP", 0) != 0 && H->width >= 1 && H->width <= 4 &&
                        (R == 2 || R == 4 || R == 8) && n >= 2 * kGroupRows;
     int sweep_grid = 0, sweep_slack = 0;
     if (sweep) {

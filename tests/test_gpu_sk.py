@@ -75,6 +75,36 @@ def test_moments_and_dos_on_the_orbital_matrix(key, nx, ny, cutoff, beta, kw, R)
     assert np.abs(rho - rho_ref).max() <= 1e-8 * rho_ref.max()
 
 
+@pytest.mark.parametrize("key,nx,ny,cutoff,beta,kw", CASES)
+@pytest.mark.parametrize("R_total,R_batch", [(2, 2), (4, 4), (8, 8), (6, 4), (3, 3)])
+def test_blocked_pass_matches_oracle_and_scalar_path(key, nx, ny, cutoff, beta, kw, R_total, R_batch):
+    """K7b (mode | MODE_ORB4): whole 4x4 blocks per thread.  R_batch = 3 falls back to the scalar path."""
+    w, inp, Ho, Hg = _both(key, nx, ny, cutoff, beta, **kw)
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    M = 65
+    ref = oracle.kpm_moments(Ho, a, b, M, R_total, 21, mode=0, algo=0)
+    got = gtb.kpm_moments(Hg, a, b, M, R_total, R_batch, 21, mode=gtb.MODE_ORB4, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+    plain = gtb.kpm_moments(Hg, a, b, M, R_total, R_batch, 21, mode=0).cpu().numpy()
+    assert np.abs(got - plain).max() <= 1e-13         # same vectors, another summation order
+    # without the diagonal array as well
+    Hn = gtb.Ell(Hg.n, Hg.width, Hg.cols, Hg.vals, None)
+    Hon = oracle.Ell(Ho.n, Ho.width, Ho.cols, Ho.vals, None)
+    ref = oracle.kpm_moments(Hon, a, b, 33, R_total, 22, mode=0, algo=0)
+    got = gtb.kpm_moments(Hn, a, b, 33, R_total, R_batch, 22, mode=gtb.MODE_ORB4).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+
+
+def test_blocked_exact_trace_against_eigvalsh():
+    w, inp, Ho, Hg = _both("c2b", 5, 4, 2.65, 3.37)
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    got = gtb.kpm_moments(Hg, a, b, 40, mode=1 | gtb.MODE_ORB4, R_batch=8).cpu().numpy()
+    th = np.arccos((np.linalg.eigvalsh(Ho.to_dense()) - b) / a)
+    assert np.abs(got - np.array([np.cos(k * th).mean() for k in range(40)])).max() <= 1e-12
+
+
 def test_exact_trace_against_eigvalsh():
     w, inp, Ho, Hg = _both("c2b", 5, 4, 2.65, 3.37)
     lo, hi = oracle.spectral_bounds(Ho)
