@@ -205,7 +205,8 @@ int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32_t R, doubl
  *   psiL_r(tau) = U(tau) phi_r,  psiR_r(tau) = U(tau) V phi_r,  U(tau_j) = U(dt)^j,
  * by chi_0 = V psiR, chi_1 = H~ chi_0, chi_{n+1} = 2 H~ chi_n - chi_{n-1}, C_n = Re<psiL|chi_n>:
  * M-1 fused passes per time step (the DOS kernel with the dot products taken against psiL).
- * mode, R_total, R_batch, seed: as gtb_kpm_moments (mode 1: / N).  C is DEVICE [n_steps][M].
+ * mode (incl. the GTB_MODE_ORB4 flag), R_total, R_batch, seed: as gtb_kpm_moments (mode 1: / N).
+ * C is DEVICE [n_steps][M].
  * Workspace: gtb_vac_workspace_bytes(n, M, n_steps, R_batch); gtb_kpm_status(ws) reports
  * non-finite results as GTB_ERR_DIVERGED. */
 size_t gtb_vac_workspace_bytes(int64_t n, int32_t M, int32_t n_steps, int32_t R_batch);

@@ -367,7 +367,7 @@ def vac_moments(H: Ell, vvals: torch.Tensor, a: float, b: float, M: int, n_steps
     """C[j][n], j < n_steps, n < M (readings V2, V3)."""
     dev = H.vals.device
     if R_batch is None:
-        R_batch = R_total if mode == 0 else 8
+        R_batch = R_total if (mode & 1) == 0 else 8
     if out is None:
         out = torch.empty((n_steps, M), dtype=torch.float64, device=dev)
     if ws is None:

@@ -399,7 +399,7 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
 // neighbour's four orbital elements as four gathers, and does the 4x4xVW FMAs in registers:
 // a quarter of the L1 wavefronts and 144 instead of 192 bytes of H per block from HBM.
 // Same arithmetic per element as K7 (slot order, then diagonal), so the vectors agree bit for bit.
-template <int LOG2T, bool kFirst, bool kDiag>
+template <int LOG2T, bool kFirst, bool kDiag, bool kDotL>
 __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
@@ -444,8 +444,9 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
     for (int mu = 0; mu < 4; ++mu) {
       const int64_t at = (4 * i + mu) * kOrb + t * VW;
       const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
-      Vec<VW> prev;
+      Vec<VW> prev, with;
       if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+      if (kDotL) with = load_stream<VW>(a.dot_with + at);
       Vec<VW> y;
 #pragma unroll
       for (int q = 0; q < VW; ++q) {
@@ -453,8 +454,8 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
         if (kDiag) h = fma(dg.v[mu], own.v[q], h);
         y.v[q] = (h - b * own.v[q]) * scale;
         if (!kFirst) y.v[q] -= prev.v[q];
-        s1 = fma(own.v[q], own.v[q], s1);
-        s2 = fma(y.v[q], own.v[q], s2);
+        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
       }
       store_stream<VW>(a.phi_io + at, y);
     }
@@ -810,20 +811,25 @@ int env_int(const char* name, int dflt) {
 
 }  // namespace
 
+template <int LOG2T, bool DOT>
+void pick_orb4_dot(bool diag, StepPlan* p) {
+  p->first = diag ? cheb_orb4_kernel<LOG2T, true, true, DOT> : cheb_orb4_kernel<LOG2T, true, false, DOT>;
+  p->next = diag ? cheb_orb4_kernel<LOG2T, false, true, DOT> : cheb_orb4_kernel<LOG2T, false, false, DOT>;
+}
 template <int LOG2T>
-void pick_orb4(bool diag, StepPlan* p) {
-  p->first = diag ? cheb_orb4_kernel<LOG2T, true, true> : cheb_orb4_kernel<LOG2T, true, false>;
-  p->next = diag ? cheb_orb4_kernel<LOG2T, false, true> : cheb_orb4_kernel<LOG2T, false, false>;
+void pick_orb4(bool diag, bool dot, StepPlan* p) {
+  if (dot) pick_orb4_dot<LOG2T, true>(diag, p);
+  else pick_orb4_dot<LOG2T, false>(diag, p);
 }
 
 // K7b plan: one thread per (atom, 256-bit element); falls back (returns false) when H or R does not fit
-bool make_plan_orb4(const gtb_ell* H, int R, StepPlan* p) {
+bool make_plan_orb4(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   if (H->n % 4 || H->width % 4 || H->width == 0 || (R != 2 && R != 4 && R != 8) ||
       (reinterpret_cast<uintptr_t>(H->vals) & 31u) || (reinterpret_cast<uintptr_t>(H->diag) & 31u))
     return false;
-  if (R == 2) { pick_orb4<0>(H->diag != nullptr, p); p->T = 1; }
-  else if (R == 4) { pick_orb4<1>(H->diag != nullptr, p); p->T = 2; }
-  else { pick_orb4<2>(H->diag != nullptr, p); p->T = 4; }
+  if (R == 2) { pick_orb4<0>(H->diag != nullptr, dot, p); p->T = 1; }
+  else if (R == 4) { pick_orb4<1>(H->diag != nullptr, dot, p); p->T = 2; }
+  else { pick_orb4<2>(H->diag != nullptr, dot, p); p->T = 4; }
   p->vw = 4;
   p->stages = 0;
   int dev = 0, sms = kSmCount, per_sm = 0;
@@ -1026,7 +1032,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    const bool blocked = orb4 && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb4(H, R, &plan);
+    const bool blocked = orb4 && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb4(H, R, false, &plan);
     if (!blocked) {
       rc = make_plan(H, R, false, &plan);
       if (rc != GTB_OK) return rc;

@@ -271,10 +271,13 @@ thread_local VacTimer g_vac_timer;
 
 extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, double b, int32_t M,
                                int32_t n_steps, double dt, int32_t R_total, int32_t R_batch,
-                               uint64_t seed, int32_t mode, double* C, void* ws, size_t ws_bytes,
+                               uint64_t seed, int32_t mode_flags, double* C, void* ws, size_t ws_bytes,
                                void* stream) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
+  if (mode_flags & ~(1 | GTB_MODE_ORB4)) return GTB_ERR_INVALID_ARG;
+  const int32_t mode = mode_flags & 1;
+  const bool orb4 = (mode_flags & GTB_MODE_ORB4) != 0;
   if (!vvals || !C || M <= 0 || n_steps <= 0 || !(a > 0.0) || !std::isfinite(b) ||
       !std::isfinite(dt) || R_batch <= 0 || R_batch > 64 || (mode != 0 && mode != 1) ||
       (mode == 0 && R_total <= 0))
@@ -297,10 +300,12 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan, dplan;  // evolution passes (no bra) and moment passes (dot with psiL)
-    rc = make_plan(H, R, false, &plan);
-    if (rc != GTB_OK) return rc;
-    rc = make_plan(H, R, true, &dplan);
-    if (rc != GTB_OK) return rc;
+    if (!(orb4 && make_plan_orb4(H, R, false, &plan) && make_plan_orb4(H, R, true, &dplan))) {
+      rc = make_plan(H, R, false, &plan);
+      if (rc != GTB_OK) return rc;
+      rc = make_plan(H, R, true, &dplan);
+      if (rc != GTB_OK) return rc;
+    }
     double *psiL = w.buf[0], *psiR = w.buf[1], *sa_ = w.buf[2], *sb_ = w.buf[3];
     launch_fill(mode, seed, r0, R, n, psiL, st);
     GTB_LAUNCHED();

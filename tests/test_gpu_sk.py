@@ -128,6 +128,11 @@ def test_vac_moments_with_per_orbital_positions():
     ref = oracle.vac_moments(Ho, vo, a, b, 24, 3, dt, R=2, seed=4, mode=0)
     got = gtb.vac_moments(Hg, vg, a, b, 24, 3, dt, 2, 2, 4, check=True).cpu().numpy()
     assert np.abs(got - ref).max() <= 1e-11 * ref[0, 0]
+    # and with the blocked pass (propagation and bra-dot moments on 4x4 blocks)
+    for R in (2, 4, 8):
+        ref = oracle.vac_moments(Ho, vo, a, b, 17, 3, dt, R=R, seed=4, mode=0)
+        got = gtb.vac_moments(Hg, vg, a, b, 17, 3, dt, R, R, 4, mode=gtb.MODE_ORB4, check=True).cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-11 * ref[0, 0]
 
 
 def test_bad_species_and_shapes_are_reported():
