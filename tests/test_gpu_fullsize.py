@@ -197,3 +197,34 @@ def test_c5_vac_properties_at_hundred_million_atoms():
     assert abs(C[0, 0] - c00) <= bound
     assert np.abs(C[:, 1::2]).max() <= bound
     assert C[2, 0] < C[1, 0] < C[0, 0]
+
+
+# ------------------------------------------------------------------ Slater-Koster s,p blocks at full size
+def test_c4_sk_blocks_and_blocked_moments_full_size():
+    """10^6 atoms x 4 orbitals (the launch configuration `bench.py --orbitals sp --workload c4` times):
+    every block against the oracle's, and a short run of the blocked pass K7b against the oracle's
+    direct definition."""
+    w = W.CONFIGS["c4"]
+    inp = W.make_inputs(w)
+    ns = len(w.onsite)
+    ones = np.ones((ns, ns))
+    nbr_o = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, [0.0] * ns, ones,
+                                     with_diag=False, method=1)
+    Ho = oracle.sk_hamiltonian(nbr_o, inp.pos, inp.species, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
+                               W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta)
+    nbr_g = gtb.build_hamiltonian(_dev(inp.pos), _dev(inp.species), inp.box, inp.pbc, w.cutoff,
+                                  [0.0] * ns, ones, with_diag=False)
+    Hg = gtb.sk_hamiltonian(nbr_g, _dev(inp.pos), _dev(inp.species), inp.box, inp.pbc,
+                            W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta)
+    assert Hg.n == 4_000_000 and Hg.width == 12
+    assert (Hg.cols.cpu().numpy() == Ho.cols).all()
+    assert np.abs(Hg.vals.cpu().numpy() - Ho.vals).max() <= 8 * 2.0**-52 * np.abs(Ho.vals).max()
+    assert (Hg.diag.cpu().numpy() == Ho.diag).all()
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    M = 10
+    ref = oracle.kpm_moments(Ho, a, b, M, w.R, w.seed, mode=0, algo=0)
+    ws = gtb.workspace(gtb.kpm_workspace_bytes(Hg.n, M, w.R))
+    got = gtb.kpm_moments(Hg, a, b, M, w.R, w.R, w.seed, mode=gtb.MODE_ORB4, ws=ws, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-9
+    assert np.abs(got - ref).max() <= 1e-12
