@@ -283,3 +283,34 @@ def sk_hamiltonian(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, sk, r0:
     _check(lib().gtbo_sk_hamiltonian(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
                                      C.byref(model), C.byref(hc)), "sk_hamiltonian")
     return H
+
+
+# ---------------------------------------------------------------- descriptor + MLP hopping (Eq. 2, NEXT-3)
+class _MlpModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("n_features", C.c_int32), ("n_basis", C.c_int32),
+                ("n_hidden", C.c_int32), ("r_cut", C.c_double), ("weights", C.c_void_p)]
+
+
+def mlp_descriptor(dims, r_cut: float, weights, si: int, sj: int, r: float) -> np.ndarray:
+    ns, F, Nb, Hd = dims
+    w = _f64(weights)
+    m = _MlpModel(ns, F, Nb, Hd, r_cut, w.ctypes.data)
+    out = np.zeros(F)
+    _check(lib().gtbo_mlp_descriptor(C.byref(m), C.c_int32(si), C.c_int32(sj), C.c_double(r), _p(out)),
+           "mlp_descriptor")
+    return out
+
+
+def mlp_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, weights,
+                    with_diag: bool = True, return_v: bool = False):
+    """H on the pattern of `nbr` with t_ij, eps_i from the descriptor + MLPs (weight blob: gtbo_mlp.cpp)."""
+    ns, F, Nb, Hd = dims
+    pos, species, box, pbc, w = _f64(pos), _i32(species), _f64(box), _i32(pbc), _f64(weights)
+    H = Ell(nbr.n, nbr.width, nbr.cols.copy(), np.zeros((nbr.width, nbr.n)),
+            np.zeros(nbr.n) if with_diag else None)
+    v = np.zeros((nbr.n, F))
+    m = _MlpModel(ns, F, Nb, Hd, r_cut, w.ctypes.data)
+    hc = H._c()
+    _check(lib().gtbo_mlp_hamiltonian(C.byref(m), _p(pos), _p(species), _p(box), _p(pbc), C.byref(hc),
+                                      _p(v)), "mlp_hamiltonian")
+    return (H, v) if return_v else H

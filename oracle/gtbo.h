@@ -157,6 +157,20 @@ int gtbo_sk_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* s
                         const double box[3], const int32_t pbc[3],
                         const gtbo_sk_model* model, gtbo_ell* H);
 
+/* --- environment-dependent hopping from the paper's descriptor + MLPs (Eq. 2; NEXT-3) */
+/* One orbital per atom.  Formulas, readings E1-E4 and the weight blob layout: top of gtbo_mlp.cpp. */
+typedef struct gtbo_mlp_model {
+  int32_t n_species, n_features /*F*/, n_basis /*Nb*/, n_hidden /*Hd*/;
+  double r_cut;
+  const double* weights;
+} gtbo_mlp_model;
+/* C[n] = C_n(r) for the species pair (si, sj), n = 0..F-1. */
+int gtbo_mlp_descriptor(const gtbo_mlp_model* m, int32_t si, int32_t sj, double r, double* C);
+/* H->cols given (neighbour lists); fills H->vals (t_ij; padding 0) and H->diag (eps_i) if non-NULL;
+ * v_out ([n][F], optional) receives the node features v_i. */
+int gtbo_mlp_hamiltonian(const gtbo_mlp_model* m, const double* pos, const int32_t* species,
+                         const double box[3], const int32_t pbc[3], gtbo_ell* H, double* v_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -170,3 +170,33 @@ def sk_table(n_species: int) -> np.ndarray:
         if a < n_species and b < n_species:
             t[a, b] = t[b, a] = f * np.array(SK_CC)
     return t
+
+
+# ---- synthetic weights for the descriptor + MLP Hamiltonian (Eq. 2; bench.py / tests, NEXT-3) ----
+# Blob layout (doubles), shared by both implementations as an INPUT format:
+#   c [ns][ns][F][Nb] | MLP_e: W1 [Hd][F], b1 [Hd], W2 [F][Hd], b2 [F] |
+#   MLP_lambda: W1 [Hd][F], b1 [Hd], W2 [Hd], b2 [1] | per species: W1 [Hd][F], b1 [Hd], W2 [Hd], b2 [1]
+MLP_DIMS = (3, 8, 8, 16)       # species, features F, basis functions Nb, hidden width Hd
+
+
+def mlp_pack(c, env, hop, ons) -> np.ndarray:
+    """c [ns,ns,F,Nb]; env = (W1, b1, W2, b2); hop = (W1, b1, W2, b2); ons = list of the same per species."""
+    parts = [np.asarray(c, dtype=np.float64).ravel()]
+    for group in [env, hop, *ons]:
+        parts += [np.asarray(x, dtype=np.float64).ravel() for x in group]
+    return np.ascontiguousarray(np.concatenate(parts))
+
+
+def mlp_weights(dims=MLP_DIMS, seed: int = 65250) -> np.ndarray:
+    """Seeded random weights of moderate size (|t| of a few eV at bond length); c symmetric in the pair."""
+    ns, F, Nb, Hd = dims
+    rng = np.random.Generator(np.random.PCG64(seed))
+    c = rng.normal(0.0, 1.0, (ns, ns, F, Nb)) / np.sqrt(Nb)
+    c = 0.5 * (c + c.transpose(1, 0, 2, 3))
+    def layer(out_dim, scale):
+        return (rng.normal(0.0, 1.0, (Hd, F)) / np.sqrt(F), rng.normal(0.0, 0.3, Hd),
+                rng.normal(0.0, scale, (out_dim, Hd)) / np.sqrt(Hd), rng.normal(0.0, 0.1, out_dim))
+    env = layer(F, 1.0)
+    hop = layer(1, 4.0)
+    ons = [layer(1, 1.0) for _ in range(ns)]
+    return mlp_pack(c, env, hop, ons)
