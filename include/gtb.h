@@ -253,6 +253,29 @@ int gtb_sk_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* spe
                        const double box[3], const int32_t pbc[3], const gtb_sk_model* model,
                        gtb_ell* H, int32_t* status, void* stream);
 
+/* ---- environment-dependent Hamiltonian from the descriptor + MLPs of Eq. 2 ----
+ * One orbital per atom.  With f_c(r) = 1/2 [1 + cos(pi r/r_cut)] (reading E1; the paper's "smooth
+ * cutoff function" is not printed), x = 2 (r/r_cut - 1)^2 - 1:
+ *   f_k(r) = 1/2 [T_k(x) + 1] f_c(r), k = 0..Nb-1;   C_n(r_ij) = sum_k c[s_i][s_j][n][k] f_k(r_ij), n = 0..F-1;
+ *   v_i = sum_{j in N(i)} C(r_ij);   e_ij = C(r_ij) * MLP_e(v_i + v_j)  (element-wise);
+ *   t_ij = MLP_lambda(e_ij);   eps_i = MLP_{s_i}(v_i);   MLP(x) = W2 silu(W1 x + b1) + b2.
+ * weights: DEVICE blob of gtb_mlp_weight_count() doubles, laid out as
+ *   c [ns][ns][F][Nb] | MLP_e: W1 [Hd][F], b1 [Hd], W2 [F][Hd], b2 [F] |
+ *   MLP_lambda: W1 [Hd][F], b1 [Hd], W2 [Hd], b2 [1] | per species s: W1 [Hd][F], b1 [Hd], W2 [Hd], b2 [1].
+ * Instantiated sizes (F, Nb, Hd): (8, 8, 16), (4, 4, 8), (16, 8, 32); others -> GTB_ERR_INVALID_ARG. */
+typedef struct gtb_mlp_model {
+  int32_t n_species, n_features, n_basis, n_hidden;
+  double r_cut;
+  const double* weights; /* DEVICE */
+} gtb_mlp_model;
+size_t gtb_mlp_weight_count(int32_t n_species, int32_t n_features, int32_t n_basis, int32_t n_hidden);
+/* ASYNC.  H->cols must hold the neighbour lists (e.g. from gtb_build_hamiltonian with the same
+ * cutoff <= r_cut); H->vals and, if non-NULL, H->diag are overwritten (padding slots: 0).
+ * v: DEVICE [n][F], receives the node features.  *status (DEVICE) non-zero: species out of range. */
+int gtb_mlp_hamiltonian(const gtb_mlp_model* m, const double* pos, const int32_t* species,
+                        const double box[3], const int32_t pbc[3], gtb_ell* H, double* v,
+                        int32_t* status, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

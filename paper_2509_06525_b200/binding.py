@@ -32,7 +32,7 @@ EXPORTS = (
     "gtb_kpm_last_loop_ms", "gtb_dos", "gtb_jackson",
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
-    "gtb_sk_hamiltonian",
+    "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
 )
 
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
@@ -441,3 +441,37 @@ def sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc,
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "sk_hamiltonian", "species index out of range")
     return H
+
+
+# ---------------------------------------------------------------- descriptor + MLP Hamiltonian (Eq. 2, NEXT-3)
+class _MlpModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("n_features", C.c_int32), ("n_basis", C.c_int32),
+                ("n_hidden", C.c_int32), ("r_cut", C.c_double), ("weights", C.c_void_p)]
+
+
+def mlp_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, dims, r_cut: float,
+                    weights: torch.Tensor, with_diag: bool = True, return_v: bool = False):
+    """H on the neighbour lists of `nbr` (its cols are shared, not copied) with t_ij, eps_i from Eq. 2."""
+    ns, F, Nb, Hd = dims
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    weights = _dev(weights, torch.float64, "weights")
+    lib().gtb_mlp_weight_count.restype = C.c_size_t
+    need = int(lib().gtb_mlp_weight_count(C.c_int32(ns), C.c_int32(F), C.c_int32(Nb), C.c_int32(Hd)))
+    if weights.numel() != need:
+        raise GtbError(ERR_INVALID_ARG, "mlp_hamiltonian", f"weight blob has {weights.numel()} doubles, {need} expected")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    dev = pos.device
+    H = Ell(nbr.n, nbr.width, nbr.cols, torch.empty((nbr.width, nbr.n), dtype=torch.float64, device=dev),
+            torch.empty(nbr.n, dtype=torch.float64, device=dev) if with_diag else None)
+    v = torch.empty((nbr.n, F), dtype=torch.float64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    model = _MlpModel(ns, F, Nb, Hd, r_cut, weights.data_ptr())
+    hc = H._c()
+    st = lib().gtb_mlp_hamiltonian(C.byref(model), _ptr(pos), _ptr(species), C.c_void_p(box_h.ctypes.data),
+                                   C.c_void_p(pbc_h.ctypes.data), C.byref(hc), _ptr(v), _ptr(status), _stream())
+    _check(st, "mlp_hamiltonian")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "mlp_hamiltonian", "species index out of range")
+    return (H, v) if return_v else H
