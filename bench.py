@@ -34,6 +34,7 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
+HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
 ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom) or "sp" (s, px, py, pz)
 VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in hbar/eV
 
@@ -122,12 +123,15 @@ def _oracle_step(w, inp, energies_of):
     t0 = time.perf_counter()
     H = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0,
                                  w.r0, w.beta, inp.onsite_shift, method=1, with_diag=w.use_diag)
+    if HOPPING == "mlp":
+        H = oracle.mlp_hamiltonian(H, inp.pos, inp.species, inp.box, inp.pbc, W.MLP_DIMS,
+                                   max(2.0, 1.05 * w.cutoff), W.mlp_weights(), with_diag=True)
     if ORBITALS == "sp":
         ns = len(w.onsite)
         H = oracle.sk_hamiltonian(H, inp.pos, inp.species, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
                                   W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
                                   onsite_shift=inp.onsite_shift)
-    if w.a is None or ORBITALS == "sp":
+    if w.a is None or ORBITALS == "sp" or HOPPING == "mlp":
         lo, hi = oracle.spectral_bounds(H)
         a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
     else:
@@ -250,16 +254,25 @@ def run_ours(args):
     mu = torch.empty(w.M, dtype=torch.float64, device=dev)
     h_rho = torch.empty(w.n_energies, dtype=torch.float64).pin_memory()
     state = {}
+    if HOPPING == "mlp":
+        state["mlp_w"] = torch.from_numpy(W.mlp_weights()).to(dev)
 
     def step(pos, spec, shift):
         H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
                                   w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
+        if HOPPING == "mlp":   # Eq. 2: descriptor + MLPs on the neighbour lists just built
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            H = gtb.mlp_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.MLP_DIMS, max(2.0, 1.05 * w.cutoff),
+                                    state["mlp_w"], with_diag=True)
+            e1.record()
+            state["mlp_events"] = (e0, e1)
         if ORBITALS == "sp":   # Slater-Koster s,p blocks on the neighbour lists just built
             ns = len(w.onsite)
             H = gtb.sk_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
                                    W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
                                    onsite_shift=shift)
-        if w.a is None or ORBITALS == "sp":
+        if w.a is None or ORBITALS == "sp" or HOPPING == "mlp":
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
@@ -350,6 +363,10 @@ def run_ours(args):
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": h_rho.numel() * 8, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": launches, "roofline": roofline, "clocks": clk.summary()}
+    if HOPPING == "mlp":
+        torch.cuda.synchronize()
+        line["config"]["hopping"] = "descriptor + MLPs of Eq. 2, F, Nb, Hd = %d, %d, %d (synthetic weights)" % W.MLP_DIMS[1:]
+        line["mlp_hamiltonian_ms"] = state["mlp_events"][0].elapsed_time(state["mlp_events"][1])
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             s = _cpu_sample(w)
@@ -504,11 +521,16 @@ def main():
     p.add_argument("--quantity", default="dos", choices=["dos", "vac"],
                    help="dos: the headline path (Eq. 4); vac: the VAC conductivity (Eq. 3, NEXT-1)")
     p.add_argument("--time-steps", type=int, default=24, help="vac: points of the time grid (dt = 0.1 fs)")
+    p.add_argument("--hopping", default="analytic", choices=["analytic", "mlp"],
+                   help="analytic: t(r) of the configs; mlp: descriptor + MLPs of Eq. 2 with synthetic weights (NEXT-3)")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS
+    global ORBITALS, HOPPING
     ORBITALS = args.orbitals
+    HOPPING = args.hopping
+    if args.hopping == "mlp" and (args.orbitals == "sp" or args.quantity == "vac"):
+        raise SystemExit("bench.py: --hopping mlp is wired for --orbitals pz --quantity dos")
     if args.orbitals == "sp" and args.quantity == "vac":
         raise SystemExit("bench.py: --orbitals sp is wired for --quantity dos only")
     if args.quantity == "vac" and not args.moments:
