@@ -337,7 +337,10 @@ def run_ours(args):
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
-    k7_name = ("cheb_orb4_kernel (K7b: fused Chebyshev pass on 4x4 orbital blocks)" if orb4 else
+    small = (not orb4 and w.R in (2, 4, 8) and n_orb * (w.R // 2) <= 148 * 4 * 256
+             and os.environ.get("GTB_K7_SMALL", "1") != "0" and os.environ.get("GTB_K7_SWEEP", "0") == "0")
+    k7_name = ("cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
+               "cheb_orb4_kernel (K7b: fused Chebyshev pass on 4x4 orbital blocks)" if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
                if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
                else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")

@@ -14,6 +14,8 @@
 // and one 256-bit load for a pair of vectors), streams phi_{n-1}, writes phi_{n+1} over it, and
 // accumulates <phi_n|phi_n> and Re<phi_{n+1}|phi_n> in registers -> warp shuffles -> one slot per
 // block.  H is read once per pass for all R vectors.
+#include <cooperative_groups.h>
+
 #include <cmath>
 #include <cstdlib>
 
@@ -386,6 +388,95 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
       s2 += red[w][1];
     }
     a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+// ---- K7p: all passes of a small system in ONE cooperative launch ----------------------------------
+// Config 1 (2 304 atoms) is 128 passes of ~0.5 MB each: as separate launches it runs at the launch
+// cadence (4-5 us per pass), not at any memory roof.  When every element of phi has its own resident
+// thread (n * T <= SMs x occupancy x 256), one cooperative kernel runs the first pass and all S - 1
+// recursion passes with a grid-wide barrier between them; phi never leaves L2.  Gathers bypass L1
+// (ld.global.cg): the vectors are rewritten by other SMs between passes.  Same arithmetic order per
+// element and the same per-(pass, block) partial sums as K6/K7.
+__device__ __forceinline__ Vec<4> load_l2(const double* p) {
+  Vec<4> r;
+  asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3])
+               : "l"(p)
+               : "memory");
+  return r;
+}
+
+template <int LOG2T, bool kDiag>
+__global__ void __launch_bounds__(kBlock) cheb_small_kernel(const StepArgs a, const int S,
+                                                            const double inv_a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const int64_t n = a.n;
+  const int64_t total = n * T;
+  const int width = a.width;
+  const double b = a.b;
+  const int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x;   // one element per thread
+  const bool live = e < total;
+  const int64_t row = live ? (e >> LOG2T) : 0;
+  const int64_t t = e - row * T;
+  const double* cur = a.phi_cur;
+  double* io = a.phi_io;
+  __shared__ double red[kBlock / 32][2];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int k = 0; k < S; ++k) {
+    const double scale = k == 0 ? inv_a : 2.0 * inv_a;
+    double s1 = 0.0, s2 = 0.0;
+    if (live) {
+      const double* xt = cur + t * VW;
+      Vec<VW> acc, prev;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = prev.v[q] = 0.0;
+      if (k > 0) prev = load_l2(io + e * VW);
+      const Vec<VW> own = load_l2(cur + e * VW);
+#pragma unroll 4
+      for (int s = 0; s < width; ++s) {
+        const int64_t c = __ldg(a.cols + (size_t)s * n + row);
+        const double v = __ldg(a.vals + (size_t)s * n + row);
+        const Vec<VW> x = load_l2(xt + c * T * VW);
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc.v[q] = fma(v, x.v[q], acc.v[q]);
+      }
+      if (kDiag) {
+        const double d = __ldg(a.diag + row);
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc.v[q] = fma(d, own.v[q], acc.v[q]);
+      }
+      Vec<VW> y;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
+        if (k > 0) y.v[q] -= prev.v[q];
+        s1 = fma(own.v[q], own.v[q], s1);
+        s2 = fma(y.v[q], own.v[q], s2);
+      }
+      store_stream<VW>(io + e * VW, y);
+    }
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if (lane == 0) {
+      red[wid][0] = s1;
+      red[wid][1] = s2;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int w = 1; w < kBlock / 32; ++w) {
+        s1 += red[w][0];
+        s2 += red[w][1];
+      }
+      a.partial[(size_t)k * kMaxGrid + blockIdx.x] = make_double2(s1, s2);
+    }
+    grid.sync();  // every phi_{k+1} element is written and visible before anyone gathers it
+    const double* tmp = cur;
+    cur = io;
+    io = const_cast<double*>(tmp);
   }
 }
 
@@ -1060,6 +1151,22 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
       halo_kernel<<<fill_grid(n * H->width), kBlock, 0, st>>>(H->cols, n, H->width, w.status + 2);
       GTB_LAUNCHED();
     }
+    // K7p: every element of phi on its own resident thread -> all passes in one cooperative launch
+    int small_grid = 0;
+    void* small_fn = nullptr;
+    if (!blocked && !sweep && plan.vw == 4 && S >= 2 && env_int("GTB_K7_SMALL", 1) != 0) {
+      const bool dg = H->diag != nullptr;
+      small_fn = plan.T == 1 ? (dg ? (void*)cheb_small_kernel<0, true> : (void*)cheb_small_kernel<0, false>)
+               : plan.T == 2 ? (dg ? (void*)cheb_small_kernel<1, true> : (void*)cheb_small_kernel<1, false>)
+                             : (dg ? (void*)cheb_small_kernel<2, true> : (void*)cheb_small_kernel<2, false>);
+      int dev = 0, sms = kSmCount, per_sm = 0, coop = 0;
+      GTB_CUDA_TRY(cudaGetDevice(&dev));
+      GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      GTB_CUDA_TRY(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_fn, kBlock, 0));
+      const int64_t blocks = (n * plan.T + kBlock - 1) / kBlock;
+      if (coop && blocks <= (int64_t)sms * per_sm && blocks <= kMaxGrid) small_grid = (int)blocks;
+    }
     double* cur = w.phi_a;   // phi_k
     double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
     if (mode == 0) {
@@ -1071,6 +1178,22 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     }
     GTB_LAUNCHED();
     StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, cur, io, 1.0 / a, b, w.partial};
+    if (small_grid > 0) {  // K7p: K6 and all K7 passes in one launch
+      if (last_batch) GTB_CUDA_TRY(cudaEventRecord(g_timer.beg, st));
+      int S_arg = S;
+      double inv_a = 1.0 / a;
+      void* args[] = {&sa, &S_arg, &inv_a};
+      GTB_CUDA_TRY(cudaLaunchCooperativeKernel(small_fn, dim3(small_grid), dim3(kBlock), args, 0, st));
+      count_launch();
+      if (last_batch) {
+        GTB_CUDA_TRY(cudaEventRecord(g_timer.end, st));
+        g_timer.passes = S;
+        g_timer.armed = true;
+      }
+      reduce_partials_kernel<<<S, 128, 0, st>>>(w.partial, kMaxGrid, small_grid, w.sums);
+      GTB_LAUNCHED();
+      continue;
+    }
     launch_step(plan, true, sa, st);  // K6: phi_1, <phi_0|phi_0>, Re<phi_1|phi_0>
     GTB_LAUNCHED();
     if (last_batch) GTB_CUDA_TRY(cudaEventRecord(g_timer.beg, st));

@@ -265,6 +265,29 @@ def test_two_step_sweep_matches_oracle(monkeypatch, key, nx, ny, kw, R, chunk, s
     assert np.abs(got - one).max() <= 1e-13          # same vectors, another summation order
 
 
+# K7p: small systems run all passes in one cooperative launch (default); GTB_K7_SMALL=0 takes the
+# per-pass launches.  Both must agree with the oracle and with each other.
+@pytest.mark.parametrize("key,nx,ny,kw,R", [("c1", 24, 24, {}, 4), ("c2", 37, 23, {}, 8), ("c3", 33, 31, {}, 2),
+                                             ("c4", 48, 21, {"stripe": 6}, 8), ("c5", 57, 43, {}, 2)])
+@pytest.mark.parametrize("M", [2, 3, 64, 257])
+def test_single_launch_path_matches_oracle_and_per_pass_path(monkeypatch, key, nx, ny, kw, R, M):
+    w, inp = _small(key, nx, ny, kw)
+    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
+    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
+    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
+    ref = oracle.kpm_moments(Ho, a, b, M, R, 9, mode=0, algo=0)
+    l0 = gtb.launch_count()
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True).cpu().numpy()
+    used = gtb.launch_count() - l0
+    assert np.abs(got - ref).max() <= 1e-12
+    monkeypatch.setenv("GTB_K7_SMALL", "0")
+    l0 = gtb.launch_count()
+    per_pass = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True).cpu().numpy()
+    assert np.abs(got - per_pass).max() <= 1e-13
+    if M >= 64:
+        assert used < (gtb.launch_count() - l0) // 4      # the single-launch path really was taken
+
+
 @pytest.mark.parametrize("drop", [1, 2, 3])
 def test_atom_count_not_a_multiple_of_four_takes_the_register_path(drop):
     # bulk copies need 16-byte aligned slot rows (n % 4 == 0); any other n must still be exact
