@@ -314,3 +314,30 @@ def mlp_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, weight
     _check(lib().gtbo_mlp_hamiltonian(C.byref(m), _p(pos), _p(species), _p(box), _p(pbc), C.byref(hc),
                                       _p(v)), "mlp_hamiltonian")
     return (H, v) if return_v else H
+
+
+# ---------------------------------------------------------------- Slater-Koster s,p,d blocks (NEXT-2)
+class _SpdModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite_s", C.c_void_p), ("onsite_p", C.c_void_p),
+                ("onsite_d", C.c_void_p), ("sk", C.c_void_p), ("r0", C.c_double), ("beta", C.c_double),
+                ("onsite_shift", C.c_void_p)]
+
+
+def spd_hamiltonian(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, onsite_d, sk, r0: float = 1.0,
+                    beta: float = 0.0, onsite_shift=None, with_diag: bool = True) -> Ell:
+    """Scalar ELL over the 9n orbitals (s, p, d per atom) from the neighbour lists of `nbr`."""
+    pos, species, box, pbc = _f64(pos), _i32(species), _f64(box), _i32(pbc)
+    es, ep, ed = (_f64(x).reshape(-1) for x in (onsite_s, onsite_p, onsite_d))
+    sk = _f64(sk).reshape(-1)
+    ns = es.shape[0]
+    assert sk.shape[0] == ns * ns * 10
+    shift = _f64(onsite_shift) if onsite_shift is not None else None
+    n, K = nbr.n, nbr.width
+    H = Ell(9 * n, 9 * K, np.zeros((9 * K, 9 * n), dtype=np.int32), np.zeros((9 * K, 9 * n)),
+            np.zeros(9 * n) if with_diag else None)
+    model = _SpdModel(ns, es.ctypes.data, ep.ctypes.data, ed.ctypes.data, sk.ctypes.data, r0, beta,
+                      shift.ctypes.data if shift is not None else None)
+    nc, hc = nbr._c(), H._c()
+    _check(lib().gtbo_spd_hamiltonian(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
+                                      C.byref(model), C.byref(hc)), "spd_hamiltonian")
+    return H

@@ -11,7 +11,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["gtbo_hamiltonian.cpp", "gtbo_kpm.cpp", "gtbo_vac.cpp", "gtbo_sk.cpp", "gtbo_mlp.cpp"]
+SOURCES = ["gtbo_hamiltonian.cpp", "gtbo_kpm.cpp", "gtbo_vac.cpp", "gtbo_sk.cpp", "gtbo_mlp.cpp", "gtbo_spd.cpp"]
 LIB = os.path.join(HERE, "libgtbo.so")
 
 

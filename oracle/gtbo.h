@@ -171,6 +171,23 @@ int gtbo_mlp_descriptor(const gtbo_mlp_model* m, int32_t si, int32_t sj, double 
 int gtbo_mlp_hamiltonian(const gtbo_mlp_model* m, const double* pos, const int32_t* species,
                          const double box[3], const int32_t pbc[3], gtbo_ell* H, double* v_out);
 
+/* --- Slater-Koster blocks for the s,p,d basis (9 orbitals; NEXT-2) */
+/* Orbital order s, px, py, pz, dxy, dyz, dzx, dx2-y2, dz2; construction: top of gtbo_spd.cpp. */
+typedef struct gtbo_spd_model {
+  int32_t n_species;
+  const double* onsite_s;     /* [n_species] eV */
+  const double* onsite_p;
+  const double* onsite_d;
+  const double* sk;           /* [n_species][n_species][10]: ss_s, sp_s, pp_s, pp_p, sd_s, pd_s, pd_p, dd_s, dd_p, dd_d */
+  double r0;
+  double beta;
+  const double* onsite_shift; /* [n] or NULL */
+} gtbo_spd_model;
+/* H: caller-allocated scalar ELL over 9n orbitals, width 9*nbr->width, diag [9n] or NULL. */
+int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* species,
+                         const double box[3], const int32_t pbc[3],
+                         const gtbo_spd_model* model, gtbo_ell* H);
+
 #ifdef __cplusplus
 }
 #endif
