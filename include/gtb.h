@@ -57,7 +57,8 @@ enum {
   GTB_ERR_INDEX_RANGE = -7    /* n too large for int32 indices                     */
 };
 
-#define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian */
+#define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian  (4 orbitals) */
+#define GTB_MODE_ORB9 32 /* ... from gtb_spd_hamiltonian (9 orbitals per atom)                           */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
 
@@ -132,9 +133,9 @@ int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, doubl
  *         R_batch at a time (each pass of H serves R_batch vectors).
  * mode 1: exact trace over all n basis vectors e_i (R_total and seed ignored),
  *         R_batch of them per pass.
- * mode | GTB_MODE_ORB4: the caller promises that H is the orbital-blocked matrix written by
- *         gtb_sk_hamiltonian (4 orbitals per atom); the fused pass then works on whole 4x4
- *         blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
+ * mode | GTB_MODE_ORB4 (or GTB_MODE_ORB9): the caller promises that H is the orbital-blocked matrix
+ *         written by gtb_sk_hamiltonian (4 orbitals per atom; gtb_spd_hamiltonian: 9); the fused pass
+ *         then works on whole 4x4 (9x9) blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
  *         when R_batch is not 2, 4 or 8.  A matrix without that structure gives wrong results.
  * R_batch: 1..64.  R_batch in {2,4,8} takes the 256-bit vector path.
  * ASYNC.  mu is DEVICE [M].  Workspace: gtb_kpm_workspace_bytes(n, M, R_batch). */
@@ -275,6 +276,31 @@ size_t gtb_mlp_weight_count(int32_t n_species, int32_t n_features, int32_t n_bas
 int gtb_mlp_hamiltonian(const gtb_mlp_model* m, const double* pos, const int32_t* species,
                         const double box[3], const int32_t pbc[3], gtb_ell* H, double* v,
                         int32_t* status, void* stream);
+
+/* ---- Slater-Koster blocks for the s, p, d basis of the paper's runs (reading S4) ----
+ * 9 orbitals per atom in the order s, px, py, pz, dxy, dyz, dzx, dx2-y2, dz2.  Two-centre integrals are
+ * diagonal in the bond frame (e1, e2, u), u = (x_j - x_i)/r; with c_{a,m} the coefficient of lab orbital a on
+ * the frame orbital m (sigma, pi1, pi2, delta1, delta2):
+ *   E_ab = sum_m c_{a,m} V_{l_a l_b |m|} c_{b,m},  times (-1)^{l_a + l_b} when l_a > l_b,
+ * V = { ss_sigma, sp_sigma, pp_sigma, pp_pi, sd_sigma, pd_sigma, pd_pi, dd_sigma, dd_pi, dd_delta } per
+ * species pair, each times exp(-beta (r/r0 - 1)); onsite eps_s, eps_p, eps_d (+ onsite_shift[i]).
+ * Output: scalar ELL over the 9n orbitals, laid out as gtb_sk_hamiltonian's with 9 in place of 4. */
+typedef struct gtb_spd_model {
+  int32_t n_species;
+  const double* onsite_s;     /* HOST [n_species] eV */
+  const double* onsite_p;
+  const double* onsite_d;
+  const double* sk;           /* HOST [n_species][n_species][10] eV */
+  double r0;
+  double beta;
+  const double* onsite_shift; /* DEVICE [n] or NULL */
+} gtb_spd_model;
+size_t gtb_spd_workspace_bytes(void);
+/* SYNC on the parameter upload, then ASYNC.  H->n = 9 n, H->width = 9 nbr->width, H->diag [9 n] or NULL.
+ * Workspace: gtb_spd_workspace_bytes() (holds the parameter block while the kernels run). */
+int gtb_spd_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* species,
+                        const double box[3], const int32_t pbc[3], const gtb_spd_model* model,
+                        gtb_ell* H, int32_t* status, void* ws, size_t ws_bytes, void* stream);
 
 #ifdef __cplusplus
 }

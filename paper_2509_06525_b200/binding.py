@@ -33,8 +33,10 @@ EXPORTS = (
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
+    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian",
 )
 
+MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
 
@@ -475,3 +477,42 @@ def mlp_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "mlp_hamiltonian", "species index out of range")
     return (H, v) if return_v else H
+
+
+# ---------------------------------------------------------------- Slater-Koster s,p,d blocks (NEXT-2)
+class _SpdModel(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("onsite_s", C.c_void_p), ("onsite_p", C.c_void_p),
+                ("onsite_d", C.c_void_p), ("sk", C.c_void_p), ("r0", C.c_double), ("beta", C.c_double),
+                ("onsite_shift", C.c_void_p)]
+
+
+def spd_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, onsite_s, onsite_p,
+                    onsite_d, sk, r0: float = 1.0, beta: float = 0.0,
+                    onsite_shift: Optional[torch.Tensor] = None, with_diag: bool = True) -> Ell:
+    """Scalar ELL over the 9n orbitals (s, p, d per atom) from the neighbour lists of `nbr`."""
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    es, ep, ed = (np.ascontiguousarray(x, dtype=np.float64).reshape(-1) for x in (onsite_s, onsite_p, onsite_d))
+    ns = es.shape[0]
+    sk_h = _host_f64(sk, ns * ns * 10)
+    if onsite_shift is not None:
+        onsite_shift = _dev(onsite_shift, torch.float64, "onsite_shift")
+    n, K, dev = nbr.n, nbr.width, pos.device
+    H = Ell(9 * n, 9 * K, torch.empty((9 * K, 9 * n), dtype=torch.int32, device=dev),
+            torch.empty((9 * K, 9 * n), dtype=torch.float64, device=dev),
+            torch.empty(9 * n, dtype=torch.float64, device=dev) if with_diag else None)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    lib().gtb_spd_workspace_bytes.restype = C.c_size_t
+    ws = workspace(int(lib().gtb_spd_workspace_bytes()), dev)
+    model = _SpdModel(ns, es.ctypes.data, ep.ctypes.data, ed.ctypes.data, sk_h.ctypes.data, r0, beta,
+                      onsite_shift.data_ptr() if onsite_shift is not None else None)
+    nc, hc = nbr._c(), H._c()
+    st = lib().gtb_spd_hamiltonian(C.byref(nc), _ptr(pos), _ptr(species), C.c_void_p(box_h.ctypes.data),
+                                   C.c_void_p(pbc_h.ctypes.data), C.byref(model), C.byref(hc), _ptr(status),
+                                   _ptr(ws), C.c_size_t(ws.numel()), _stream())
+    _check(st, "spd_hamiltonian")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "spd_hamiltonian", "species index out of range")
+    return H

@@ -40,8 +40,9 @@ struct StepPlan {
 // dot = false: the DOS pass (dot products with phi_n itself); dot = true: with StepArgs::dot_with.
 int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p);
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st);
-// K7b plan for an orbital-blocked matrix (gtb_sk_hamiltonian's); false when H or R does not fit
-bool make_plan_orb4(const gtb_ell* H, int R, bool dot, StepPlan* p);
+// K7b plan for an orbital-blocked matrix (B = 4: gtb_sk_hamiltonian's, B = 9: gtb_spd_hamiltonian's);
+// false when H or R does not fit
+bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, StepPlan* p);
 
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);

@@ -570,6 +570,91 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
   }
 }
 
+// ---- K7b9: the blocked pass for 9 orbitals per atom (s, p, d) ---------------------------------------
+// Same idea as K7b with the block streamed one column at a time: per neighbour one column index, then
+// for each of the 9 neighbour orbitals nu one gather of its 256-bit element and the 9 block entries
+// E[mu][nu] (72 contiguous bytes, broadcast across the T threads of the atom), 36 FMAs.  The 9 x VW
+// accumulators stay in registers.
+template <int LOG2T, bool kFirst, bool kDiag, bool kDotL>
+__global__ void __launch_bounds__(kBlock, 2) cheb_orb9_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int B = 9;
+  const int64_t N = a.n;
+  const int64_t n_atoms = N / B;
+  const int K = a.width / B;
+  const int64_t total = n_atoms * T;
+  const double scale = a.scale, b = a.b;
+  constexpr int64_t kOrb = (int64_t)T * VW;
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t i = e >> LOG2T;
+    const int64_t t = e - i * T;
+    const double* xt = a.phi_cur + t * VW;
+    const int32_t* cp = a.cols + B * i;
+    const double* vp = a.vals + B * i;
+    Vec<VW> acc[B];
+#pragma unroll
+    for (int mu = 0; mu < B; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    int64_t j = K > 0 ? (int64_t)(__ldg(cp) / B) : 0;
+    for (int k = 0; k < K; ++k) {
+      const int64_t jn = k + 1 < K ? (int64_t)(__ldg(cp + (size_t)(B * (k + 1)) * N) / B) : 0;
+#pragma unroll 3
+      for (int nu = 0; nu < B; ++nu) {
+        const Vec<VW> x = load_gather<VW>(xt + (B * j + nu) * kOrb);
+        const double* col = vp + (size_t)(B * k + nu) * N;
+#pragma unroll
+        for (int mu = 0; mu < B; ++mu) {
+          const double h = __ldg(col + mu);
+#pragma unroll
+          for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(h, x.v[q], acc[mu].v[q]);
+        }
+      }
+      j = jn;
+    }
+#pragma unroll
+    for (int mu = 0; mu < B; ++mu) {
+      const int64_t at = (B * i + mu) * kOrb + t * VW;
+      const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
+      Vec<VW> prev, with;
+      if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+      if (kDotL) with = load_stream<VW>(a.dot_with + at);
+      const double dg = kDiag ? __ldg(a.diag + B * i + mu) : 0.0;
+      Vec<VW> y;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        double h = acc[mu].v[q];
+        if (kDiag) h = fma(dg, own.v[q], h);
+        y.v[q] = (h - b * own.v[q]) * scale;
+        if (!kFirst) y.v[q] -= prev.v[q];
+        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+      }
+      store_stream<VW>(a.phi_io + at, y);
+    }
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
 // ---- K7s: two Chebyshev steps per HBM sweep (temporal blocking through L2) -----------------------
 // One pass of K7 moves 12K + 48R bytes per atom through HBM for one step.  Here one launch advances
 // every row by TWO steps: rows are cut into chunks of `chunk_rows`; task (j, l) = step l (0 or 1)
@@ -903,24 +988,31 @@ int env_int(const char* name, int dflt) {
 }  // namespace
 
 template <int LOG2T, bool DOT>
-void pick_orb4_dot(bool diag, StepPlan* p) {
-  p->first = diag ? cheb_orb4_kernel<LOG2T, true, true, DOT> : cheb_orb4_kernel<LOG2T, true, false, DOT>;
-  p->next = diag ? cheb_orb4_kernel<LOG2T, false, true, DOT> : cheb_orb4_kernel<LOG2T, false, false, DOT>;
+void pick_orb_dot(int B, bool diag, StepPlan* p) {
+  if (B == 4) {
+    p->first = diag ? cheb_orb4_kernel<LOG2T, true, true, DOT> : cheb_orb4_kernel<LOG2T, true, false, DOT>;
+    p->next = diag ? cheb_orb4_kernel<LOG2T, false, true, DOT> : cheb_orb4_kernel<LOG2T, false, false, DOT>;
+  } else {
+    p->first = diag ? cheb_orb9_kernel<LOG2T, true, true, DOT> : cheb_orb9_kernel<LOG2T, true, false, DOT>;
+    p->next = diag ? cheb_orb9_kernel<LOG2T, false, true, DOT> : cheb_orb9_kernel<LOG2T, false, false, DOT>;
+  }
 }
 template <int LOG2T>
-void pick_orb4(bool diag, bool dot, StepPlan* p) {
-  if (dot) pick_orb4_dot<LOG2T, true>(diag, p);
-  else pick_orb4_dot<LOG2T, false>(diag, p);
+void pick_orb(int B, bool diag, bool dot, StepPlan* p) {
+  if (dot) pick_orb_dot<LOG2T, true>(B, diag, p);
+  else pick_orb_dot<LOG2T, false>(B, diag, p);
 }
 
-// K7b plan: one thread per (atom, 256-bit element); falls back (returns false) when H or R does not fit
-bool make_plan_orb4(const gtb_ell* H, int R, bool dot, StepPlan* p) {
-  if (H->n % 4 || H->width % 4 || H->width == 0 || (R != 2 && R != 4 && R != 8) ||
-      (reinterpret_cast<uintptr_t>(H->vals) & 31u) || (reinterpret_cast<uintptr_t>(H->diag) & 31u))
+// K7b plan (B = 4 or 9 orbitals per atom): one thread per (atom, 256-bit element); false when H or R
+// does not fit and the scalar kernels must be used
+bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, StepPlan* p) {
+  if ((B != 4 && B != 9) || H->n % B || H->width % B || H->width == 0 || (R != 2 && R != 4 && R != 8) ||
+      (B == 4 && ((reinterpret_cast<uintptr_t>(H->vals) & 31u) || (reinterpret_cast<uintptr_t>(H->diag) & 31u))))
     return false;
-  if (R == 2) { pick_orb4<0>(H->diag != nullptr, dot, p); p->T = 1; }
-  else if (R == 4) { pick_orb4<1>(H->diag != nullptr, dot, p); p->T = 2; }
-  else { pick_orb4<2>(H->diag != nullptr, dot, p); p->T = 4; }
+  const bool diag = H->diag != nullptr;
+  if (R == 2) { pick_orb<0>(B, diag, dot, p); p->T = 1; }
+  else if (R == 4) { pick_orb<1>(B, diag, dot, p); p->T = 2; }
+  else { pick_orb<2>(B, diag, dot, p); p->T = 4; }
   p->vw = 4;
   p->stages = 0;
   int dev = 0, sms = kSmCount, per_sm = 0;
@@ -929,7 +1021,7 @@ bool make_plan_orb4(const gtb_ell* H, int R, bool dot, StepPlan* p) {
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0) != cudaSuccess)
     return false;
   per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
-  const int64_t total = H->n / 4 * p->T;
+  const int64_t total = H->n / B * p->T;
   p->grid = (int)std::max<int64_t>(1, std::min<int64_t>((total + kBlock - 1) / kBlock, (int64_t)sms * per_sm));
   return true;
 }
@@ -1099,9 +1191,11 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
                                size_t ws_bytes, void* stream) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
-  if (mode_flags & ~(1 | GTB_MODE_ORB4)) return GTB_ERR_INVALID_ARG;
+  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9)) ||
+      ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)))
+    return GTB_ERR_INVALID_ARG;
   const int32_t mode = mode_flags & 1;
-  const bool orb4 = (mode_flags & GTB_MODE_ORB4) != 0;
+  const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   if (!mu || M <= 0 || !(a > 0.0) || !std::isfinite(b) || R_batch <= 0 || R_batch > 64 ||
       (mode != 0 && mode != 1) || (mode == 0 && R_total <= 0))
     return GTB_ERR_INVALID_ARG;
@@ -1123,7 +1217,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    const bool blocked = orb4 && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb4(H, R, false, &plan);
+    const bool blocked = orb && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb(H, R, orb, false, &plan);
     if (!blocked) {
       rc = make_plan(H, R, false, &plan);
       if (rc != GTB_OK) return rc;

@@ -275,9 +275,11 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
                                void* stream) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
-  if (mode_flags & ~(1 | GTB_MODE_ORB4)) return GTB_ERR_INVALID_ARG;
+  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9)) ||
+      ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)))
+    return GTB_ERR_INVALID_ARG;
   const int32_t mode = mode_flags & 1;
-  const bool orb4 = (mode_flags & GTB_MODE_ORB4) != 0;
+  const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   if (!vvals || !C || M <= 0 || n_steps <= 0 || !(a > 0.0) || !std::isfinite(b) ||
       !std::isfinite(dt) || R_batch <= 0 || R_batch > 64 || (mode != 0 && mode != 1) ||
       (mode == 0 && R_total <= 0))
@@ -300,7 +302,7 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan, dplan;  // evolution passes (no bra) and moment passes (dot with psiL)
-    if (!(orb4 && make_plan_orb4(H, R, false, &plan) && make_plan_orb4(H, R, true, &dplan))) {
+    if (!(orb && make_plan_orb(H, R, orb, false, &plan) && make_plan_orb(H, R, orb, true, &dplan))) {
       rc = make_plan(H, R, false, &plan);
       if (rc != GTB_OK) return rc;
       rc = make_plan(H, R, true, &dplan);
