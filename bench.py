@@ -35,7 +35,8 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
 HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
-ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom) or "sp" (s, px, py, pz)
+ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom), "sp" (4) or "spd" (9)
+ORB_COUNT = {"pz": 1, "sp": 4, "spd": 9}
 VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in hbar/eV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
@@ -131,7 +132,12 @@ def _oracle_step(w, inp, energies_of):
         H = oracle.sk_hamiltonian(H, inp.pos, inp.species, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
                                   W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
                                   onsite_shift=inp.onsite_shift)
-    if w.a is None or ORBITALS == "sp" or HOPPING == "mlp":
+    elif ORBITALS == "spd":
+        ns = len(w.onsite)
+        H = oracle.spd_hamiltonian(H, inp.pos, inp.species, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
+                                   W.SK_ONSITE_P[:ns], W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42,
+                                   beta=w.beta, onsite_shift=inp.onsite_shift)
+    if w.a is None or ORBITALS != "pz" or HOPPING == "mlp":
         lo, hi = oracle.spectral_bounds(H)
         a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
     else:
@@ -171,8 +177,8 @@ def _cpu_sample(w: W.Workload) -> W.Workload:
     n = 4 * nx * ny
     width_guess = {1.95: 3, 2.65: 10, 4.0: 20}.get(w.cutoff, 10)
     budget = 4e9 * 8 / (width_guess + 5)     # updates that take ~20 s at ~2e8 upd/s for width 3
-    if ORBITALS == "sp":
-        budget /= 16                         # 4x the rows, 4x the width
+    if ORBITALS != "pz":
+        budget /= ORB_COUNT[ORBITALS] ** 2   # B x the rows, B x the width
     M = int(max(16, min(w.M, budget / (n * w.R))))
     return w.scaled(nx, ny, M=M)
 
@@ -202,7 +208,7 @@ def run_reference(args):
         inp = W.make_inputs(s)
         times = [_oracle_step(s, inp, W.energy_grid)[0] for _ in range(args.steps)]
         t = float(np.mean(times))
-        orb = 4 if ORBITALS == "sp" else 1
+        orb = ORB_COUNT[ORBITALS]
         value = orb * s.n_atoms * s.M * s.R / t
         sample = f"{s.name}: N={s.n_atoms} x {orb} orbitals, M={s.M}, R={s.R}, build+moments(direct)+dos"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
@@ -248,7 +254,7 @@ def run_ours(args):
 
     ws_build = gtb.workspace(gtb.build_workspace_bytes(n), dev)
     width = gtb.neighbor_width(d_pos, inp.box, inp.pbc, w.cutoff, ws=ws_build)
-    n_orb = 4 * n if ORBITALS == "sp" else n          # rows of H: the unit of the metric
+    n_orb = ORB_COUNT[ORBITALS] * n                   # rows of H: the unit of the metric
     ws_kpm = gtb.workspace(gtb.kpm_workspace_bytes(n_orb, w.M, w.R), dev)
     ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n_orb), dev)
     mu = torch.empty(w.M, dtype=torch.float64, device=dev)
@@ -272,12 +278,17 @@ def run_ours(args):
             H = gtb.sk_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
                                    W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
                                    onsite_shift=shift)
-        if w.a is None or ORBITALS == "sp" or HOPPING == "mlp":
+        elif ORBITALS == "spd":
+            ns = len(w.onsite)
+            H = gtb.spd_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
+                                    W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42, beta=w.beta,
+                                    onsite_shift=shift)
+        if w.a is None or ORBITALS != "pz" or HOPPING == "mlp":
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode=gtb.MODE_ORB4 if ORBITALS == "sp" else 0,
+        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode={"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0),
                         ws=ws_kpm, mu=mu)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
@@ -329,10 +340,11 @@ def run_ours(args):
     e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
-    orb4 = ORBITALS == "sp" and os.environ.get("GTB_K7_ORB4", "1") != "0" and w.R in (2, 4, 8)
+    orb4 = ORBITALS != "pz" and os.environ.get("GTB_K7_ORB4", "1") != "0" and w.R in (2, 4, 8)
+    B = ORB_COUNT[ORBITALS]
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
-    if orb4:   # per orbital row: K blocks of (4 B column + 128 B values) shared by 4 rows, + diag + vectors
-        per_atom = (H.width // 4) * 132 // 4 + (8 if H.diag is not None else 0) + 48 * w.R
+    if orb4:   # per orbital row: K blocks of (4 B column + 8 B^2 B values) shared by B rows, + diag + vectors
+        per_atom = (H.width // B) * (4 + 8 * B * B) // B + (8 if H.diag is not None else 0) + 48 * w.R
     bytes_per_launch = float(n_orb) * per_atom
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
@@ -340,7 +352,7 @@ def run_ours(args):
     small = (not orb4 and w.R in (2, 4, 8) and n_orb * (w.R // 2) <= 148 * 4 * 256
              and os.environ.get("GTB_K7_SMALL", "1") != "0" and os.environ.get("GTB_K7_SWEEP", "0") == "0")
     k7_name = ("cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
-               "cheb_orb4_kernel (K7b: fused Chebyshev pass on 4x4 orbital blocks)" if orb4 else
+               ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
                if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
                else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
@@ -374,7 +386,7 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             s = _cpu_sample(w)
             t, _ = _oracle_step(s, W.make_inputs(s), W.energy_grid)
-            orb = 4 if ORBITALS == "sp" else 1
+            orb = ORB_COUNT[ORBITALS]
             line["cpu_baseline"] = {
                 "value": orb * s.n_atoms * s.M * s.R / t, "unit": UNIT, "cores": _cores(), "kind": "oracle",
                 "sample": f"{s.name}: N={s.n_atoms} x {orb} orbitals, M={s.M}, R={s.R}, build+moments(direct)+dos, {t:.1f} s"}
@@ -526,16 +538,16 @@ def main():
     p.add_argument("--time-steps", type=int, default=24, help="vac: points of the time grid (dt = 0.1 fs)")
     p.add_argument("--hopping", default="analytic", choices=["analytic", "mlp"],
                    help="analytic: t(r) of the configs; mlp: descriptor + MLPs of Eq. 2 with synthetic weights (NEXT-3)")
-    p.add_argument("--orbitals", default="pz", choices=["pz", "sp"],
+    p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
     global ORBITALS, HOPPING
     ORBITALS = args.orbitals
     HOPPING = args.hopping
-    if args.hopping == "mlp" and (args.orbitals == "sp" or args.quantity == "vac"):
+    if args.hopping == "mlp" and (args.orbitals != "pz" or args.quantity == "vac"):
         raise SystemExit("bench.py: --hopping mlp is wired for --orbitals pz --quantity dos")
-    if args.orbitals == "sp" and args.quantity == "vac":
-        raise SystemExit("bench.py: --orbitals sp is wired for --quantity dos only")
+    if args.orbitals != "pz" and args.quantity == "vac":
+        raise SystemExit("bench.py: --orbitals sp/spd is wired for --quantity dos only")
     if args.quantity == "vac" and not args.moments:
         args.moments = 512
     if args.impl == "reference":

@@ -573,73 +573,106 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
 // ---- K7b9: the blocked pass for 9 orbitals per atom (s, p, d) ---------------------------------------
 // Same idea as K7b with the block streamed one column at a time: per neighbour one column index, then
 // for each of the 9 neighbour orbitals nu one gather of its 256-bit element and the 9 block entries
-// E[mu][nu] (72 contiguous bytes, broadcast across the T threads of the atom), 36 FMAs.  The 9 x VW
-// accumulators stay in registers.
-template <int LOG2T, bool kFirst, bool kDiag, bool kDotL>
+// E[mu][nu], 36 FMAs; the 9 x VW accumulators stay in registers.  The block columns of a warp's atoms
+// are one contiguous run (72 bytes per atom, atoms consecutive): the warp reads the run with coalesced
+// 64-bit loads one column ahead, parks it in its own slice of shared memory and every lane picks its
+// atom's 9 entries from there (conflict-free: stride 18 words) -- 72-byte-strided loads straight from
+// global memory cost 9 times the L1 wavefronts.
+template <int LOG2T, bool kFirst, bool kDiag, bool kDotL, bool kStage>
 __global__ void __launch_bounds__(kBlock, 2) cheb_orb9_kernel(const StepArgs a) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
   constexpr int B = 9;
+  constexpr int A = 32 / T;                 // atoms per warp
+  constexpr int NL = (B * A + 31) / 32;     // coalesced loads per lane per block column
+  __shared__ double s_col[kBlock / 32][kStage ? B * A : 1];
   const int64_t N = a.n;
   const int64_t n_atoms = N / B;
   const int K = a.width / B;
   const int64_t total = n_atoms * T;
   const double scale = a.scale, b = a.b;
   constexpr int64_t kOrb = (int64_t)T * VW;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  double* const sm = s_col[wid];
   double s1 = 0.0, s2 = 0.0;
-  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
-       e += (int64_t)gridDim.x * kBlock) {
-    const int64_t i = e >> LOG2T;
-    const int64_t t = e - i * T;
+  for (int64_t e0 = (int64_t)blockIdx.x * kBlock + wid * 32; e0 < total; e0 += (int64_t)gridDim.x * kBlock) {
+    const int64_t e = e0 + lane;
+    const bool live = e < total;
+    const int64_t i0 = e0 >> LOG2T;                                    // first atom of the warp
+    const int run = B * (int)min((int64_t)A, n_atoms - i0);            // doubles per block column
+    const int64_t i = live ? (e >> LOG2T) : i0;
+    const int64_t t = e - (e >> LOG2T) * T;
+    const int la = (int)(i - i0);
     const double* xt = a.phi_cur + t * VW;
     const int32_t* cp = a.cols + B * i;
-    const double* vp = a.vals + B * i;
+    const double* vrun = a.vals + B * i0;
     Vec<VW> acc[B];
 #pragma unroll
     for (int mu = 0; mu < B; ++mu)
 #pragma unroll
       for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    double pre[NL];
+    if (kStage) {
+#pragma unroll
+      for (int q = 0; q < NL; ++q) pre[q] = (K > 0 && lane + 32 * q < run) ? __ldg(vrun + lane + 32 * q) : 0.0;
+    }
     int64_t j = K > 0 ? (int64_t)(__ldg(cp) / B) : 0;
     for (int k = 0; k < K; ++k) {
       const int64_t jn = k + 1 < K ? (int64_t)(__ldg(cp + (size_t)(B * (k + 1)) * N) / B) : 0;
 #pragma unroll 3
       for (int nu = 0; nu < B; ++nu) {
-        const Vec<VW> x = load_gather<VW>(xt + (B * j + nu) * kOrb);
-        const double* col = vp + (size_t)(B * k + nu) * N;
+        if (kStage) {
+          __syncwarp();  // the previous column has been read by every lane
 #pragma unroll
-        for (int mu = 0; mu < B; ++mu) {
-          const double h = __ldg(col + mu);
+          for (int q = 0; q < NL; ++q)
+            if (lane + 32 * q < B * A) sm[lane + 32 * q] = pre[q];
+          __syncwarp();
+          const int nxt = B * k + nu + 1;   // next column of this row of blocks, one ahead
+          if (nxt < B * K) {
+            const double* src = vrun + (size_t)nxt * N;
 #pragma unroll
-          for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(h, x.v[q], acc[mu].v[q]);
+            for (int q = 0; q < NL; ++q) pre[q] = lane + 32 * q < run ? __ldg(src + lane + 32 * q) : 0.0;
+          }
+        }
+        if (live) {
+          const Vec<VW> x = load_gather<VW>(xt + (B * j + nu) * kOrb);
+          const double* col = a.vals + (size_t)(B * k + nu) * N + B * i;   // direct path (kStage = 0)
+#pragma unroll
+          for (int mu = 0; mu < B; ++mu) {
+            const double h = kStage ? sm[B * la + mu] : __ldg(col + mu);
+#pragma unroll
+            for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(h, x.v[q], acc[mu].v[q]);
+          }
         }
       }
       j = jn;
     }
+    if (live) {
 #pragma unroll
-    for (int mu = 0; mu < B; ++mu) {
-      const int64_t at = (B * i + mu) * kOrb + t * VW;
-      const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
-      Vec<VW> prev, with;
-      if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
-      if (kDotL) with = load_stream<VW>(a.dot_with + at);
-      const double dg = kDiag ? __ldg(a.diag + B * i + mu) : 0.0;
-      Vec<VW> y;
+      for (int mu = 0; mu < B; ++mu) {
+        const int64_t at = (B * i + mu) * kOrb + t * VW;
+        const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
+        Vec<VW> prev, with;
+        if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+        if (kDotL) with = load_stream<VW>(a.dot_with + at);
+        const double dg = kDiag ? __ldg(a.diag + B * i + mu) : 0.0;
+        Vec<VW> y;
 #pragma unroll
-      for (int q = 0; q < VW; ++q) {
-        double h = acc[mu].v[q];
-        if (kDiag) h = fma(dg, own.v[q], h);
-        y.v[q] = (h - b * own.v[q]) * scale;
-        if (!kFirst) y.v[q] -= prev.v[q];
-        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
-        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+        for (int q = 0; q < VW; ++q) {
+          double h = acc[mu].v[q];
+          if (kDiag) h = fma(dg, own.v[q], h);
+          y.v[q] = (h - b * own.v[q]) * scale;
+          if (!kFirst) y.v[q] -= prev.v[q];
+          s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+          s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+        }
+        store_stream<VW>(a.phi_io + at, y);
       }
-      store_stream<VW>(a.phi_io + at, y);
     }
   }
   __shared__ double red[kBlock / 32][2];
   s1 = warp_sum(s1);
   s2 = warp_sum(s2);
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   if (lane == 0) {
     red[wid][0] = s1;
     red[wid][1] = s2;
@@ -992,9 +1025,12 @@ void pick_orb_dot(int B, bool diag, StepPlan* p) {
   if (B == 4) {
     p->first = diag ? cheb_orb4_kernel<LOG2T, true, true, DOT> : cheb_orb4_kernel<LOG2T, true, false, DOT>;
     p->next = diag ? cheb_orb4_kernel<LOG2T, false, true, DOT> : cheb_orb4_kernel<LOG2T, false, false, DOT>;
+  } else if (env_int("GTB_K7_ORB9_STAGE", 1)) {  // block columns through shared memory
+    p->first = diag ? cheb_orb9_kernel<LOG2T, true, true, DOT, true> : cheb_orb9_kernel<LOG2T, true, false, DOT, true>;
+    p->next = diag ? cheb_orb9_kernel<LOG2T, false, true, DOT, true> : cheb_orb9_kernel<LOG2T, false, false, DOT, true>;
   } else {
-    p->first = diag ? cheb_orb9_kernel<LOG2T, true, true, DOT> : cheb_orb9_kernel<LOG2T, true, false, DOT>;
-    p->next = diag ? cheb_orb9_kernel<LOG2T, false, true, DOT> : cheb_orb9_kernel<LOG2T, false, false, DOT>;
+    p->first = diag ? cheb_orb9_kernel<LOG2T, true, true, DOT, false> : cheb_orb9_kernel<LOG2T, true, false, DOT, false>;
+    p->next = diag ? cheb_orb9_kernel<LOG2T, false, true, DOT, false> : cheb_orb9_kernel<LOG2T, false, false, DOT, false>;
   }
 }
 template <int LOG2T>

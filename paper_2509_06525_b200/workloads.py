@@ -164,6 +164,19 @@ SK_ONSITE_P = (0.0, 2.3, -2.3)
 _SK_PAIR_SCALE = {(0, 0): 1.0, (1, 2): 0.96, (0, 1): 0.93, (0, 2): 1.04, (1, 1): 0.5, (2, 2): 0.5}
 
 
+SK_D = (-2.1, -1.7, 0.9, -1.3, 0.8, -0.15)      # sd_sigma, pd_sigma, pd_pi, dd_sigma, dd_pi, dd_delta
+SK_ONSITE_D = (6.5, 7.0, 5.5)
+
+
+def spd_table(n_species: int) -> np.ndarray:
+    """[ns][ns][10]: ss_sigma, sp_sigma, pp_sigma, pp_pi, sd_sigma, pd_sigma, pd_pi, dd_sigma, dd_pi, dd_delta."""
+    t = np.zeros((n_species, n_species, 10))
+    for (a, b), f in _SK_PAIR_SCALE.items():
+        if a < n_species and b < n_species:
+            t[a, b] = t[b, a] = f * np.array(SK_CC + SK_D)
+    return t
+
+
 def sk_table(n_species: int) -> np.ndarray:
     t = np.zeros((n_species, n_species, 4))
     for (a, b), f in _SK_PAIR_SCALE.items():
