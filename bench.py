@@ -34,6 +34,7 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
+GROUPED = os.environ.get("GTB_BENCH_GROUPED", "0") != "0"   # opt-in: K7g (row groups) for wide single-orbital rows
 HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
 ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom), "sp" (4) or "spd" (9)
 ORB_COUNT = {"pz": 1, "sp": 4, "spd": 9}
@@ -288,8 +289,11 @@ def run_ours(args):
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode={"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0),
-                        ws=ws_kpm, mu=mu)
+        Hk, kmode = H, {"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0)
+        if GROUPED and ORBITALS == "pz" and H.width > 4 and n % 4 == 0 and w.R in (2, 4, 8):
+            Hk, kmode = gtb.group_rows(H), gtb.MODE_GROUP4     # K7g: part of the timed step
+            state["grouped_width"] = Hk.width
+        gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         rho = gtb.dos(mu, a, b, state["E"])
@@ -351,7 +355,10 @@ def run_ours(args):
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
     small = (not orb4 and w.R in (2, 4, 8) and n_orb * (w.R // 2) <= 148 * 4 * 256
              and os.environ.get("GTB_K7_SMALL", "1") != "0" and os.environ.get("GTB_K7_SWEEP", "0") == "0")
-    k7_name = ("cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
+    if "grouped_width" in state:
+        small = orb4 = False
+    k7_name = ("cheb_grp4_kernel (K7g: fused Chebyshev pass on groups of 4 rows, union width %d)" % state["grouped_width"]
+               if "grouped_width" in state else "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
                ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
                if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0

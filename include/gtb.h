@@ -58,6 +58,7 @@ enum {
 };
 
 #define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian  (4 orbitals) */
+#define GTB_MODE_GROUP4 64 /* ... H is the row-grouped matrix written by gtb_group_rows                    */
 #define GTB_MODE_ORB9 32 /* ... from gtb_spd_hamiltonian (9 orbitals per atom)                           */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
@@ -137,6 +138,7 @@ int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, doubl
  *         written by gtb_sk_hamiltonian (4 orbitals per atom; gtb_spd_hamiltonian: 9); the fused pass
  *         then works on whole 4x4 (9x9) blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
  *         when R_batch is not 2, 4 or 8.  A matrix without that structure gives wrong results.
+ * mode | GTB_MODE_GROUP4: H is the row-grouped matrix of gtb_group_rows (R_batch must be 2, 4 or 8).
  * R_batch: 1..64.  R_batch in {2,4,8} takes the 256-bit vector path.
  * ASYNC.  mu is DEVICE [M].  Workspace: gtb_kpm_workspace_bytes(n, M, R_batch). */
 size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch);
@@ -301,6 +303,19 @@ size_t gtb_spd_workspace_bytes(void);
 int gtb_spd_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* species,
                         const double box[3], const int32_t pbc[3], const gtb_spd_model* model,
                         gtb_ell* H, int32_t* status, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- row groups: 4 consecutive rows share their gathered neighbours (K7g) ----
+ * A re-arrangement of an ELL matrix for the fused pass, not a different operator: for rows 4g..4g+3 the
+ * ascending UNION of their column lists (padding slots skipped) and, per union column, the 4 values (zero
+ * where a row lacks the column).  Layout of the grouped matrix G (a gtb_ell read differently):
+ *   G->n = H->n (a multiple of 4), G->width = U = largest union, G->cols int32 [U][n/4] (row indices),
+ *   G->vals double [U][n/4][4] (32-byte aligned), G->diag = H->diag or NULL; unused slots hold column 4g, zeros.
+ * gtb_kpm_moments(G, ..., mode | GTB_MODE_GROUP4) then gathers each neighbour once per group instead of
+ * once per row.  Same moments (the per-row sums run over the same non-zero terms in the same order). */
+/* SYNC.  *width_out (HOST) = U.  scratch: DEVICE int32. */
+int gtb_group_width(const gtb_ell* H, int32_t* scratch, void* stream, int32_t* width_out);
+/* SYNC.  Fills G->cols, G->vals (caller-allocated for G->width); GTB_ERR_ELL_OVERFLOW if G->width < U. */
+int gtb_group_rows(const gtb_ell* H, gtb_ell* G, int32_t* scratch, void* stream);
 
 #ifdef __cplusplus
 }

@@ -33,9 +33,10 @@ EXPORTS = (
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
-    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian",
+    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_group_width", "gtb_group_rows",
 )
 
+MODE_GROUP4 = 64            # H is the row-grouped matrix of group_rows()
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
@@ -516,3 +517,20 @@ def spd_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "spd_hamiltonian", "species index out of range")
     return H
+
+
+# ---------------------------------------------------------------- row groups (K7g)
+def group_rows(H: Ell) -> Ell:
+    """The row-grouped re-arrangement of H for kpm_moments(..., mode=MODE_GROUP4): cols [U][n/4],
+    vals [U][n/4][4]; the diagonal array is shared."""
+    dev = H.vals.device
+    scratch = torch.zeros(1, dtype=torch.int32, device=dev)
+    U = C.c_int32(0)
+    hc = H._c()
+    _check(lib().gtb_group_width(C.byref(hc), _ptr(scratch), _stream(), C.byref(U)), "group_width")
+    ng = H.n // 4
+    G = Ell(H.n, int(U.value), torch.empty((U.value, ng), dtype=torch.int32, device=dev),
+            torch.empty((U.value, ng, 4), dtype=torch.float64, device=dev), H.diag)
+    gc = G._c()
+    _check(lib().gtb_group_rows(C.byref(hc), C.byref(gc), _ptr(scratch), _stream()), "group_rows")
+    return G

@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
     const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
     if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
     __syncwarp();
-    for (int j = lane; j < 2 * width + 4; j += 32) {
+    for (int j = lane; j < 2 * width + (kDotL ? 4 : 3); j += 32) {
       if (j < width) {
         bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
       } else if (j < 2 * width) {
@@ -567,6 +567,152 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
       s2 += red[w][1];
     }
     a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+// ---- K7g: the fused pass on row groups (4 consecutive rows share their gathered neighbours) ----------
+// With wide rows K7t sits on the L1 data pipe: one wavefront per (row, neighbour) gather.  Consecutive rows
+// of a lattice share most of their neighbours (the 4 atoms of a graphene cell within 4.0 A: 33 distinct
+// neighbours instead of 4 x 18), so the matrix is regrouped once (gtb_group_rows): for rows 4g..4g+3 the
+// sorted UNION of their column lists, and per union column the 4 hoppings (zero where a row lacks it) as one
+// 32-byte vector: cols [U][n/4], vals [U][n/4][4].  One thread owns (group, one 256-bit element of the R
+// vectors): per union column one index, one 256-bit load of the 4 hoppings, ONE gather, 4 x VW FMAs.
+// Gathers per row drop from K to U/4 (8.25 at config 2) at the price of ~25 % more matrix bytes.  Per row
+// the slot order of the sum is the union's (ascending column), which is the ELL's own order with exact
+// zeros skipped in between: the vectors agree with K7 bit for bit except for the sign of zero.
+template <int LOG2T, bool kFirst, bool kDiag, bool kDotL>
+__global__ void __launch_bounds__(kBlock) cheb_grp4_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  const int64_t ng = a.n >> 2;
+  const int U = a.width;
+  const int64_t total = ng * T;
+  const double scale = a.scale, b = a.b;
+  constexpr int64_t kRow = (int64_t)T * VW;  // doubles per row of phi
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock) {
+    const int64_t g = e >> LOG2T;
+    const int64_t t = e - g * T;
+    const double* xt = a.phi_cur + t * VW;
+    const int32_t* cp = a.cols + g;
+    const double* vp = a.vals + 4 * g;
+    Vec<VW> acc[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    // CH union columns at a time: all CH indices are loaded before the CH gathers that depend on them
+    constexpr int CH = 8;
+    for (int u0 = 0; u0 < U; u0 += CH) {
+      int32_t c[CH];
+#pragma unroll
+      for (int j = 0; j < CH; ++j) c[j] = u0 + j < U ? __ldg(cp + (size_t)(u0 + j) * ng) : (int32_t)(4 * g);
+      Vec<VW> x[CH];
+#pragma unroll
+      for (int j = 0; j < CH; ++j) x[j] = load_gather<VW>(xt + (int64_t)c[j] * kRow);
+#pragma unroll
+      for (int j = 0; j < CH; ++j) {
+        if (u0 + j < U) {
+          const Vec<VW> h = load_stream<VW>(vp + (size_t)(u0 + j) * ng * 4);
+#pragma unroll
+          for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+            for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(h.v[mu], x[j].v[q], acc[mu].v[q]);
+        }
+      }
+    }
+    Vec<VW> dg;
+    if (kDiag) dg = load_stream<VW>(a.diag + 4 * g);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      const int64_t at = (4 * g + mu) * kRow + t * VW;
+      const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
+      Vec<VW> prev, with;
+      if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+      if (kDotL) with = load_stream<VW>(a.dot_with + at);
+      Vec<VW> y;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        double hh = acc[mu].v[q];
+        if (kDiag) hh = fma(dg.v[mu], own.v[q], hh);
+        y.v[q] = (hh - b * own.v[q]) * scale;
+        if (!kFirst) y.v[q] -= prev.v[q];
+        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+      }
+      store_stream<VW>(a.phi_io + at, y);
+    }
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+// regrouping: one thread per group merges the 4 sorted column lists (padding = own row index, skipped).
+// kFill = false: *width_out = max union size;  kFill = true: writes cols/vals (width U given).
+template <bool kFill>
+__global__ void __launch_bounds__(kBlock) group_rows_kernel(const int32_t* __restrict__ cols,
+                                                            const double* __restrict__ vals, int64_t n,
+                                                            int32_t K, int32_t U, int32_t* __restrict__ gcols,
+                                                            double* __restrict__ gvals,
+                                                            int32_t* __restrict__ width_out) {
+  const int64_t ng = n >> 2;
+  int worst = 0;
+  for (int64_t g = (int64_t)blockIdx.x * kBlock + threadIdx.x; g < ng; g += (int64_t)gridDim.x * kBlock) {
+    int pos[4] = {0, 0, 0, 0};
+    int u = 0;
+    for (;;) {
+      int64_t best = INT64_MAX;
+      int64_t cur[4];
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) {
+        const int64_t row = 4 * g + mu;
+        while (pos[mu] < K && cols[(size_t)pos[mu] * n + row] == row) ++pos[mu];  // padding slots
+        cur[mu] = pos[mu] < K ? (int64_t)cols[(size_t)pos[mu] * n + row] : INT64_MAX;
+        best = min(best, cur[mu]);
+      }
+      if (best == INT64_MAX) break;
+      if (kFill && u < U) {
+        gcols[(size_t)u * ng + g] = (int32_t)best;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu)
+          gvals[((size_t)u * ng + g) * 4 + mu] =
+              cur[mu] == best ? vals[(size_t)pos[mu] * n + 4 * g + mu] : 0.0;
+      }
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu)
+        if (cur[mu] == best) ++pos[mu];
+      ++u;
+    }
+    if (kFill) {
+      for (; u < U; ++u) {  // padding: the group's first row, zeros
+        gcols[(size_t)u * ng + g] = (int32_t)(4 * g);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) gvals[((size_t)u * ng + g) * 4 + mu] = 0.0;
+      }
+    }
+    worst = max(worst, u);
+  }
+  if (!kFill) {
+    worst = warp_max_i(worst);
+    if ((threadIdx.x & 31) == 0 && worst > 0) atomicMax(width_out, worst);
+  } else if (worst > U) {
+    atomicMax(width_out, worst);  // overflow: reported by the host wrapper
   }
 }
 
@@ -1062,6 +1208,34 @@ bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, StepPlan* p) {
   return true;
 }
 
+template <int LOG2T, bool DOT>
+void pick_grp_dot(bool diag, StepPlan* p) {
+  p->first = diag ? cheb_grp4_kernel<LOG2T, true, true, DOT> : cheb_grp4_kernel<LOG2T, true, false, DOT>;
+  p->next = diag ? cheb_grp4_kernel<LOG2T, false, true, DOT> : cheb_grp4_kernel<LOG2T, false, false, DOT>;
+}
+
+// K7g plan: H holds the grouped arrays of gtb_group_rows (cols [U][n/4], vals [U][n/4][4])
+bool make_plan_grp4(const gtb_ell* H, int R, bool dot, StepPlan* p) {
+  if (H->n % 4 || H->width == 0 || (R != 2 && R != 4 && R != 8) ||
+      (reinterpret_cast<uintptr_t>(H->vals) & 31u) || (reinterpret_cast<uintptr_t>(H->diag) & 31u))
+    return false;
+  const bool diag = H->diag != nullptr;
+  if (R == 2) { if (dot) pick_grp_dot<0, true>(diag, p); else pick_grp_dot<0, false>(diag, p); p->T = 1; }
+  else if (R == 4) { if (dot) pick_grp_dot<1, true>(diag, p); else pick_grp_dot<1, false>(diag, p); p->T = 2; }
+  else { if (dot) pick_grp_dot<2, true>(diag, p); else pick_grp_dot<2, false>(diag, p); p->T = 4; }
+  p->vw = 4;
+  p->stages = 0;
+  int dev = 0, sms = kSmCount, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0) != cudaSuccess)
+    return false;
+  per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
+  const int64_t total = H->n / 4 * p->T;
+  p->grid = (int)std::max<int64_t>(1, std::min<int64_t>((total + kBlock - 1) / kBlock, (int64_t)sms * per_sm));
+  return true;
+}
+
 int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   const int64_t n = H->n;
   const int width = H->width;
@@ -1227,11 +1401,13 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
                                size_t ws_bytes, void* stream) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
-  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9)) ||
-      ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)))
+  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_GROUP4)) ||
+      ((mode_flags & GTB_MODE_ORB4) != 0) + ((mode_flags & GTB_MODE_ORB9) != 0) +
+              ((mode_flags & GTB_MODE_GROUP4) != 0) > 1)
     return GTB_ERR_INVALID_ARG;
   const int32_t mode = mode_flags & 1;
   const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
+  const bool grouped = (mode_flags & GTB_MODE_GROUP4) != 0;
   if (!mu || M <= 0 || !(a > 0.0) || !std::isfinite(b) || R_batch <= 0 || R_batch > 64 ||
       (mode != 0 && mode != 1) || (mode == 0 && R_total <= 0))
     return GTB_ERR_INVALID_ARG;
@@ -1253,7 +1429,8 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
-    const bool blocked = orb && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb(H, R, orb, false, &plan);
+    if (grouped && !make_plan_grp4(H, R, false, &plan)) return GTB_ERR_INVALID_ARG;  // no scalar reading
+    const bool blocked = grouped || (orb && env_int("GTB_K7_ORB4", 1) != 0 && make_plan_orb(H, R, orb, false, &plan));
     if (!blocked) {
       rc = make_plan(H, R, false, &plan);
       if (rc != GTB_OK) return rc;
@@ -1384,6 +1561,38 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
   finish_moments_kernel<<<(M + kBlock - 1) / kBlock, kBlock, 0, st>>>(w.sums, M, norm, mu, w.status);
   GTB_LAUNCHED();
   return GTB_OK;
+}
+
+extern "C" int gtb_group_width(const gtb_ell* H, int32_t* scratch, void* stream, int32_t* width_out) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if (!scratch || !width_out || H->n % 4 || H->width == 0) return GTB_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GTB_CUDA_TRY(cudaMemsetAsync(scratch, 0, sizeof(int32_t), st));
+  group_rows_kernel<false><<<fill_grid(H->n / 4), kBlock, 0, st>>>(H->cols, H->vals, H->n, H->width, 0,
+                                                                   nullptr, nullptr, scratch);
+  GTB_LAUNCHED();
+  GTB_CUDA_TRY(cudaMemcpyAsync(width_out, scratch, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  GTB_CUDA_TRY(cudaStreamSynchronize(st));
+  if (*width_out < 1) *width_out = 1;  // a matrix without off-diagonal entries still gets one (zero) slot
+  return GTB_OK;
+}
+
+extern "C" int gtb_group_rows(const gtb_ell* H, gtb_ell* G, int32_t* scratch, void* stream) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if (!G || !scratch || H->n % 4 || H->width == 0 || G->n != H->n || G->width < 1 || !G->cols ||
+      !G->vals || (reinterpret_cast<uintptr_t>(G->vals) & 31u))
+    return GTB_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GTB_CUDA_TRY(cudaMemsetAsync(scratch, 0, sizeof(int32_t), st));
+  group_rows_kernel<true><<<fill_grid(H->n / 4), kBlock, 0, st>>>(H->cols, H->vals, H->n, H->width,
+                                                                  G->width, G->cols, G->vals, scratch);
+  GTB_LAUNCHED();
+  int32_t needed = 0;
+  GTB_CUDA_TRY(cudaMemcpyAsync(&needed, scratch, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  GTB_CUDA_TRY(cudaStreamSynchronize(st));
+  return needed > G->width ? GTB_ERR_ELL_OVERFLOW : GTB_OK;
 }
 
 extern "C" int gtb_kpm_status(const void* ws, void* stream) {

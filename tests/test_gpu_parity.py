@@ -288,6 +288,52 @@ def test_single_launch_path_matches_oracle_and_per_pass_path(monkeypatch, key, n
         assert used < (gtb.launch_count() - l0) // 4      # the single-launch path really was taken
 
 
+# K7g: row groups (4 consecutive rows share their gathered neighbours).  The grouped arrays are checked
+# against the union built here from the oracle's ELL, the moments against the oracle's.
+@pytest.mark.parametrize("key,nx,ny,kw", SMALL)
+def test_row_groups_and_grouped_moments(key, nx, ny, kw):
+    w, inp = _small(key, nx, ny, kw)
+    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
+    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
+    G = gtb.group_rows(Hg)
+    n, ng = Ho.n, Ho.n // 4
+    gc, gv = G.cols.cpu().numpy(), G.vals.cpu().numpy()
+    assert gc.shape == (G.width, ng) and gv.shape == (G.width, ng, 4)
+    worst = 0
+    for g in range(0, ng, max(1, ng // 97)):                # sampled groups, incl. the first
+        rows = np.arange(4 * g, 4 * g + 4)
+        union = sorted({int(c) for r in rows for c in Ho.cols[:, r] if c != r})
+        worst = max(worst, len(union))
+        assert gc[:len(union), g].tolist() == union and (gc[len(union):, g] == 4 * g).all()
+        for mu, r in enumerate(rows):
+            want = {int(c): v for c, v in zip(Ho.cols[:, r], Ho.vals[:, r]) if c != r}
+            got = gv[:, g, mu]
+            assert (got[len(union):] == 0).all()
+            for u, c in enumerate(union):
+                ref = want.get(c, 0.0)
+                assert abs(got[u] - ref) <= ULP4 * max(abs(ref), 1e-300) or got[u] == ref
+    assert worst <= G.width
+    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
+    for R, M in ((2, 33), (4, 64), (8, 65)):
+        ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
+        got = gtb.kpm_moments(G, a, b, M, R, R, 5, mode=gtb.MODE_GROUP4, check=True).cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-12
+    exact = gtb.kpm_moments(G, a, b, 16, mode=1 | gtb.MODE_GROUP4, R_batch=8).cpu().numpy()
+    plain = gtb.kpm_moments(Hg, a, b, 16, mode=1, R_batch=8).cpu().numpy()
+    assert np.abs(exact - plain).max() <= 1e-13
+    with pytest.raises(gtb.GtbError):                      # the grouped layout has no scalar reading
+        gtb.kpm_moments(G, a, b, 8, 3, 3, 5, mode=gtb.MODE_GROUP4)
+
+
+def test_row_groups_need_a_multiple_of_four_rows():
+    w, inp = _small("c2b", 23, 17, {})
+    n = inp.pos.shape[0] - 1
+    args = (inp.box, (0, 0, 0), w.cutoff, w.onsite, w.t0, w.r0, w.beta)
+    Hg = gtb.build_hamiltonian(_dev(inp.pos[:n]), _dev(inp.species[:n]), *args, _dev(inp.onsite_shift[:n]))
+    with pytest.raises(gtb.GtbError):
+        gtb.group_rows(Hg)
+
+
 @pytest.mark.parametrize("drop", [1, 2, 3])
 def test_atom_count_not_a_multiple_of_four_takes_the_register_path(drop):
     # bulk copies need 16-byte aligned slot rows (n % 4 == 0); any other n must still be exact
