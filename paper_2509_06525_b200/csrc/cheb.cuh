@@ -35,6 +35,7 @@ struct StepPlan {
   int grid = 0;
   int stages = 0;
   size_t smem = 0;
+  int block = 0;   // threads per CTA of the staged kernel (0: the default of K7t)
 };
 
 // dot = false: the DOS pass (dot products with phi_n itself); dot = true: with StepArgs::dot_with.

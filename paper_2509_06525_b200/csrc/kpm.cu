@@ -663,6 +663,150 @@ __global__ void __launch_bounds__(kBlock) cheb_grp4_kernel(const StepArgs a) {
   }
 }
 
+// ---- K7gt: K7g with the grouped slots staged by TMA -------------------------------------------------
+// K7g alone is latency-bound (column index -> gather, hoppings from HBM).  Here the union columns and the
+// hopping vectors of a tile of TG groups arrive in a shared-memory ring by cp.async.bulk (one copy per union
+// slot and array), exactly as K7t stages the ELL slots; a stage is U x TG x 36 bytes (76 KB at U = 33,
+// TG = 64), so one CTA per SM with two stages and up to 255 registers per thread: the 4 rows' phi_{n-1} and
+// phi_n elements are loaded before the wait and the gathers are issued CH at a time from shared indices.
+template <int LOG2T, int NT, bool kFirst, bool kDiag, bool kDotL>
+__global__ void __launch_bounds__(NT, 1) cheb_grp4_tile_kernel(const StepArgs a, const int nstages) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int TG = NT / T;                 // groups per tile
+#ifndef GTB_GRP_CH
+#define GTB_GRP_CH 11
+#endif
+  constexpr int CH = GTB_GRP_CH;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int64_t ng = a.n >> 2;
+  const int U = a.width;
+  const double scale = a.scale, b = a.b;
+  const uint32_t vals_bytes = (uint32_t)U * TG * 32;
+  const uint32_t stage_bytes = vals_bytes + (uint32_t)U * TG * 4;
+  const uint32_t bar0 = smem_u32(smem);
+  unsigned char* const stage0 = smem + kBarBytes;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int64_t n_tiles = (ng + TG - 1) / TG;
+  const int64_t my_tiles = blockIdx.x < n_tiles ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0;
+  constexpr int64_t kRow = (int64_t)T * VW;
+  if (tid == 0) {
+    for (int s = 0; s < nstages; ++s) mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  auto issue = [&](int64_t i) {
+    const int s = (int)(i % nstages);
+    const int64_t g0 = (blockIdx.x + i * gridDim.x) * TG;
+    const uint32_t groups = (uint32_t)min((int64_t)TG, ng - g0);
+    const uint32_t bar = bar0 + 8 * s;
+    const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
+    if (lane == 0) mbar_expect_tx(bar, groups * (uint32_t)U * 36);
+    __syncwarp();
+    for (int j = lane; j < 2 * U + 3; j += 32) {
+      if (j < U) {
+        bulk_g2s(base + (uint32_t)j * TG * 32, a.vals + ((size_t)j * ng + g0) * 4, groups * 32, bar);
+      } else if (j < 2 * U) {
+        const int u = j - U;
+        bulk_g2s(base + vals_bytes + (uint32_t)u * TG * 4, a.cols + (size_t)u * ng + g0, groups * 4, bar);
+      } else if (j == 2 * U) {
+        bulk_prefetch_l2(a.phi_cur + 4 * g0 * kRow, groups * 4 * (uint32_t)(kRow * 8));
+      } else if (j == 2 * U + 1) {
+        if (!kFirst) bulk_prefetch_l2(a.phi_io + 4 * g0 * kRow, groups * 4 * (uint32_t)(kRow * 8));
+      } else {
+        if (kDotL) bulk_prefetch_l2(a.dot_with + 4 * g0 * kRow, groups * 4 * (uint32_t)(kRow * 8));
+      }
+    }
+  };
+  if (wid == 0)
+    for (int64_t i = 0; i < min((int64_t)nstages, my_tiles); ++i) issue(i);
+  double s1 = 0.0, s2 = 0.0;
+  const int gl = tid >> LOG2T;
+  const int t = tid & (T - 1);
+  const double* xt = a.phi_cur + t * VW;
+  for (int64_t i = 0; i < my_tiles; ++i) {
+    const int s = (int)(i % nstages);
+    const int64_t g = (blockIdx.x + i * gridDim.x) * TG + gl;
+    const bool live = g < ng;
+    Vec<VW> own[4], prev[4], acc[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = own[mu].v[q] = prev[mu].v[q] = 0.0;
+      if (live) {
+        const int64_t at = (4 * g + mu) * kRow + t * VW;
+        own[mu] = load_gather<VW>(a.phi_cur + at);
+        if (!kFirst) prev[mu] = load_stream<VW>(a.phi_io + at);
+      }
+    }
+    mbar_wait(bar0 + 8 * s, (uint32_t)((i / nstages) & 1));
+    const unsigned char* st = stage0 + (size_t)s * stage_bytes;
+    const double* sv = reinterpret_cast<const double*>(st) + gl * 4;
+    const int32_t* sc = reinterpret_cast<const int32_t*>(st + vals_bytes) + gl;
+    if (live) {
+      for (int u0 = 0; u0 < U; u0 += CH) {
+        int32_t c[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) c[j] = u0 + j < U ? sc[(u0 + j) * TG] : (int32_t)(4 * g);
+        Vec<VW> x[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) x[j] = load_gather<VW>(xt + (int64_t)c[j] * kRow);
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+          if (u0 + j < U) {
+            const double* h = sv + (size_t)(u0 + j) * TG * 4;
+#pragma unroll
+            for (int mu = 0; mu < 4; ++mu) {
+              const double hm = h[mu];
+#pragma unroll
+              for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(hm, x[j].v[q], acc[mu].v[q]);
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();  // every thread has read stage s
+    if (wid == 0 && i + nstages < my_tiles) issue(i + nstages);
+    if (live) {
+      Vec<VW> dg;
+      if (kDiag) dg = load_stream<VW>(a.diag + 4 * g);
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) {
+        const int64_t at = (4 * g + mu) * kRow + t * VW;
+        Vec<VW> with;
+        if (kDotL) with = load_stream<VW>(a.dot_with + at);
+        Vec<VW> y;
+#pragma unroll
+        for (int q = 0; q < VW; ++q) {
+          double hh = acc[mu].v[q];
+          if (kDiag) hh = fma(dg.v[mu], own[mu].v[q], hh);
+          y.v[q] = (hh - b * own[mu].v[q]) * scale;
+          if (!kFirst) y.v[q] -= prev[mu].v[q];
+          s1 = fma(own[mu].v[q], kDotL ? with.v[q] : own[mu].v[q], s1);
+          s2 = fma(y.v[q], kDotL ? with.v[q] : own[mu].v[q], s2);
+        }
+        store_stream<VW>(a.phi_io + at, y);
+      }
+    }
+  }
+  __shared__ double red[NT / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int w = 1; w < NT / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
 // regrouping: one thread per group merges the 4 sorted column lists (padding = own row index, skipped).
 // kFill = false: *width_out = max union size;  kFill = true: writes cols/vals (width U given).
 template <bool kFill>
@@ -1225,10 +1369,35 @@ bool make_plan_grp4(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   else { if (dot) pick_grp_dot<2, true>(diag, p); else pick_grp_dot<2, false>(diag, p); p->T = 4; }
   p->vw = 4;
   p->stages = 0;
+  p->block = kBlock;
   int dev = 0, sms = kSmCount, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess ||
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0) != cudaSuccess)
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return false;
+  // K7gt: TMA-staged variant for R = 8 (one CTA of 256 threads per SM, 64 groups per tile)
+  if (R == 8 && !dot && H->n % 16 == 0 && !(reinterpret_cast<uintptr_t>(H->cols) & 15u) &&
+      env_int("GTB_K7_GROUP_TILE", 1) != 0) {
+    int max_smem = 0;
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const size_t stage_bytes = (size_t)H->width * 64 * 36;
+    int stages = env_int("GTB_K7_STAGES", 2);
+    while (stages > 1 && kBarBytes + stages * stage_bytes > (size_t)max_smem) --stages;
+    const size_t smem = kBarBytes + stages * stage_bytes;
+    if (smem <= (size_t)max_smem) {
+      p->tfirst = diag ? cheb_grp4_tile_kernel<2, 256, true, true, false> : cheb_grp4_tile_kernel<2, 256, true, false, false>;
+      p->tnext = diag ? cheb_grp4_tile_kernel<2, 256, false, true, false> : cheb_grp4_tile_kernel<2, 256, false, false, false>;
+      if (cudaFuncSetAttribute(p->tfirst, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+          cudaFuncSetAttribute(p->tnext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+        const int64_t n_tiles = (H->n / 4 + 63) / 64;
+        p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, sms));
+        p->stages = stages;
+        p->smem = smem;
+        p->block = 256;
+        return true;
+      }
+    }
+  }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, kBlock, 0) != cudaSuccess)
     return false;
   per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
   const int64_t total = H->n / 4 * p->T;
@@ -1293,7 +1462,7 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
 
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st) {
   if (p.stages > 0)
-    (first ? p.tfirst : p.tnext)<<<p.grid, kTileBlock, p.smem, st>>>(sa, p.stages);
+    (first ? p.tfirst : p.tnext)<<<p.grid, p.block ? p.block : kTileBlock, p.smem, st>>>(sa, p.stages);
   else
     (first ? p.first : p.next)<<<p.grid, kBlock, 0, st>>>(sa);
 }
