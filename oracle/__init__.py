@@ -341,3 +341,18 @@ def spd_hamiltonian(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, onsite
     _check(lib().gtbo_spd_hamiltonian(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
                                       C.byref(model), C.byref(hc)), "spd_hamiltonian")
     return H
+
+
+def mlp_sk_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, weights,
+                       with_diag: bool = True) -> Ell:
+    """Eq. 2 feeding the s,p Slater-Koster blocks: scalar ELL over 4n orbitals (blob with 4 / 2 outputs)."""
+    ns, F, Nb, Hd = dims
+    pos, species, box, pbc, w = _f64(pos), _i32(species), _f64(box), _i32(pbc), _f64(weights)
+    n, K = nbr.n, nbr.width
+    H = Ell(4 * n, 4 * K, np.zeros((4 * K, 4 * n), dtype=np.int32), np.zeros((4 * K, 4 * n)),
+            np.zeros(4 * n) if with_diag else None)
+    m = _MlpModel(ns, F, Nb, Hd, r_cut, w.ctypes.data)
+    nc, hc = nbr._c(), H._c()
+    _check(lib().gtbo_mlp_sk_hamiltonian(C.byref(m), C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
+                                         C.byref(hc)), "mlp_sk_hamiltonian")
+    return H

@@ -188,6 +188,13 @@ int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* 
                          const double box[3], const int32_t pbc[3],
                          const gtbo_spd_model* model, gtbo_ell* H);
 
+/* Eq. 2 feeding the s,p Slater-Koster blocks: MLP_lambda with four outputs (ss_sigma,
+ * sp_sigma, pp_sigma, pp_pi of the pair), onsite MLP with two (eps_s, eps_p); blob layout in gtbo_mlp.cpp.
+ * H: scalar ELL over 4n orbitals as gtbo_sk_hamiltonian's. */
+int gtbo_mlp_sk_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* nbr, const double* pos,
+                            const int32_t* species, const double box[3], const int32_t pbc[3],
+                            gtbo_ell* H);
+
 #ifdef __cplusplus
 }
 #endif

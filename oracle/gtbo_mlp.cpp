@@ -128,3 +128,75 @@ extern "C" int gtbo_mlp_hamiltonian(const gtbo_mlp_model* m, const double* pos, 
   if (v_out) for (size_t q = 0; q < v.size(); ++q) v_out[q] = v[q];
   return GTBO_OK;
 }
+
+// ---- Eq. 2 feeding the Slater-Koster blocks: the paper's full hopping formula ----------------------
+//   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i)
+// for the s,p basis: MLP_lambda has four outputs, the bond integrals ss_sigma, sp_sigma,
+// pp_sigma, pp_pi of the pair, which enter the two-centre table of gtbo_sk.cpp; the onsite MLP has two
+// outputs (eps_s, eps_p).  Reading E6: one MLP_lambda with a 4-vector output
+// instead of four networks.  Blob layout as above with MLP_lambda: W1 [Hd][F], b1 [Hd], W2 [4][Hd],
+// b2 [4] and per species: W1 [Hd][F], b1 [Hd], W2 [2][Hd], b2 [2].
+extern "C" int gtbo_mlp_sk_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* nbr, const double* pos,
+                                       const int32_t* species, const double box[3],
+                                       const int32_t pbc[3], gtbo_ell* H) {
+  if (!m || !nbr || !pos || !species || !box || !pbc || !H || !H->cols || !H->vals || !m->weights ||
+      H->n != 4 * nbr->n || H->width != 4 * nbr->width || !(m->r_cut > 0.0))
+    return GTBO_ERR_INVALID_ARG;
+  const int ns = m->n_species, F = m->n_features, Nb = m->n_basis, Hd = m->n_hidden;
+  const double* w = m->weights;
+  const double* w_env = w + (size_t)ns * ns * F * Nb;
+  const double* w_hop = w_env + (size_t)Hd * F + Hd + (size_t)F * Hd + F;
+  const size_t hop_size = (size_t)Hd * F + Hd + 4 * (size_t)Hd + 4;
+  const size_t ons_size = (size_t)Hd * F + Hd + 2 * (size_t)Hd + 2;
+  const int64_t n = nbr->n, N = 4 * n;
+  std::vector<double> v((size_t)n * F, 0.0), C(F), u(F), env(F), e(F);
+  for (int64_t i = 0; i < n; ++i)
+    for (int32_t k = 0; k < nbr->width; ++k) {
+      const int64_t j = nbr->cols[(size_t)k * n + i];
+      if (j == i) continue;
+      descriptor(w + ((size_t)species[i] * ns + species[j]) * F * Nb, F, Nb, distance(pos, i, j, box, pbc),
+                 m->r_cut, C.data());
+      for (int q = 0; q < F; ++q) v[(size_t)i * F + q] += C[q];
+    }
+  for (int64_t i = 0; i < n; ++i) {
+    for (int32_t k = 0; k < nbr->width; ++k) {
+      const int64_t j = nbr->cols[(size_t)k * n + i];
+      double E[4][4] = {{0.0}};
+      if (j != i) {
+        double d[3];
+        for (int a = 0; a < 3; ++a) {
+          d[a] = pos[3 * j + a] - pos[3 * i + a];
+          if (pbc[a]) d[a] = d[a] - box[a] * std::rint(d[a] / box[a]);
+        }
+        const double r = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
+        const double c[3] = {d[0] / r, d[1] / r, d[2] / r};
+        descriptor(w + ((size_t)species[i] * ns + species[j]) * F * Nb, F, Nb, r, m->r_cut, C.data());
+        for (int q = 0; q < F; ++q) u[q] = v[(size_t)i * F + q] + v[(size_t)j * F + q];
+        mlp(w_env, F, Hd, F, u.data(), env.data());
+        for (int q = 0; q < F; ++q) e[q] = C[q] * env[q];
+        double V[4];
+        mlp(w_hop, F, Hd, 4, e.data(), V);
+        E[0][0] = V[0];
+        for (int a = 0; a < 3; ++a) {
+          E[0][1 + a] = c[a] * V[1];
+          E[1 + a][0] = -(c[a] * V[1]);
+          for (int b = 0; b < 3; ++b)
+            E[1 + a][1 + b] = c[a] * c[b] * V[2] + ((a == b ? 1.0 : 0.0) - c[a] * c[b]) * V[3];
+        }
+      }
+      for (int mu = 0; mu < 4; ++mu)
+        for (int nu = 0; nu < 4; ++nu) {
+          const size_t at = (size_t)(4 * k + nu) * N + (4 * i + mu);
+          H->cols[at] = (int32_t)(j != i ? 4 * j + nu : 4 * i + mu);
+          H->vals[at] = j != i ? E[mu][nu] : 0.0;
+        }
+    }
+    if (H->diag) {
+      double eps[2];
+      mlp(w_hop + hop_size + (size_t)species[i] * ons_size, F, Hd, 2, &v[(size_t)i * F], eps);
+      H->diag[4 * i] = eps[0];
+      for (int a = 1; a < 4; ++a) H->diag[4 * i + a] = eps[1];
+    }
+  }
+  return GTBO_OK;
+}

@@ -200,8 +200,9 @@ def mlp_pack(c, env, hop, ons) -> np.ndarray:
     return np.ascontiguousarray(np.concatenate(parts))
 
 
-def mlp_weights(dims=MLP_DIMS, seed: int = 65250) -> np.ndarray:
-    """Seeded random weights of moderate size (|t| of a few eV at bond length); c symmetric in the pair."""
+def mlp_weights(dims=MLP_DIMS, seed: int = 65250, hop_out: int = 1, onsite_out: int = 1) -> np.ndarray:
+    """Seeded random weights of moderate size (|t| of a few eV at bond length); c symmetric in the pair.
+    hop_out / onsite_out: outputs of MLP_lambda / the onsite MLPs (1, 1: one orbital; 4, 2: s,p blocks)."""
     ns, F, Nb, Hd = dims
     rng = np.random.Generator(np.random.PCG64(seed))
     c = rng.normal(0.0, 1.0, (ns, ns, F, Nb)) / np.sqrt(Nb)
@@ -210,6 +211,6 @@ def mlp_weights(dims=MLP_DIMS, seed: int = 65250) -> np.ndarray:
         return (rng.normal(0.0, 1.0, (Hd, F)) / np.sqrt(F), rng.normal(0.0, 0.3, Hd),
                 rng.normal(0.0, scale, (out_dim, Hd)) / np.sqrt(Hd), rng.normal(0.0, 0.1, out_dim))
     env = layer(F, 1.0)
-    hop = layer(1, 4.0)
-    ons = [layer(1, 1.0) for _ in range(ns)]
+    hop = layer(hop_out, 4.0)
+    ons = [layer(onsite_out, 1.0) for _ in range(ns)]
     return mlp_pack(c, env, hop, ons)

@@ -155,3 +155,72 @@ def test_symmetry_and_rigid_motion_invariance():
     q, _ = np.linalg.qr(np.random.default_rng(3).standard_normal((3, 3)))
     e1 = spectrum((inp.pos - inp.pos.mean(0)) @ q.T + 100.0)
     assert np.abs(e1 - e0).max() <= 1e-11
+
+
+# ---------------------------------------------------------------------------------- P36
+def _blob_sk(c, env, hop4, ons2):
+    return W.mlp_pack(c, env, hop4, ons2)
+
+
+def test_mlp_sk_with_constant_networks_is_the_slater_koster_oracle():
+    """MLP_lambda with zero weights and the four integrals as output bias, onsite MLPs with (eps_s, eps_p)
+    as bias: the result must be gtbo_sk_hamiltonian's with those constants (beta = 0)."""
+    w = W.CONFIGS["c4"].scaled(8, 3, stripe=2)
+    inp = W.make_inputs(w)
+    ns = 3
+    nbr = _nbr(w, inp, 1.95)
+    V = np.array([-6.769, 5.580, 5.037, -3.033])
+    es, ep = [-8.9, -6.0, -11.0], [0.0, 2.3, -2.3]
+    c = np.random.default_rng(0).normal(size=(NS, NS, F, NB))
+    c = 0.5 * (c + c.transpose(1, 0, 2, 3))
+    env = (np.zeros((HD, F)), np.zeros(HD), np.zeros((F, HD)), np.ones(F))
+    hop4 = (np.zeros((HD, F)), np.zeros(HD), np.zeros((4, HD)), V)
+    ons2 = [(np.zeros((HD, F)), np.zeros(HD), np.zeros((2, HD)), np.array([es[s], ep[s]])) for s in range(NS)]
+    H = oracle.mlp_sk_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, DIMS, RC,
+                                  _blob_sk(c, env, hop4, ons2))
+    table = np.broadcast_to(V, (ns, ns, 4))
+    Hs = oracle.sk_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, es, ep, table, beta=0.0)
+    assert (H.cols == Hs.cols).all()
+    assert np.abs(H.vals - Hs.vals).max() <= 1e-15 and np.abs(H.diag - Hs.diag).max() == 0.0
+
+
+def test_mlp_sk_parameters_are_the_mlp_outputs_and_the_matrix_is_symmetric():
+    w = W.CONFIGS["c2b"].scaled(5, 4)
+    inp = W.make_inputs(w)
+    blob = W.mlp_weights(DIMS, 11, hop_out=4, onsite_out=2)
+    nbr = _nbr(w, inp, 1.95)
+    H = oracle.mlp_sk_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, DIMS, RC, blob)
+    D = H.to_dense()
+    assert np.abs(D - D.T).max() <= 1e-14
+    # the s-s entry of every block is MLP_lambda's first output: redo it in numpy for a few pairs
+    c = blob[:NS * NS * F * NB].reshape(NS, NS, F, NB)
+    off = NS * NS * F * NB
+    def take(shape):
+        nonlocal off
+        size = int(np.prod(shape))
+        out = blob[off:off + size].reshape(shape)
+        off += size
+        return out
+    envp = (take((HD, F)), take((HD,)), take((F, HD)), take((F,)))
+    hopp = (take((HD, F)), take((HD,)), take((4, HD)), take((4,)))
+    def Cn(i, j):
+        d = inp.pos[j] - inp.pos[i]
+        d -= inp.box * np.rint(d / inp.box) * inp.pbc
+        return oracle.mlp_descriptor(DIMS, RC, blob, 0, 0, float(np.linalg.norm(d))), d / np.linalg.norm(d)
+    v = np.zeros((nbr.n, F))
+    for i in range(nbr.n):
+        for k in range(nbr.width):
+            j = nbr.cols[k, i]
+            if j != i:
+                v[i] += Cn(i, j)[0]
+    B = D.reshape(nbr.n, 4, nbr.n, 4)
+    for i in range(0, nbr.n, 9):
+        for k in range(nbr.width):
+            j = nbr.cols[k, i]
+            if j == i:
+                continue
+            Cij, u = Cn(i, j)
+            Vp = _np_mlp(hopp, Cij * _np_mlp(envp, v[i] + v[j]))
+            assert abs(B[i, 0, j, 0] - Vp[0]) <= 1e-12
+            assert np.abs(B[i, 0, j, 1:] - u * Vp[1]).max() <= 1e-12
+            assert abs(np.trace(B[i, 1:, j, 1:]) - (Vp[2] + 2 * Vp[3])) <= 1e-12   # tr of the p-p block
