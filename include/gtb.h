@@ -317,6 +317,19 @@ int gtb_group_width(const gtb_ell* H, int32_t* scratch, void* stream, int32_t* w
 /* SYNC.  Fills G->cols, G->vals (caller-allocated for G->width); GTB_ERR_ELL_OVERFLOW if G->width < U. */
 int gtb_group_rows(const gtb_ell* H, gtb_ell* G, int32_t* scratch, void* stream);
 
+/* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
+ *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):
+ * MLP_lambda has four outputs, the bond integrals ss_sigma, sp_sigma, pp_sigma, pp_pi of the pair (reading E6),
+ * which enter the two-centre table of gtb_sk_hamiltonian; the onsite MLPs have two (eps_s, eps_p).
+ * Weight blob as gtb_mlp_hamiltonian's with MLP_lambda: ..., W2 [4][Hd], b2 [4] and per species
+ * ..., W2 [2][Hd], b2 [2]: gtb_mlp_sk_weight_count() doubles.  (F, Nb, Hd) = (8, 8, 16) only.
+ * ASYNC.  nbr: neighbour lists over the n atoms; H: scalar ELL over 4n orbitals (H->n = 4 n,
+ * H->width = 4 nbr->width, diag [4 n] or NULL), usable with GTB_MODE_ORB4; v: DEVICE [n][F]. */
+size_t gtb_mlp_sk_weight_count(int32_t n_species, int32_t n_features, int32_t n_basis, int32_t n_hidden);
+int gtb_mlp_sk_hamiltonian(const gtb_mlp_model* m, const gtb_ell* nbr, const double* pos,
+                           const int32_t* species, const double box[3], const int32_t pbc[3],
+                           gtb_ell* H, double* v, int32_t* status, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

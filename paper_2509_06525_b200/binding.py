@@ -34,6 +34,7 @@ EXPORTS = (
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_group_width", "gtb_group_rows",
+    "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian",
 )
 
 MODE_GROUP4 = 64            # H is the row-grouped matrix of group_rows()
@@ -534,3 +535,33 @@ def group_rows(H: Ell) -> Ell:
     gc = G._c()
     _check(lib().gtb_group_rows(C.byref(hc), C.byref(gc), _ptr(scratch), _stream()), "group_rows")
     return G
+
+
+def mlp_sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, dims, r_cut: float,
+                       weights: torch.Tensor, with_diag: bool = True) -> Ell:
+    """Eq. 2 feeding the s,p Slater-Koster blocks: scalar ELL over the 4n orbitals (use mode=MODE_ORB4)."""
+    ns, F, Nb, Hd = dims
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    weights = _dev(weights, torch.float64, "weights")
+    lib().gtb_mlp_sk_weight_count.restype = C.c_size_t
+    need = int(lib().gtb_mlp_sk_weight_count(C.c_int32(ns), C.c_int32(F), C.c_int32(Nb), C.c_int32(Hd)))
+    if weights.numel() != need:
+        raise GtbError(ERR_INVALID_ARG, "mlp_sk_hamiltonian", f"weight blob has {weights.numel()} doubles, {need} expected")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    n, K, dev = nbr.n, nbr.width, pos.device
+    H = Ell(4 * n, 4 * K, torch.empty((4 * K, 4 * n), dtype=torch.int32, device=dev),
+            torch.empty((4 * K, 4 * n), dtype=torch.float64, device=dev),
+            torch.empty(4 * n, dtype=torch.float64, device=dev) if with_diag else None)
+    v = torch.empty((n, F), dtype=torch.float64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    model = _MlpModel(ns, F, Nb, Hd, r_cut, weights.data_ptr())
+    nc, hc = nbr._c(), H._c()
+    st = lib().gtb_mlp_sk_hamiltonian(C.byref(model), C.byref(nc), _ptr(pos), _ptr(species),
+                                      C.c_void_p(box_h.ctypes.data), C.c_void_p(pbc_h.ctypes.data),
+                                      C.byref(hc), _ptr(v), _ptr(status), _stream())
+    _check(st, "mlp_sk_hamiltonian")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "mlp_sk_hamiltonian", "species index out of range")
+    return H

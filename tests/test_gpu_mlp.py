@@ -85,3 +85,28 @@ def test_other_instantiated_sizes_and_rejections():
     with pytest.raises(gtb.GtbError):            # species out of range is reported, not dereferenced
         gtb.mlp_hamiltonian(nbr_g, _dev(inp.pos), _dev(bad), inp.box, inp.pbc, (1, 8, 8, 16), RC,
                             _dev(W.mlp_weights((1, 8, 8, 16), 3)))
+
+
+@pytest.mark.parametrize("key,nx,ny,cutoff,kw", CASES)
+def test_mlp_feeding_the_slater_koster_blocks(key, nx, ny, cutoff, kw):
+    """Eq. 2 -> four bond integrals per pair -> s,p blocks; then moments with the blocked pass."""
+    w = W.CONFIGS[key].scaled(nx, ny, **kw)
+    inp = W.make_inputs(w)
+    ns = len(w.onsite)
+    blob = W.mlp_weights(DIMS, 21, hop_out=4, onsite_out=2)
+    ones = np.ones((ns, ns))
+    nbr_o = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, cutoff, [0.0] * ns, ones,
+                                     with_diag=False, method=1)
+    Ho = oracle.mlp_sk_hamiltonian(nbr_o, inp.pos, inp.species, inp.box, inp.pbc, DIMS, RC, blob)
+    nbr_g = gtb.build_hamiltonian(_dev(inp.pos), _dev(inp.species), inp.box, inp.pbc, cutoff, [0.0] * ns,
+                                  ones, with_diag=False)
+    Hg = gtb.mlp_sk_hamiltonian(nbr_g, _dev(inp.pos), _dev(inp.species), inp.box, inp.pbc, DIMS, RC, _dev(blob))
+    assert (Hg.cols.cpu().numpy() == Ho.cols).all()
+    scale = np.abs(Ho.vals).max()
+    assert np.abs(Hg.vals.cpu().numpy() - Ho.vals).max() <= 1e-12 * scale
+    assert np.abs(Hg.diag.cpu().numpy() - Ho.diag).max() <= 1e-12 * max(1.0, np.abs(Ho.diag).max())
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    ref = oracle.kpm_moments(Ho, a, b, 48, 4, 3, mode=0, algo=0)
+    got = gtb.kpm_moments(Hg, a, b, 48, 4, 4, 3, mode=gtb.MODE_ORB4, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-9 and np.abs(got - ref).max() <= 1e-11
