@@ -361,7 +361,9 @@ def run_ours(args):
                if "grouped_width" in state else "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
                ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
-               if (H.width > 4 or w.R >= 4) and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
+               if H.width > 4 and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
+               else "cheb_step_x2_kernel (K7x2: fused Chebyshev pass, two elements in flight per thread)"
+               if H.width <= 4 and w.R in (2, 4, 8) and os.environ.get("GTB_K7_X2", "1") != "0"
                else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
     roofline = {"bound": "hbm", "kernel": k7_name,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

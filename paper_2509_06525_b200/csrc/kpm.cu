@@ -212,6 +212,112 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
   }
 }
 
+// ---- K7x2: K7 for narrow rows with two independent elements in flight per thread --------------------
+// K7 above is latency-bound at K = 3 (ncu: 94 % of the stall cycles on long_scoreboard, DRAM at 76 %):
+// per element a thread issues its two streamed loads and the K column/hopping loads, and only then the K
+// gathers that depend on the columns.  Here every thread works on TWO elements per iteration, one grid
+// stride apart: all 2 x (2 + 2W) independent loads are issued first, then the 2 x W gathers, then the FMAs
+// and the two stores.  W (3 or 4) is a compile-time bound on the row width, so everything is unrolled and
+// lives in registers (64 registers: still 4 blocks per SM).  Same arithmetic order per element as K7.
+// Config 5: 2.20 -> 1.99 ms per pass.
+template <int LOG2T, bool kDiag, int W, bool kDotL>
+__global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int NE = 2;
+  const int64_t n = a.n;
+  const int64_t total = n * T;
+  const int width = a.width;
+  const double scale = a.scale, b = a.b;
+  const int64_t stride = (int64_t)gridDim.x * kBlock;
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e0 = (int64_t)blockIdx.x * kBlock + threadIdx.x; e0 < total; e0 += NE * stride) {
+    int64_t e[NE];
+    bool live[NE];
+#pragma unroll
+    for (int r = 0; r < NE; ++r) {
+      e[r] = e0 + r * stride;
+      live[r] = e[r] < total;
+      if (!live[r]) e[r] = e0;   // a harmless duplicate: loaded, never stored or summed
+    }
+    int64_t row[NE];
+    Vec<VW> prev[NE], own[NE], acc[NE], with[NE];
+    int32_t c[NE][W];
+    double v[NE][W];
+#pragma unroll
+    for (int r = 0; r < NE; ++r) {
+      row[r] = e[r] >> LOG2T;
+      prev[r] = load_stream<VW>(a.phi_io + e[r] * VW);
+      own[r] = load_gather<VW>(a.phi_cur + e[r] * VW);
+      if (kDotL) with[r] = load_stream<VW>(a.dot_with + e[r] * VW);
+#pragma unroll
+      for (int k = 0; k < W; ++k) {
+        const bool ok = k < width;
+        c[r][k] = ok ? __ldg(a.cols + (size_t)k * n + row[r]) : (int32_t)row[r];
+        v[r][k] = ok ? __ldg(a.vals + (size_t)k * n + row[r]) : 0.0;
+      }
+    }
+    Vec<VW> x[NE][W];
+#pragma unroll
+    for (int r = 0; r < NE; ++r) {
+      const double* xt = a.phi_cur + (e[r] - row[r] * T) * VW;
+#pragma unroll
+      for (int k = 0; k < W; ++k) x[r][k] = load_gather<VW>(xt + (int64_t)c[r][k] * T * VW);
+    }
+#pragma unroll
+    for (int r = 0; r < NE; ++r) {
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[r].v[q] = 0.0;
+#pragma unroll
+      for (int k = 0; k < W; ++k)
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc[r].v[q] = fma(v[r][k], x[r][k].v[q], acc[r].v[q]);
+      if (kDiag) {
+        const double d = __ldg(a.diag + row[r]);
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc[r].v[q] = fma(d, own[r].v[q], acc[r].v[q]);
+      }
+      if (live[r]) {
+        Vec<VW> y;
+#pragma unroll
+        for (int q = 0; q < VW; ++q) {
+          y.v[q] = (acc[r].v[q] - b * own[r].v[q]) * scale - prev[r].v[q];
+          s1 = fma(own[r].v[q], kDotL ? with[r].v[q] : own[r].v[q], s1);
+          s2 = fma(y.v[q], kDotL ? with[r].v[q] : own[r].v[q], s2);
+        }
+        store_stream<VW>(a.phi_io + e[r] * VW, y);
+      }
+    }
+  }
+  __shared__ double red[kBlock / 32][2];
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) {
+    red[wid][0] = s1;
+    red[wid][1] = s2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int w = 1; w < kBlock / 32; ++w) {
+      s1 += red[w][0];
+      s2 += red[w][1];
+    }
+    a.partial[blockIdx.x] = make_double2(s1, s2);
+  }
+}
+
+template <int LOG2T, int W, bool DOT>
+StepFn pick_x2(bool diag) {
+  return diag ? cheb_step_x2_kernel<LOG2T, true, W, DOT> : cheb_step_x2_kernel<LOG2T, false, W, DOT>;
+}
+template <int LOG2T>
+StepFn pick_x2(bool diag, int width, bool dot) {
+  if (width <= 3) return dot ? pick_x2<LOG2T, 3, true>(diag) : pick_x2<LOG2T, 3, false>(diag);
+  return dot ? pick_x2<LOG2T, 4, true>(diag) : pick_x2<LOG2T, 4, false>(diag);
+}
+
 // ---- K7t: the same pass with the Hamiltonian stream staged by TMA ------------------------------
 // With wide rows (K ~ 10-20) the register path above is latency-bound: every gather waits for a
 // column index that itself comes from HBM.  Here one lane-parallel producer (warp 0) copies the
@@ -1416,6 +1522,10 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
   else if (R == 8) { pick<4, 2>(diag, ch, dot, p); p->vw = 4; p->T = 4; log2t = 2; }
   else if (R == 1) { pick<2, 0>(diag, ch, dot, p); p->vw = 2; p->T = 1; }
   else { pick<2, -1>(diag, ch, dot, p); p->vw = 2; p->T = R; }
+  // K7x2: narrow rows (K <= 4) take the two-elements-in-flight kernel for every pass but the first
+  const bool x2 = env_int("GTB_K7_X2", 1) != 0 && log2t >= 0 && width >= 1 && width <= 4;
+  if (x2) p->next = log2t == 0 ? pick_x2<0>(diag, width, dot) : log2t == 1 ? pick_x2<1>(diag, width, dot)
+                                                                          : pick_x2<2>(diag, width, dot);
   int dev = 0, sms = kSmCount, per_sm = 0;
   GTB_CUDA_TRY(cudaGetDevice(&dev));
   GTB_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -1424,7 +1534,7 @@ int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p) {
                        !(reinterpret_cast<uintptr_t>(H->cols) & 15u) &&
                        !(reinterpret_cast<uintptr_t>(H->vals) & 15u) &&
                        !(reinterpret_cast<uintptr_t>(H->diag) & 15u);
-  int stages = env_int("GTB_K7_TILE", (width > 4 || R >= 4) ? 1 : 0) ? env_int("GTB_K7_STAGES", 2) : 0;
+  int stages = env_int("GTB_K7_TILE", width > 4 ? 1 : 0) ? env_int("GTB_K7_STAGES", 2) : 0;
   if (log2t < 0 || !aligned) stages = 0;
   p->stages = 0;
   if (stages > 0) {
