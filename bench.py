@@ -43,7 +43,7 @@ VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
 # `ncu --set full` captures summarised under profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = {
-    "c5-pristine-5000x5000": 13.178e9,     # profiles/r01_c5_k7_full.md (10.00 GB read + 3.18 GB written)
+    "c5-pristine-5000x5000": 13.355e9,     # profiles/r01_c5_k7_full.md, K7x2 (10.18 GB read + 3.18 GB written)
     "c2-disordered-500x500-rc4.0": 0.6125e9,    # profiles/r01_wide_k7_full.md (504.5 MB + 108.0 MB)
     "c3-disordered-1600x1600-rc4.0": 4.508e9,   # profiles/r01_wide_k7_full.md (3.865 GB + 643.5 MB)
 }
