@@ -334,6 +334,43 @@ def test_row_groups_need_a_multiple_of_four_rows():
         gtb.group_rows(Hg)
 
 
+# K7x2 (narrow rows: two elements in flight per thread) against the oracle's rows and against K7, on sizes
+# whose element count is odd in units of the grid stride, with width 3 and a padded width 4.
+@pytest.mark.parametrize("key,nx,ny,kw,R,width", [("c5", 57, 43, {}, 2, None), ("c5", 57, 43, {}, 8, 4),
+                                                   ("c4", 48, 21, {"stripe": 6}, 8, None),
+                                                   ("c1", 24, 24, {}, 4, 4), ("c5", 301, 127, {}, 2, None)])
+def test_two_elements_in_flight_path(monkeypatch, key, nx, ny, kw, R, width):
+    monkeypatch.setenv("GTB_K7_SMALL", "0")
+    monkeypatch.setenv("GTB_K7_TILE", "0")
+    w, inp = _small(key, nx, ny, kw)
+    Ho = _oracle_H(w, inp, width=width, with_diag=w.use_diag)
+    Hg = _gpu_H(w, inp, width=width, with_diag=w.use_diag)
+    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
+    n = Ho.n
+    phi0 = oracle.random_phase_fill(11, 0, R, n)
+    rows = np.arange(n) if n < 20000 else np.unique(np.r_[0:300, n - 300:n, np.arange(0, n, 97)])
+    phi1 = oracle.kpm_step_rows(Ho, a, b, True, None, phi0, np.arange(n))
+    phi2 = oracle.kpm_step_rows(Ho, a, b, False, phi0, phi1, rows)
+    out = {}
+    for x2 in ("1", "0"):
+        monkeypatch.setenv("GTB_K7_X2", x2)
+        g1, g0 = _dev(phi1), _dev(phi0)
+        s = gtb.kpm_step(Hg, a, b, False, g1, g0).cpu().numpy()       # g0 <- phi_2
+        out[x2] = g0.cpu().numpy()
+        assert np.abs(out[x2][rows] - phi2).max() <= 1e-14
+        assert s[0] == pytest.approx((phi1 * phi1).sum(), rel=1e-13)
+    assert (out["1"] == out["0"]).all()                               # same arithmetic per element
+    M = 33
+    ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0) if n < 20000 else None
+    monkeypatch.setenv("GTB_K7_X2", "1")
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
+    monkeypatch.setenv("GTB_K7_X2", "0")
+    old = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
+    assert np.abs(got - old).max() <= 1e-13
+    if ref is not None:
+        assert np.abs(got - ref).max() <= 1e-12
+
+
 @pytest.mark.parametrize("drop", [1, 2, 3])
 def test_atom_count_not_a_multiple_of_four_takes_the_register_path(drop):
     # bulk copies need 16-byte aligned slot rows (n % 4 == 0); any other n must still be exact
