@@ -212,6 +212,17 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
   }
 }
 
+__device__ __forceinline__ int32_t ld_stream_i32(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ double ld_stream_f64(const double* p) {
+  double v;
+  asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+
 // ---- K7x2: K7 for narrow rows with two independent elements in flight per thread --------------------
 // K7 above is latency-bound at K = 3 (ncu: 94 % of the stall cycles on long_scoreboard, DRAM at 76 %):
 // per element a thread issues its two streamed loads and the K column/hopping loads, and only then the K
@@ -253,8 +264,9 @@ __global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) 
 #pragma unroll
       for (int k = 0; k < W; ++k) {
         const bool ok = k < width;
-        c[r][k] = ok ? __ldg(a.cols + (size_t)k * n + row[r]) : (int32_t)row[r];
-        v[r][k] = ok ? __ldg(a.vals + (size_t)k * n + row[r]) : 0.0;
+        // the H stream is read once: keep it out of L1, which the gathers use
+        c[r][k] = ok ? ld_stream_i32(a.cols + (size_t)k * n + row[r]) : (int32_t)row[r];
+        v[r][k] = ok ? ld_stream_f64(a.vals + (size_t)k * n + row[r]) : 0.0;
       }
     }
     Vec<VW> x[NE][W];
