@@ -356,3 +356,21 @@ def mlp_sk_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, wei
     _check(lib().gtbo_mlp_sk_hamiltonian(C.byref(m), C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
                                          C.byref(hc)), "mlp_sk_hamiltonian")
     return H
+
+
+def carrier_density(rho, energies, e_ref: float) -> np.ndarray:
+    """n(E_j) = int_{e_ref}^{E_j} rho dE by the trapezoid rule (reading V7)."""
+    rho, energies = _f64(rho), _f64(energies)
+    out = np.zeros_like(rho)
+    _check(lib().gtbo_carrier_density(_p(rho), _p(energies), C.c_int32(rho.shape[0]), C.c_double(e_ref),
+                                      _p(out)), "carrier_density")
+    return out
+
+
+def mobility(sigma, n, scale: float = 1.0, n_min: float = 0.0) -> np.ndarray:
+    """mu = scale * sigma / |n| where |n| > n_min, else 0 (reading V8)."""
+    sigma, n = _f64(sigma), _f64(n)
+    out = np.zeros_like(sigma)
+    _check(lib().gtbo_mobility(_p(sigma), _p(n), C.c_int32(sigma.shape[0]), C.c_double(scale),
+                               C.c_double(n_min), _p(out)), "mobility")
+    return out

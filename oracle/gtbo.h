@@ -195,6 +195,12 @@ int gtbo_mlp_sk_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* nbr, const 
                             const int32_t* species, const double box[3], const int32_t pbc[3],
                             gtbo_ell* H);
 
+/* Fig. 4b post-processing (readings V7, V8 in gtbo_vac.cpp): n(E_j) = int_{e_ref}^{E_j} rho dE (trapezoid,
+ * rho interpolated at e_ref; energies strictly ascending, e_ref inside the grid);
+ * mu_j = scale * sigma_j / |n_j| where |n_j| > n_min, else 0. */
+int gtbo_carrier_density(const double* rho, const double* energies, int32_t G, double e_ref, double* n_out);
+int gtbo_mobility(const double* sigma, const double* n, int32_t G, double scale, double n_min, double* mu);
+
 #ifdef __cplusplus
 }
 #endif

@@ -237,3 +237,39 @@ extern "C" int gtbo_vac_conductivity(const double* C, int32_t M, int32_t n_steps
   if (rho_vv) std::memcpy(rho_vv, rv.data(), sizeof(double) * rv.size());
   return GTBO_OK;
 }
+
+// --- post-processing of Fig. 4b: carrier density and mobility --------------------
+// The paper plots mobility against carrier concentration and prints no formula; readings (DESIGN.md
+// sec. 11, V7-V8): V7 carrier density relative to the reference energy E_ref (the charge-neutrality
+// point), n(E_j) = int_{E_ref}^{E_j} rho(E) dE by the trapezoid rule on the given grid, with rho
+// interpolated linearly at E_ref; negative below E_ref (holes).  V8 semiclassical mobility
+// mu(E_j) = sigma(E_j) / (e |n(E_j)|) with e folded into `scale`; where |n| <= n_min the mobility is
+// reported as 0 (the neutrality point itself has no carriers to carry it).
+extern "C" int gtbo_carrier_density(const double* rho, const double* energies, int32_t G, double e_ref,
+                                    double* n_out) {
+  if (!rho || !energies || !n_out || G < 2) return GTBO_ERR_INVALID_ARG;
+  for (int32_t j = 1; j < G; ++j)
+    if (!(energies[j] > energies[j - 1])) return GTBO_ERR_INVALID_ARG;
+  if (!(e_ref >= energies[0] && e_ref <= energies[G - 1])) return GTBO_ERR_INVALID_ARG;
+  std::vector<double> cum(G, 0.0);   // int_{E_0}^{E_j}
+  for (int32_t j = 1; j < G; ++j)
+    cum[j] = cum[j - 1] + (energies[j] - energies[j - 1]) * (rho[j - 1] + rho[j]) / 2.0;
+  int32_t k = 0;                      // E_k <= e_ref <= E_{k+1}
+  while (k + 2 < G && energies[k + 1] < e_ref) ++k;
+  const double h = energies[k + 1] - energies[k];
+  const double t = (e_ref - energies[k]) / h;
+  const double rho_ref = rho[k] + t * (rho[k + 1] - rho[k]);
+  const double cum_ref = cum[k] + (e_ref - energies[k]) * (rho[k] + rho_ref) / 2.0;
+  for (int32_t j = 0; j < G; ++j) n_out[j] = cum[j] - cum_ref;
+  return GTBO_OK;
+}
+
+extern "C" int gtbo_mobility(const double* sigma, const double* n, int32_t G, double scale, double n_min,
+                             double* mu) {
+  if (!sigma || !n || !mu || G < 0 || !(n_min >= 0.0)) return GTBO_ERR_INVALID_ARG;
+  for (int32_t j = 0; j < G; ++j) {
+    const double a = std::fabs(n[j]);
+    mu[j] = a > n_min ? scale * sigma[j] / a : 0.0;
+  }
+  return GTBO_OK;
+}

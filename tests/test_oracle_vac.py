@@ -169,3 +169,30 @@ def test_vac_density_at_time_zero_is_non_negative_and_particle_hole_symmetric():
     assert rv[0].min() >= -1e-12                        # Tr[delta(E-H) V^2] >= 0 with a positive kernel
     assert np.abs(rv[0] - rv[0][::-1]).max() <= 1e-10   # bipartite lattice, zero onsite
     assert np.abs(Cm[0, 1::2]).max() <= 1e-12           # odd moments vanish for the same reason
+
+
+# ---------------------------------------------------------------------------------- P37 (Fig. 4b post-processing)
+def test_carrier_density_closed_forms_and_mobility():
+    E = np.linspace(-2.0, 3.0, 501)
+    # graphene-like DOS rho = |E|: n(E) = E|E|/2 relative to the neutrality point E = 0 (trapezoid is exact
+    # on the linear pieces; the grid contains 0)
+    n = oracle.carrier_density(np.abs(E), E, 0.0)
+    assert np.abs(n - E * np.abs(E) / 2).max() <= 1e-13
+    # constant DOS, reference off the grid points: n = rho0 (E - e_ref)
+    n = oracle.carrier_density(np.full_like(E, 0.7), E, 0.123456)
+    assert np.abs(n - 0.7 * (E - 0.123456)).max() <= 1e-13
+    # against numpy's trapezoid on a non-uniform grid, reference at a grid point
+    rng = np.random.default_rng(0)
+    Eg = np.sort(rng.uniform(-1, 1, 64))
+    rho = rng.uniform(0.1, 1.0, 64)
+    n = oracle.carrier_density(rho, Eg, Eg[20])
+    want = np.array([np.trapezoid(rho[20:j + 1], Eg[20:j + 1]) if j >= 20 else -np.trapezoid(rho[j:21], Eg[j:21])
+                     for j in range(64)])
+    assert np.abs(n - want).max() <= 1e-13
+    sigma = rng.uniform(0.0, 2.0, 64)
+    mu = oracle.mobility(sigma, n, scale=3.0, n_min=1e-6)
+    live = np.abs(n) > 1e-6
+    assert (mu[~live] == 0).all() and np.abs(mu[live] - 3.0 * sigma[live] / np.abs(n[live])).max() <= 1e-12
+    assert mu[20] == 0.0                                    # no carriers at the reference energy
+    with pytest.raises(oracle.OracleError):
+        oracle.carrier_density(rho, Eg, 2.0)                # reference outside the grid
