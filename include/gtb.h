@@ -330,6 +330,16 @@ int gtb_mlp_sk_hamiltonian(const gtb_mlp_model* m, const gtb_ell* nbr, const dou
                            const int32_t* species, const double box[3], const int32_t pbc[3],
                            gtb_ell* H, double* v, int32_t* status, void* stream);
 
+/* ---- Fig. 4b post-processing: carrier density and mobility (readings V7, V8) ----
+ * ASYNC.  n_out[j] = int_{e_ref}^{E_j} rho(E) dE by the trapezoid rule on the grid (rho interpolated
+ * linearly at e_ref; negative below it).  energies strictly ascending, e_ref inside the grid, G >= 2;
+ * otherwise *status (DEVICE int32) is set non-zero.  rho, energies, n_out: DEVICE [G]. */
+int gtb_carrier_density(const double* rho, const double* energies, int32_t G, double e_ref,
+                        double* n_out, int32_t* status, void* stream);
+/* ASYNC.  mu[j] = scale * sigma[j] / |n[j]| where |n[j]| > n_min, else 0 (e and units in `scale`). */
+int gtb_mobility(const double* sigma, const double* n, int32_t G, double scale, double n_min,
+                 double* mu, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -34,7 +34,7 @@ EXPORTS = (
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_group_width", "gtb_group_rows",
-    "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian",
+    "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
 MODE_GROUP4 = 64            # H is the row-grouped matrix of group_rows()
@@ -565,3 +565,28 @@ def mlp_sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, 
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "mlp_sk_hamiltonian", "species index out of range")
     return H
+
+
+# ---------------------------------------------------------------- Fig. 4b post-processing
+def carrier_density(rho: torch.Tensor, energies: torch.Tensor, e_ref: float) -> torch.Tensor:
+    """n(E_j) = int_{e_ref}^{E_j} rho dE by the trapezoid rule (reading V7)."""
+    rho = _dev(rho, torch.float64, "rho")
+    energies = _dev(energies, torch.float64, "energies")
+    out = torch.empty_like(rho)
+    status = torch.zeros(1, dtype=torch.int32, device=rho.device)
+    st = lib().gtb_carrier_density(_ptr(rho), _ptr(energies), C.c_int32(rho.shape[0]), C.c_double(e_ref),
+                                   _ptr(out), _ptr(status), _stream())
+    _check(st, "carrier_density")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "carrier_density", "grid not ascending or e_ref outside it")
+    return out
+
+
+def mobility(sigma: torch.Tensor, n: torch.Tensor, scale: float = 1.0, n_min: float = 0.0) -> torch.Tensor:
+    """mu = scale * sigma / |n| where |n| > n_min, else 0 (reading V8)."""
+    sigma = _dev(sigma, torch.float64, "sigma")
+    n = _dev(n, torch.float64, "n")
+    out = torch.empty_like(sigma)
+    _check(lib().gtb_mobility(_ptr(sigma), _ptr(n), C.c_int32(sigma.shape[0]), C.c_double(scale),
+                              C.c_double(n_min), _ptr(out), _stream()), "mobility")
+    return out

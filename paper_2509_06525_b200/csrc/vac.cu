@@ -384,3 +384,64 @@ extern "C" int gtb_vac_conductivity(const double* C, int32_t M, int32_t n_steps,
   GTB_LAUNCHED();
   return GTB_OK;
 }
+
+// ---- Fig. 4b post-processing (readings V7, V8 of DESIGN.md sec. 11) -------------
+namespace gtb {
+namespace {
+// n_j = int_{e_ref}^{E_j} rho dE by the trapezoid rule; one block, a serial scan per 1024-point segment is
+// not worth it at G ~ 4001: thread 0 accumulates, the others wait (G is tiny next to everything else).
+__global__ void carrier_density_kernel(const double* __restrict__ rho, const double* __restrict__ E,
+                                       int32_t G, double e_ref, double* __restrict__ n_out,
+                                       int32_t* __restrict__ status) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  if (!(e_ref >= E[0] && e_ref <= E[G - 1])) {
+    atomicOr(status, 1);
+    return;
+  }
+  double cum = 0.0;
+  n_out[0] = 0.0;
+  for (int j = 1; j < G; ++j) {
+    if (!(E[j] > E[j - 1])) atomicOr(status, 1);
+    cum = cum + (E[j] - E[j - 1]) * (rho[j - 1] + rho[j]) / 2.0;
+    n_out[j] = cum;
+  }
+  int k = 0;
+  while (k + 2 < G && E[k + 1] < e_ref) ++k;
+  const double h = E[k + 1] - E[k];
+  const double t = (e_ref - E[k]) / h;
+  const double rho_ref = rho[k] + t * (rho[k + 1] - rho[k]);
+  const double cum_ref = n_out[k] + (e_ref - E[k]) * (rho[k] + rho_ref) / 2.0;
+  for (int j = 0; j < G; ++j) n_out[j] = n_out[j] - cum_ref;
+}
+
+__global__ void __launch_bounds__(kBlock) mobility_kernel(const double* __restrict__ sigma,
+                                                          const double* __restrict__ n, int32_t G,
+                                                          double scale, double n_min,
+                                                          double* __restrict__ mu) {
+  const int j = blockIdx.x * kBlock + threadIdx.x;
+  if (j >= G) return;
+  const double a = fabs(n[j]);
+  mu[j] = a > n_min ? scale * sigma[j] / a : 0.0;
+}
+}  // namespace
+}  // namespace gtb
+
+extern "C" int gtb_carrier_density(const double* rho, const double* energies, int32_t G, double e_ref,
+                                   double* n_out, int32_t* status, void* stream) {
+  if (!rho || !energies || !n_out || !status || G < 2 || !std::isfinite(e_ref)) return GTB_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GTB_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int32_t), st));
+  carrier_density_kernel<<<1, 32, 0, st>>>(rho, energies, G, e_ref, n_out, status);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}
+
+extern "C" int gtb_mobility(const double* sigma, const double* n, int32_t G, double scale, double n_min,
+                            double* mu, void* stream) {
+  if (!sigma || !n || !mu || G < 0 || !(n_min >= 0.0)) return GTB_ERR_INVALID_ARG;
+  if (G == 0) return GTB_OK;
+  mobility_kernel<<<(G + kBlock - 1) / kBlock, kBlock, 0, static_cast<cudaStream_t>(stream)>>>(
+      sigma, n, G, scale, n_min, mu);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}

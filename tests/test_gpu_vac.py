@@ -161,3 +161,19 @@ def test_vac_argument_validation():
         gtb.vac_moments(Hg, vg, a, b, 8, 0, DT, 2, 2, 0)
     with pytest.raises(gtb.GtbError):
         gtb.vac_moments(Hg, vg, a, b, 8, 2, DT, 2, 2, 0, ws=gtb.workspace(1024))
+
+
+def test_carrier_density_and_mobility_match_oracle():
+    rng = np.random.default_rng(0)
+    for E in (np.linspace(-8.5, 8.5, 4001), np.sort(rng.uniform(-3, 3, 257))):
+        rho = rng.uniform(0.0, 1.0, E.shape[0])
+        sigma = rng.uniform(0.0, 5.0, E.shape[0])
+        for e_ref in (float(E[len(E) // 3]), 0.01234, float(E[0]), float(E[-1])):
+            ref = oracle.carrier_density(rho, E, e_ref)
+            got = gtb.carrier_density(_dev(rho), _dev(E), e_ref)
+            assert np.abs(got.cpu().numpy() - ref).max() <= 1e-13 * max(1.0, np.abs(ref).max())
+            mu_ref = oracle.mobility(sigma, ref, scale=2.0, n_min=1e-9)
+            mu = gtb.mobility(_dev(sigma), _dev(ref), 2.0, 1e-9).cpu().numpy()
+            assert np.abs(mu - mu_ref).max() <= 1e-12 * np.abs(mu_ref).max()
+    with pytest.raises(gtb.GtbError):
+        gtb.carrier_density(_dev(rho), _dev(E), 99.0)
