@@ -47,10 +47,15 @@ extern "C" int gtbo_sk_hamiltonian(const gtbo_ell* nbr, const double* pos, const
         const double f = model->beta == 0.0 ? 1.0 : std::exp(-model->beta * (r / model->r0 - 1.0));
         const double* V = model->sk + ((size_t)si * ns + sj) * 4;  // ss_sigma, sp_sigma, pp_sigma, pp_pi
         const double Vss = V[0] * f, Vsp = V[1] * f, Vpp_s = V[2] * f, Vpp_p = V[3] * f;
+        // H_ij^{p,s} = (-1)^{1+0} H_ji^{s,p}, and H_ji^{s,p} is made of the (s on j, p on i)
+        // integral, i.e. the table entry of the pair (s_j, s_i): with a species-asymmetric table
+        // (V_sp(A s, B p) != V_sp(B s, A p)) this is what keeps H symmetric.  The bond direction seen
+        // from j is -c, so H_ji^{s,p_a} = -c_a V_sp(ji) and E_{p_a,s} = H_ji^{s,p_a} = -c_a V_sp(ji).
+        const double Vsp_ji = model->sk[((size_t)sj * ns + si) * 4 + 1] * f;
         E[0][0] = Vss;
         for (int a = 0; a < 3; ++a) {
           E[0][1 + a] = c[a] * Vsp;
-          E[1 + a][0] = -(c[a] * Vsp);
+          E[1 + a][0] = -(c[a] * Vsp_ji);
           for (int b = 0; b < 3; ++b)
             E[1 + a][1 + b] = c[a] * c[b] * Vpp_s + ((a == b ? 1.0 : 0.0) - c[a] * c[b]) * Vpp_p;
         }

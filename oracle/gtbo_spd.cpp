@@ -107,8 +107,14 @@ extern "C" int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, cons
         const double r = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
         const double u[3] = {d[0] / r, d[1] / r, d[2] / r};
         const double f = model->beta == 0.0 ? 1.0 : std::exp(-model->beta * (r / model->r0 - 1.0));
-        double V[10];
-        for (int q = 0; q < 10; ++q) V[q] = model->sk[((size_t)si * ns + sj) * 10 + q] * f;
+        // V: integrals of the pair (s_i, s_j), used for l_a <= l_b; Vt: those of (s_j, s_i), used for
+        // l_a > l_b -- PAPER.md:88, H_ij^{l l'} = (-1)^{l+l'} H_ji^{l' l}: the (l_a > l_b) element of the
+        // (i, j) block is the (l_b, l_a) element of the (j, i) block, whose lower-l orbital sits on j.
+        double V[10], Vt[10];
+        for (int q = 0; q < 10; ++q) {
+          V[q] = model->sk[((size_t)si * ns + sj) * 10 + q] * f;
+          Vt[q] = model->sk[((size_t)sj * ns + si) * 10 + q] * f;
+        }
         double c[kOrb][5];
         frame_coefficients(u, c);
         for (int a = 0; a < kOrb; ++a)
@@ -116,7 +122,7 @@ extern "C" int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, cons
             const int la = kL[a], lb = kL[b];
             const int lo = la < lb ? la : lb, hi = la < lb ? lb : la;
             double s = 0.0;
-            for (int m = 0; m < 5; ++m) s += c[a][m] * integral(V, lo, hi, m) * c[b][m];
+            for (int m = 0; m < 5; ++m) s += c[a][m] * integral(la > lb ? Vt : V, lo, hi, m) * c[b][m];
             E[a][b] = (la > lb && ((la + lb) & 1)) ? -s : s;
           }
       }

@@ -131,3 +131,29 @@ def test_layout_padding_and_onsite():
             assert (H.vals[4 * k + nu][pad] == 0).all()
     assert np.allclose(H.diag.reshape(-1, 4), np.stack([ES + shift, EP + shift, EP + shift, EP + shift], 1),
                        rtol=0, atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------- P38
+@pytest.mark.parametrize("direction", [(0, 0, 1), (1, 2, -2), (-3, 1, 0.5)])
+def test_heteronuclear_diatomic_with_a_species_asymmetric_table(direction):
+    """H_ij^{p,s} = -H_ji^{s,p}, and H_ji^{s,p} carries the integral of (s on j, p on i), i.e.
+    the table entry of the species pair (s_j, s_i).  With V_sp(A s, B p) != V_sp(B s, A p) the sigma sector
+    in the basis (s_A, p_sigma_A, s_B, p_sigma_B), p_sigma pointing from A to B, is
+    [[es_A, 0, V_ss, V_sp(AB)], [0, ep_A, -V_sp(BA), V_pp_sigma], [., ., es_B, 0], [., ., 0, ep_B]]."""
+    sk = np.array([[[0.0] * 4, [-5.1, 4.2, 3.9, -2.2]], [[-5.1, 6.3, 3.9, -2.2], [0.0] * 4]])
+    es, ep = [-8.0, -5.5], [0.3, -1.1]
+    u = np.array(direction, dtype=float)
+    u /= np.linalg.norm(u)
+    pos = np.array([[5.0, 5.0, 5.0], [5.0, 5.0, 5.0] + 1.3 * u])
+    species = np.array([0, 1], dtype=np.int32)
+    nbr = oracle.build_hamiltonian(pos, species, [20.0] * 3, [0, 0, 0], 2.0, [0.0, 0.0], np.ones((2, 2)),
+                                   with_diag=False, method=0)
+    H = oracle.sk_hamiltonian(nbr, pos, species, [20.0] * 3, [0, 0, 0], es, ep, sk, r0=1.42).to_dense()
+    assert np.abs(H - H.T).max() <= 1e-14
+    vss, vsp_ab, vpps, vppp = sk[0, 1]
+    vsp_ba = sk[1, 0, 1]
+    sig = np.linalg.eigvalsh(np.array([[es[0], 0.0, vss, vsp_ab], [0.0, ep[0], -vsp_ba, vpps],
+                                       [vss, -vsp_ba, es[1], 0.0], [vsp_ab, vpps, 0.0, ep[1]]]))
+    pi = np.linalg.eigvalsh(np.array([[ep[0], vppp], [vppp, ep[1]]]))
+    want = np.sort(np.concatenate([sig, pi, pi]))
+    assert np.abs(np.linalg.eigvalsh(H) - want).max() <= 1e-13

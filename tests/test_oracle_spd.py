@@ -114,3 +114,59 @@ def test_layout_padding_and_onsite():
             assert (c[~pad] == 9 * j[~pad] + nu).all() and (c[pad] == rows[pad]).all()
             assert (H.vals[9 * k + nu][pad] == 0).all()
     assert (H.diag.reshape(-1, 9) == np.array([ES, EP, EP, EP, ED, ED, ED, ED, ED])).all()
+
+
+# ---------------------------------------------------------------------------------- P39
+def _asym_table(seed=3):
+    """[2][2][10], same-l integrals (ss, pp, dd) symmetric in the species pair, mixed-l ones
+    (sp_sigma, sd_sigma, pd_sigma, pd_pi) different for (A, B) and (B, A) -- the normal heteronuclear case."""
+    rng = np.random.default_rng(seed)
+    t = rng.uniform(-3.0, 3.0, (2, 2, 10))
+    for q in (0, 2, 3, 7, 8, 9):
+        t[1, 0, q] = t[0, 1, q]
+    return t
+
+
+@pytest.mark.parametrize("u", [(0, 0, 1), (1, 2, -2), (-3, 1, 0.5)])
+def test_heteronuclear_diatomic_with_a_species_asymmetric_table(u):
+    """PAPER.md:88, H_ij^{l l'} = (-1)^{l+l'} H_ji^{l' l}: the (l_a > l_b) element of the (A, B) block is made
+    of the (B, A) integral.  Closed form by m-sectors with orbitals of both atoms quantised along the bond
+    A -> B: <l_A|H|l'_B> = V_{l l'}(AB) for l <= l', (-1)^{l+l'} V_{l' l}(BA) for l > l'.  A wrong species
+    order in any mixed-l element changes the spectrum (the (A,B) and (B,A) entries differ by O(1))."""
+    t = _asym_table()
+    es, ep, ed = [-8.0, -5.5], [0.3, -1.1], [6.5, 4.0]
+    u = np.asarray(u, dtype=float) / np.linalg.norm(u)
+    pos = np.array([[5.0, 5.0, 5.0], 5.0 + 1.3 * u])
+    species = np.array([0, 1], dtype=np.int32)
+    nbr = oracle.build_hamiltonian(pos, species, [30.0] * 3, [0, 0, 0], 2.0, [0.0, 0.0], np.ones((2, 2)),
+                                   with_diag=False, method=0)
+    H = oracle.spd_hamiltonian(nbr, pos, species, [30.0] * 3, [0, 0, 0], es, ep, ed, t, r0=1.42).to_dense()
+    assert np.abs(H - H.T).max() <= 1e-14
+    ab, ba = t[0, 1], t[1, 0]
+    def sector(on_a, on_b, T):
+        return np.linalg.eigvalsh(np.block([[np.diag(on_a), T], [T.T, np.diag(on_b)]]))
+    sig = sector([es[0], ep[0], ed[0]], [es[1], ep[1], ed[1]],
+                 np.array([[ab[0], ab[1], ab[4]], [-ba[1], ab[2], ab[5]], [ba[4], -ba[5], ab[7]]]))
+    pi = sector([ep[0], ed[0]], [ep[1], ed[1]], np.array([[ab[3], ab[6]], [-ba[6], ab[8]]]))
+    dl = sector([ed[0]], [ed[1]], np.array([[ab[9]]]))
+    want = np.sort(np.concatenate([sig, pi, pi, dl, dl]))
+    assert np.abs(np.linalg.eigvalsh(H) - want).max() <= 1e-13
+
+
+def test_asymmetric_table_keeps_h_symmetric_and_the_doubling_identities_valid():
+    """On a two-species disordered lattice: H = H^T, and the direct and the doubling moments agree (the
+    identities need a symmetric H)."""
+    w = W.CONFIGS["c4"].scaled(6, 3, stripe=3)
+    inp = W.make_inputs(w)
+    species = (inp.species > 0).astype(np.int32)
+    nbr = oracle.build_hamiltonian(inp.pos, species, inp.box, inp.pbc, 2.65, [0.0, 0.0], np.ones((2, 2)),
+                                   with_diag=False)
+    H = oracle.spd_hamiltonian(nbr, inp.pos, species, inp.box, inp.pbc, [-8.0, -5.5], [0.3, -1.1], [6.5, 4.0],
+                               _asym_table(), r0=1.42, beta=1.5)
+    D = H.to_dense()
+    assert np.abs(D - D.T).max() <= 1e-13
+    lo, hi = oracle.spectral_bounds(H)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    m0 = oracle.kpm_moments(H, a, b, 24, 2, 7, mode=0, algo=0)
+    m1 = oracle.kpm_moments(H, a, b, 24, 2, 7, mode=0, algo=1)
+    assert np.abs(m0 - m1).max() <= 1e-12
