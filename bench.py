@@ -34,26 +34,24 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
-GROUPED = os.environ.get("GTB_BENCH_GROUPED", "0") != "0"   # opt-in: K7g (row groups) for wide single-orbital rows
+KERNEL = "auto"                 # set by --kernel: pins the fused-pass kernel through gtb_kpm_options
 HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
 ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom), "sp" (4) or "spd" (9)
 ORB_COUNT = {"pz": 1, "sp": 4, "spd": 9}
 VAC_DT = 0.1 / 0.6582119569     # the paper's 0.1 fs time step in hbar/eV
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused pass (K7), from the
-# `ncu --set full` captures summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {
-    "c5-pristine-5000x5000": 13.355e9,     # profiles/r01_c5_k7_full.md, K7x2 (10.18 GB read + 3.18 GB written)
-    "c2-disordered-500x500-rc4.0": 0.6125e9,    # profiles/r01_wide_k7_full.md (504.5 MB + 108.0 MB)
-    "c3-disordered-1600x1600-rc4.0": 4.508e9,   # profiles/r01_wide_k7_full.md (3.865 GB + 643.5 MB)
-}
-
-
-# the same for the bra-dot pass of the VAC path (profiles/r01_vac_c2.md)
-NCU_TRAFFIC_VAC_BYTES = {
-    "c2-disordered-500x500-rc4.0": 0.7451e9,    # 632.9 MB read + 112.2 MB written
-    "c5-pristine-5000x5000": 16.383e9,          # 13.20 GB read + 3.18 GB written
-}
+def _ncu_traffic(quantity: str, key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from
+    profiles/traffic.json (written from `ncu --set full` captures by
+    `python -m paper_2509_06525_b200.ncu_traffic`; the .md next to it names the commands).
+    None when no capture of this configuration exists."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            entry = json.load(f).get(quantity, {}).get(key)
+    except (OSError, ValueError):
+        return None
+    return float(entry["dram_bytes_per_launch"]) if entry else None
 
 
 def _peaks():
@@ -264,9 +262,15 @@ def run_ours(args):
     if HOPPING == "mlp":
         state["mlp_w"] = torch.from_numpy(W.mlp_weights()).to(dev)
 
+    timer = gtb.LoopTimer()
+    opt = gtb.options(kernel={"auto": gtb.KERNEL_AUTO, "row": gtb.KERNEL_ROW, "row_x2": gtb.KERNEL_ROW_X2,
+                              "tile": gtb.KERNEL_TILE}[KERNEL], timer=timer)
+
     def step(pos, spec, shift):
+        # the width is a property of (lattice, cutoff) found once above (gtb_neighbor_width): the
+        # assembly checks it (GTB_ERR_ELL_OVERFLOW), so the neighbour search runs once per step
         H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
-                                  w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
+                                  w.beta, shift, width=width, with_diag=w.use_diag, ws=ws_build)
         if HOPPING == "mlp":   # Eq. 2: descriptor + MLPs on the neighbour lists just built
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
@@ -289,15 +293,12 @@ def run_ours(args):
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        Hk, kmode = H, {"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0)
-        if GROUPED and ORBITALS == "pz" and H.width > 4 and n % 4 == 0 and w.R in (2, 4, 8):
-            Hk, kmode = gtb.group_rows(H), gtb.MODE_GROUP4     # K7g: part of the timed step
-            state["grouped_width"] = Hk.width
-        gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu)
+        kmode = {"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0)
+        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         rho = gtb.dos(mu, a, b, state["E"])
-        state["H"], state["a"], state["b"] = H, a, b
+        state["H"], state["a"], state["b"], state["rho"] = H, a, b, rho
         return rho
 
     def barrier():
@@ -311,7 +312,7 @@ def run_ours(args):
         e0.record()
         for _ in range(steps):
             fn()
-            ms, passes = gtb.kpm_last_loop_ms()     # CUDA events on the launching stream
+            ms, passes = timer.ms()                 # CUDA events on the launching stream
             loop_ms += ms
             loop_passes += passes
         e1.record()
@@ -338,13 +339,18 @@ def run_ours(args):
     for _ in range(min(args.warmup, 1)):
         e2e_step()
     ms_e2e, _, _, _ = timed(e2e_step, args.steps)
+    # a diverged or non-finite run must not print a throughput
+    gtb.kpm_status(ws_kpm)
+    rho_h = state["rho"].cpu().numpy()
+    if not (np.isfinite(rho_h).all() and rho_h.max() > 0.0):
+        raise SystemExit("bench.py: the density of states is not finite / not positive; no number is reported")
 
     units = float(n_orb) * w.M * w.R * args.steps        # per rank
     value = replicas.whole_job_value(units, ms)
     e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
-    orb4 = ORBITALS != "pz" and os.environ.get("GTB_K7_ORB4", "1") != "0" and w.R in (2, 4, 8)
+    orb4 = ORBITALS != "pz" and w.R in (2, 4, 8)
     B = ORB_COUNT[ORBITALS]
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
     if orb4:   # per orbital row: K blocks of (4 B column + 8 B^2 B values) shared by B rows, + diag + vectors
@@ -353,22 +359,20 @@ def run_ours(args):
     k7_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k7_ms * 1e-3) / 1e9
-    small = (not orb4 and w.R in (2, 4, 8) and n_orb * (w.R // 2) <= 148 * 4 * 256
-             and os.environ.get("GTB_K7_SMALL", "1") != "0" and os.environ.get("GTB_K7_SWEEP", "0") == "0")
-    if "grouped_width" in state:
-        small = orb4 = False
-    k7_name = ("cheb_grp4_kernel (K7g: fused Chebyshev pass on groups of 4 rows, union width %d)" % state["grouped_width"]
-               if "grouped_width" in state else "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
+    small = not orb4 and KERNEL == "auto" and w.R in (2, 4, 8) and n_orb * (w.R // 2) <= 148 * 4 * 256
+    vec = w.R in (2, 4, 8)
+    tile = KERNEL == "tile" or (KERNEL == "auto" and H.width > 4 and n % 4 == 0 and vec)
+    x2 = KERNEL == "row_x2" or (KERNEL == "auto" and H.width <= 4 and vec)
+    k7_name = ("cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
                ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
-               "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)"
-               if H.width > 4 and os.environ.get("GTB_K7_TILE", "1") != "0" and n % 4 == 0
-               else "cheb_step_x2_kernel (K7x2: fused Chebyshev pass, two elements in flight per thread)"
-               if H.width <= 4 and w.R in (2, 4, 8) and os.environ.get("GTB_K7_X2", "1") != "0"
-               else "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
+               "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)" if tile else
+               "cheb_step_x2_kernel (K7x2: fused Chebyshev pass, two elements in flight per thread)" if x2 else
+               "cheb_step_kernel (K7: fused Chebyshev pass, register path)")
     roofline = {"bound": "hbm", "kernel": k7_name,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+                "traffic": _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS, w.name)
+                if KERNEL == "auto" else None,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "bytes_per_atom_pass": per_atom,
                 "ms_per_launch": k7_ms, "launches_timed": loop_passes,
                 "share_of_step": loop_ms / ms}
@@ -440,17 +444,20 @@ def run_vac(args):
     Cm = torch.empty((T, w.M), dtype=torch.float64, device=dev)
     h_sigma = torch.empty((T, w.n_energies), dtype=torch.float64).pin_memory()
     state = {}
+    width = gtb.neighbor_width(d_pos, inp.box, inp.pbc, w.cutoff, ws=ws_build)
+    timer = gtb.LoopTimer()
+    opt = gtb.options(timer=timer)
 
     def step(pos, spec, shift):
         H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
-                                  w.beta, shift, width=None, with_diag=w.use_diag, ws=ws_build)
+                                  w.beta, shift, width=width, with_diag=w.use_diag, ws=ws_build)
         if w.a is None:
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
         vv = gtb.velocity_ell(H, pos, inp.box, inp.pbc, 0)
-        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, ws=ws_vac, out=Cm)
+        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, ws=ws_vac, out=Cm, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         _, sigma = gtb.vac_conductivity(Cm, a, b, state["E"], VAC_DT)
@@ -465,7 +472,7 @@ def run_vac(args):
         e0.record()
         for _ in range(steps):
             fn()
-            ms, passes = gtb.vac_last_loop_ms()
+            ms, passes = timer.ms()
             loop_ms += ms
             loop_passes += passes
         e1.record()
@@ -513,7 +520,7 @@ def run_vac(args):
             "roofline": {"bound": "hbm", "kernel": "fused Chebyshev pass, dot products against the evolved bra "
                                                    "(cheb_tile_kernel / cheb_step_kernel, kDotL variant)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "peak_source": peak_src, "traffic": NCU_TRAFFIC_VAC_BYTES.get(w.name),
+                         "peak_source": peak_src, "traffic": _ncu_traffic("vac", w.name),
                          "algorithmic_bytes_per_launch": bytes_per_launch,
                          "bytes_per_atom_pass": per_atom, "ms_per_launch": k_ms,
                          "launches_timed": loop_passes,
@@ -547,10 +554,13 @@ def main():
     p.add_argument("--time-steps", type=int, default=24, help="vac: points of the time grid (dt = 0.1 fs)")
     p.add_argument("--hopping", default="analytic", choices=["analytic", "mlp"],
                    help="analytic: t(r) of the configs; mlp: descriptor + MLPs of Eq. 2 with synthetic weights (NEXT-3)")
+    p.add_argument("--kernel", default="auto", choices=["auto", "row", "row_x2", "tile"],
+                   help="pin the fused-pass kernel (gtb_kpm_options.kernel); auto: picked from the matrix shape")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS, HOPPING
+    global ORBITALS, HOPPING, KERNEL
+    KERNEL = args.kernel
     ORBITALS = args.orbitals
     HOPPING = args.hopping
     if args.hopping == "mlp" and (args.orbitals != "pz" or args.quantity == "vac"):

@@ -58,8 +58,9 @@ enum {
 };
 
 #define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian  (4 orbitals) */
-#define GTB_MODE_GROUP4 64 /* ... H is the row-grouped matrix written by gtb_group_rows                    */
 #define GTB_MODE_ORB9 32 /* ... from gtb_spd_hamiltonian (9 orbitals per atom)                           */
+#define GTB_MODE_BLOCK9 64  /* ... H holds the 9x9 blocks written by gtb_spd_blocks (H->n = atoms)          */
+#define GTB_MODE_BOND9 128  /* ... H holds the bond description written by gtb_spd_bonds (matrix-free)      */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
 
@@ -83,6 +84,32 @@ typedef struct gtb_ell {
   double* vals;   /* [width][n] */
   double* diag;   /* [n] or NULL */
 } gtb_ell;
+
+/* Kernel selection and timing hooks of the fused Chebyshev pass, for callers that need to pin a
+ * kernel (the parity tests compare every variant with the oracle; bench.py times them).  Passing
+ * NULL wherever a `const gtb_kpm_options*` is taken means "all zero": the library picks the kernel
+ * from the matrix shape.  The library never reads the environment. */
+enum {
+  GTB_KERNEL_AUTO = 0,
+  GTB_KERNEL_ROW = 1,    /* K7: one 256-bit element per thread per iteration (any width)              */
+  GTB_KERNEL_ROW_X2 = 2, /* K7x2: two elements in flight per thread; width <= 4, R in {2,4,8}          */
+  GTB_KERNEL_TILE = 3    /* K7t: ELL slots staged by TMA; R in {2,4,8}, n % 4 == 0, 16-byte aligned H  */
+};
+#define GTB_OPT_PER_PASS_LAUNCH 1 /* never fold a small system's passes into one cooperative launch (K7p) */
+#define GTB_OPT_SCALAR_BLOCKS 2   /* ignore GTB_MODE_ORB4 / ORB9: run the scalar kernels on the expanded H */
+#define GTB_OPT_BLOCK_DIRECT 4    /* K7b9: strided block loads instead of the shared-memory hand-off      */
+typedef struct gtb_kpm_options {
+  int32_t kernel;       /* GTB_KERNEL_*; a kernel that cannot take (H, R_batch) -> GTB_ERR_INVALID_ARG  */
+  int32_t tile_stages;  /* K7t ring depth, 1..8; 0 = default (2)                                       */
+  int32_t flags;        /* GTB_OPT_*                                                                   */
+  /* Timing hooks: caller-owned cudaEvent_t (as void*) or NULL.  If both are given they are recorded
+   * on `stream` around the recursion loop of the LAST batch (first pass excluded; gtb_vac_moments:
+   * around the M-1 moment passes of the last time step), and *loop_passes (HOST, may be NULL)
+   * receives the number of fused passes between them.  The library keeps no timing state. */
+  void* loop_begin;
+  void* loop_end;
+  int32_t* loop_passes;
+} gtb_kpm_options;
 
 /* ---- status -------------------------------------------------------------- */
 const char* gtb_status_string(int status);
@@ -138,13 +165,12 @@ int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, doubl
  *         written by gtb_sk_hamiltonian (4 orbitals per atom; gtb_spd_hamiltonian: 9); the fused pass
  *         then works on whole 4x4 (9x9) blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
  *         when R_batch is not 2, 4 or 8.  A matrix without that structure gives wrong results.
- * mode | GTB_MODE_GROUP4: H is the row-grouped matrix of gtb_group_rows (R_batch must be 2, 4 or 8).
  * R_batch: 1..64.  R_batch in {2,4,8} takes the 256-bit vector path.
  * ASYNC.  mu is DEVICE [M].  Workspace: gtb_kpm_workspace_bytes(n, M, R_batch). */
 size_t gtb_kpm_workspace_bytes(int64_t n, int32_t M, int32_t R_batch);
 int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
                     int32_t R_batch, uint64_t seed, int32_t mode, double* mu, void* ws,
-                    size_t ws_bytes, void* stream);
+                    size_t ws_bytes, void* stream, const gtb_kpm_options* opt);
 
 /* SYNC.  GTB_ERR_DIVERGED if the last gtb_kpm_moments run on this workspace
  * produced a non-finite moment, else GTB_OK. */
@@ -158,13 +184,7 @@ int gtb_kpm_status(const void* ws, void* stream);
  * Workspace: gtb_kpm_workspace_bytes(n, 2, R). */
 int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
                  const double* phi_cur, double* phi_io, double* sums, void* ws, size_t ws_bytes,
-                 void* stream);
-
-/* Timing of the recursion loop inside the LAST gtb_kpm_moments call of this
- * thread (CUDA events recorded on the caller's stream around the fused passes,
- * first pass excluded).  SYNC (waits for the closing event).
- * *ms = device milliseconds, *passes = fused passes between the events. */
-int gtb_kpm_last_loop_ms(double* ms, int32_t* passes);
+                 void* stream, const gtb_kpm_options* opt);
 
 /* ---- density of states (Eq. 4; north_star (4); reading C6) ---- */
 /* ASYNC.  rho(E_j) = scale*[g_0 mu_0 + 2 sum_{n=1}^{M-1} g_n mu_n T_n(x_j)] / (pi a sqrt(1-x_j^2)),
@@ -215,10 +235,8 @@ int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32_t R, doubl
 size_t gtb_vac_workspace_bytes(int64_t n, int32_t M, int32_t n_steps, int32_t R_batch);
 int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, double b, int32_t M,
                     int32_t n_steps, double dt, int32_t R_total, int32_t R_batch, uint64_t seed,
-                    int32_t mode, double* C, void* ws, size_t ws_bytes, void* stream);
-/* SYNC.  Device time of the M-1 moment passes of the LAST time step of the last
- * gtb_vac_moments call of this thread (CUDA events on the caller's stream). */
-int gtb_vac_last_loop_ms(double* ms, int32_t* passes);
+                    int32_t mode, double* C, void* ws, size_t ws_bytes, void* stream,
+                    const gtb_kpm_options* opt);
 
 /* ASYNC.  V5/V6: rho_vv[j][g] = kernel-damped reconstruction of C[j][:] at E_g exactly as
  * gtb_dos (scale 1); sigma[0][g] = 0, sigma[j][g] = sigma[j-1][g] + scale*dt*(rho_vv[j-1][g] +
@@ -303,19 +321,6 @@ size_t gtb_spd_workspace_bytes(void);
 int gtb_spd_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* species,
                         const double box[3], const int32_t pbc[3], const gtb_spd_model* model,
                         gtb_ell* H, int32_t* status, void* ws, size_t ws_bytes, void* stream);
-
-/* ---- row groups: 4 consecutive rows share their gathered neighbours (K7g) ----
- * A re-arrangement of an ELL matrix for the fused pass, not a different operator: for rows 4g..4g+3 the
- * ascending UNION of their column lists (padding slots skipped) and, per union column, the 4 values (zero
- * where a row lacks the column).  Layout of the grouped matrix G (a gtb_ell read differently):
- *   G->n = H->n (a multiple of 4), G->width = U = largest union, G->cols int32 [U][n/4] (row indices),
- *   G->vals double [U][n/4][4] (32-byte aligned), G->diag = H->diag or NULL; unused slots hold column 4g, zeros.
- * gtb_kpm_moments(G, ..., mode | GTB_MODE_GROUP4) then gathers each neighbour once per group instead of
- * once per row.  Same moments (the per-row sums run over the same non-zero terms in the same order). */
-/* SYNC.  *width_out (HOST) = U.  scratch: DEVICE int32. */
-int gtb_group_width(const gtb_ell* H, int32_t* scratch, void* stream, int32_t* width_out);
-/* SYNC.  Fills G->cols, G->vals (caller-allocated for G->width); GTB_ERR_ELL_OVERFLOW if G->width < U. */
-int gtb_group_rows(const gtb_ell* H, gtb_ell* G, int32_t* scratch, void* stream);
 
 /* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
  *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):

@@ -29,15 +29,16 @@ EXPORTS = (
     "gtb_build_workspace_bytes", "gtb_neighbor_width", "gtb_build_hamiltonian",
     "gtb_bounds_workspace_bytes", "gtb_spectral_bounds", "gtb_random_phase_fill",
     "gtb_kpm_workspace_bytes", "gtb_kpm_moments", "gtb_kpm_status", "gtb_kpm_step",
-    "gtb_kpm_last_loop_ms", "gtb_dos", "gtb_jackson",
+    "gtb_dos", "gtb_jackson",
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
-    "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_last_loop_ms", "gtb_vac_conductivity",
+    "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
-    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_group_width", "gtb_group_rows",
+    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
-MODE_GROUP4 = 64            # H is the row-grouped matrix of group_rows()
+KERNEL_AUTO, KERNEL_ROW, KERNEL_ROW_X2, KERNEL_TILE = 0, 1, 2, 3      # gtb_kpm_options.kernel
+OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT = 1, 2, 4     # gtb_kpm_options.flags
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
@@ -60,6 +61,45 @@ class _Model(C.Structure):
 class _Ell(C.Structure):
     _fields_ = [("n", C.c_int64), ("width", C.c_int32), ("cols", C.c_void_p),
                 ("vals", C.c_void_p), ("diag", C.c_void_p)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("tile_stages", C.c_int32), ("flags", C.c_int32),
+                ("loop_begin", C.c_void_p), ("loop_end", C.c_void_p),
+                ("loop_passes", C.POINTER(C.c_int32))]
+
+
+class LoopTimer:
+    """Caller-owned CUDA events for the timing hooks of gtb_kpm_options (the library records them
+    around its recursion loop; it keeps no timing state of its own)."""
+
+    def __init__(self):
+        self.begin = torch.cuda.Event(enable_timing=True)
+        self.end = torch.cuda.Event(enable_timing=True)
+        self.begin.record()      # torch creates the cudaEvent_t at the first record
+        self.end.record()
+        self.passes = C.c_int32(0)
+
+    def ms(self):
+        """(device milliseconds between the two events, fused passes between them); waits for `end`."""
+        self.end.synchronize()
+        return float(self.begin.elapsed_time(self.end)), int(self.passes.value)
+
+
+def options(kernel: int = KERNEL_AUTO, tile_stages: int = 0, flags: int = 0,
+            timer: Optional[LoopTimer] = None) -> _Options:
+    """A gtb_kpm_options value (argument marshalling only)."""
+    o = _Options(kernel, tile_stages, flags, None, None, None)
+    if timer is not None:
+        o.loop_begin = timer.begin.cuda_event
+        o.loop_end = timer.end.cuda_event
+        o.loop_passes = C.pointer(timer.passes)
+        o._timer = timer         # keep the events alive as long as the struct
+    return o
+
+
+def _opt(o: Optional[_Options]):
+    return C.byref(o) if o is not None else None
 
 
 _lib: Optional[C.CDLL] = None
@@ -252,7 +292,7 @@ def random_phase_fill(seed: int, r0: int, R: int, n: int, device="cuda") -> torc
 def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
                 R_batch: Optional[int] = None, seed: int = 0, mode: int = 0,
                 ws: Optional[torch.Tensor] = None, mu: Optional[torch.Tensor] = None,
-                check: bool = False) -> torch.Tensor:
+                check: bool = False, opt: Optional[_Options] = None) -> torch.Tensor:
     dev = H.vals.device if H.width else H.diag.device
     if R_batch is None:
         R_batch = R_total if (mode & 1) == 0 else 8
@@ -264,7 +304,7 @@ def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
     st = lib().gtb_kpm_moments(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(M),
                                C.c_int32(R_total), C.c_int32(R_batch),
                                C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode), _ptr(mu), _ptr(ws),
-                               C.c_size_t(ws.numel()), _stream())
+                               C.c_size_t(ws.numel()), _stream(), _opt(opt))
     _check(st, "kpm_moments")
     if check:
         kpm_status(ws)
@@ -276,7 +316,7 @@ def kpm_status(ws: torch.Tensor) -> None:
 
 
 def kpm_step(H: Ell, a: float, b: float, first: bool, phi_cur: torch.Tensor, phi_io: torch.Tensor,
-             ws: Optional[torch.Tensor] = None) -> torch.Tensor:
+             ws: Optional[torch.Tensor] = None, opt: Optional[_Options] = None) -> torch.Tensor:
     """One fused pass; phi_io is overwritten with phi_{n+1}.  Returns the two sums (device [2])."""
     phi_cur = _dev(phi_cur, torch.float64, "phi_cur")
     phi_io = _dev(phi_io, torch.float64, "phi_io")
@@ -287,15 +327,9 @@ def kpm_step(H: Ell, a: float, b: float, first: bool, phi_cur: torch.Tensor, phi
     hc = H._c()
     st = lib().gtb_kpm_step(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(int(first)),
                             C.c_int32(R), _ptr(phi_cur), _ptr(phi_io), _ptr(sums), _ptr(ws),
-                            C.c_size_t(ws.numel()), _stream())
+                            C.c_size_t(ws.numel()), _stream(), _opt(opt))
     _check(st, "kpm_step")
     return sums
-
-
-def kpm_last_loop_ms():
-    ms, passes = C.c_double(0.0), C.c_int32(0)
-    _check(lib().gtb_kpm_last_loop_ms(C.byref(ms), C.byref(passes)), "kpm_last_loop_ms")
-    return float(ms.value), int(passes.value)
 
 
 def dos(mu: torch.Tensor, a: float, b: float, energies: torch.Tensor, kernel: int = 1,
@@ -367,7 +401,7 @@ def evolve(H: Ell, a: float, b: float, dt: float, phi: torch.Tensor,
 def vac_moments(H: Ell, vvals: torch.Tensor, a: float, b: float, M: int, n_steps: int, dt: float,
                 R_total: int = 1, R_batch: Optional[int] = None, seed: int = 0, mode: int = 0,
                 ws: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
-                check: bool = False) -> torch.Tensor:
+                check: bool = False, opt: Optional[_Options] = None) -> torch.Tensor:
     """C[j][n], j < n_steps, n < M (readings V2, V3)."""
     dev = H.vals.device
     if R_batch is None:
@@ -380,17 +414,11 @@ def vac_moments(H: Ell, vvals: torch.Tensor, a: float, b: float, M: int, n_steps
     st = lib().gtb_vac_moments(C.byref(hc), _ptr(vvals), C.c_double(a), C.c_double(b), C.c_int32(M),
                                C.c_int32(n_steps), C.c_double(dt), C.c_int32(R_total),
                                C.c_int32(R_batch), C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode),
-                               _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream())
+                               _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream(), _opt(opt))
     _check(st, "vac_moments")
     if check:
         kpm_status(ws)
     return out
-
-
-def vac_last_loop_ms():
-    ms, passes = C.c_double(0.0), C.c_int32(0)
-    _check(lib().gtb_vac_last_loop_ms(C.byref(ms), C.byref(passes)), "vac_last_loop_ms")
-    return float(ms.value), int(passes.value)
 
 
 def vac_conductivity(Cm: torch.Tensor, a: float, b: float, energies: torch.Tensor, dt: float,
@@ -518,23 +546,6 @@ def spd_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "spd_hamiltonian", "species index out of range")
     return H
-
-
-# ---------------------------------------------------------------- row groups (K7g)
-def group_rows(H: Ell) -> Ell:
-    """The row-grouped re-arrangement of H for kpm_moments(..., mode=MODE_GROUP4): cols [U][n/4],
-    vals [U][n/4][4]; the diagonal array is shared."""
-    dev = H.vals.device
-    scratch = torch.zeros(1, dtype=torch.int32, device=dev)
-    U = C.c_int32(0)
-    hc = H._c()
-    _check(lib().gtb_group_width(C.byref(hc), _ptr(scratch), _stream(), C.byref(U)), "group_width")
-    ng = H.n // 4
-    G = Ell(H.n, int(U.value), torch.empty((U.value, ng), dtype=torch.int32, device=dev),
-            torch.empty((U.value, ng, 4), dtype=torch.float64, device=dev), H.diag)
-    gc = G._c()
-    _check(lib().gtb_group_rows(C.byref(hc), C.byref(gc), _ptr(scratch), _stream()), "group_rows")
-    return G
 
 
 def mlp_sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, dims, r_cut: float,

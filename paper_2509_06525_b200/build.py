@@ -10,6 +10,7 @@ import glob
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
@@ -41,16 +42,39 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """One nvcc -c per source file (in parallel, objects under csrc/build/), then one link."""
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    tmp = LIB + ".tmp"
-    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("GTB_NVCC_EXTRA", "").split(), "-I", INCLUDE, "-I", CSRC, "-shared", "-o", tmp, *sources()]
-    res = subprocess.run(cmd, cwd=HERE, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
+    extra = os.environ.get("GTB_NVCC_EXTRA", "").split()
+    objdir = os.path.join(CSRC, "build")
+    os.makedirs(objdir, exist_ok=True)
+    headers = [p for p in _deps() if not p.endswith(".cu")]
+    newest_header = max(os.path.getmtime(p) for p in headers)
+
+    def compile_one(src: str):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        if (not force and not extra and os.path.exists(obj)
+                and os.path.getmtime(obj) > max(os.path.getmtime(src), newest_header)):
+            return obj, None
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", INCLUDE, "-I", CSRC, "-c", "-o", obj, src]
+        return obj, subprocess.run(cmd, cwd=HERE, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+        results = list(pool.map(compile_one, sources()))
+    failed = False
+    for _, res in results:
+        if res is not None and (verbose or res.returncode != 0):
+            sys.stderr.write(res.stdout + res.stderr)
+        failed = failed or (res is not None and res.returncode != 0)
+    if failed:
         raise RuntimeError("nvcc failed building libgtb_kpm.so")
+    tmp = LIB + ".tmp"
+    res = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp,
+                          *[obj for obj, _ in results]], cwd=HERE, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libgtb_kpm.so")
     os.replace(tmp, LIB)
     return LIB
 

@@ -39,11 +39,16 @@ struct StepPlan {
 };
 
 // dot = false: the DOS pass (dot products with phi_n itself); dot = true: with StepArgs::dot_with.
-int make_plan(const gtb_ell* H, int R, bool dot, StepPlan* p);
+// opt (may be NULL) pins a kernel; GTB_ERR_INVALID_ARG when the pinned kernel cannot take (H, R).
+int make_plan(const gtb_ell* H, int R, bool dot, const gtb_kpm_options* opt, StepPlan* p);
+int check_options(const gtb_kpm_options* opt);
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st);
 // K7b plan for an orbital-blocked matrix (B = 4: gtb_sk_hamiltonian's, B = 9: gtb_spd_hamiltonian's);
 // false when H or R does not fit
-bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, StepPlan* p);
+bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, bool direct, StepPlan* p);
+// s,p,d Hamiltonian held as 9x9 blocks (rep = 1: gtb_spd_blocks) or as bonds (rep = 2: gtb_spd_bonds);
+// H->n counts atoms, the vectors have 9 H->n rows.  false when R is not 2, 4 or 8.
+bool make_plan_rep9(const gtb_ell* H, int R, int rep, bool dot, StepPlan* p);
 
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);

@@ -61,11 +61,14 @@ __global__ void __launch_bounds__(kBlock) sk_block_kernel(const int32_t* __restr
       const double f = p.beta == 0.0 ? 1.0 : exp(-p.beta * (r / p.r0 - 1.0));
       const double* V = p.sk + ((size_t)si * p.n_species + sj) * 4;
       const double Vss = V[0] * f, Vsp = V[1] * f, Vpp_s = V[2] * f, Vpp_p = V[3] * f;
+      // E_{pa,s} = (-1)^{1+0} H_ji^{s,pa}: the s orbital sits on j, so the integral is the
+      // table entry of the pair (s_j, s_i) -- H stays symmetric for a species-asymmetric table
+      const double Vsp_ji = p.sk[((size_t)sj * p.n_species + si) * 4 + 1] * f;
       E[0][0] = Vss;
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         E[0][1 + a] = c[a] * Vsp;
-        E[1 + a][0] = -(c[a] * Vsp);
+        E[1 + a][0] = -(c[a] * Vsp_ji);
 #pragma unroll
         for (int b = 0; b < 3; ++b)
           E[1 + a][1 + b] = c[a] * c[b] * Vpp_s + ((a == b ? 1.0 : 0.0) - c[a] * c[b]) * Vpp_p;
@@ -202,9 +205,14 @@ __global__ void __launch_bounds__(128) spd_block_kernel(const int32_t* __restric
       c[8][m] = B22;
     }
     const double fr = p.beta == 0.0 ? 1.0 : exp(-p.beta * (r / p.r0 - 1.0));
-    double V[10];
+    // V: pair (s_i, s_j) for l_a <= l_b; Vt: pair (s_j, s_i) for l_a > l_b (that element is
+    // the transposed one of the (j, i) block, whose lower-l orbital sits on atom j)
+    double V[10], Vt[10];
 #pragma unroll
-    for (int q = 0; q < 10; ++q) V[q] = p.sk[((size_t)si * p.n_species + sj) * 10 + q] * fr;
+    for (int q = 0; q < 10; ++q) {
+      V[q] = p.sk[((size_t)si * p.n_species + sj) * 10 + q] * fr;
+      Vt[q] = p.sk[((size_t)sj * p.n_species + si) * 10 + q] * fr;
+    }
     for (int nu = 0; nu < 9; ++nu) {
       const int lb = nu == 0 ? 0 : (nu < 4 ? 1 : 2);
       for (int mu = 0; mu < 9; ++mu) {
@@ -212,7 +220,7 @@ __global__ void __launch_bounds__(128) spd_block_kernel(const int32_t* __restric
         const int lo = min(la, lb), hi = max(la, lb);
         double sum = 0.0;
 #pragma unroll
-        for (int m = 0; m < 5; ++m) sum += c[mu][m] * spd_integral(V, lo, hi, m) * c[nu][m];
+        for (int m = 0; m < 5; ++m) sum += c[mu][m] * spd_integral(la > lb ? Vt : V, lo, hi, m) * c[nu][m];
         const size_t at = (size_t)(9 * k + nu) * N + 9 * i + mu;
         cols[at] = (int32_t)(9 * j + nu);
         vals[at] = (la > lb && ((la + lb) & 1)) ? -sum : sum;

@@ -242,7 +242,7 @@ extern "C" int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const VacWs w = carve_vac(ws, H->n, 2, 1, R);
   StepPlan plan;
-  rc = make_plan(H, R, false, &plan);
+  rc = make_plan(H, R, false, nullptr, &plan);
   if (rc != GTB_OK) return rc;
   const std::vector<double2> c = bessel_coefficients(a, b, dt);
   if (terms) *terms = (int32_t)c.size();
@@ -260,21 +260,17 @@ extern "C" size_t gtb_vac_workspace_bytes(int64_t n, int32_t M, int32_t n_steps,
   return carve_vac(nullptr, n, M, n_steps, R_batch).bytes;
 }
 
-namespace {
-struct VacTimer {
-  cudaEvent_t beg = nullptr, end = nullptr;
-  int passes = 0;
-  bool armed = false;
-};
-thread_local VacTimer g_vac_timer;
-}  // namespace
-
 extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, double b, int32_t M,
                                int32_t n_steps, double dt, int32_t R_total, int32_t R_batch,
                                uint64_t seed, int32_t mode_flags, double* C, void* ws, size_t ws_bytes,
-                               void* stream) {
+                               void* stream, const gtb_kpm_options* opt) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
+  rc = check_options(opt);
+  if (rc != GTB_OK) return rc;
+  const int opt_flags = opt ? opt->flags : 0;
+  cudaEvent_t ev_beg = opt ? static_cast<cudaEvent_t>(opt->loop_begin) : nullptr;
+  cudaEvent_t ev_end = opt ? static_cast<cudaEvent_t>(opt->loop_end) : nullptr;
   if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9)) ||
       ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)))
     return GTB_ERR_INVALID_ARG;
@@ -293,19 +289,16 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2) * (size_t)n_steps * M, st));
   GTB_CUDA_TRY(cudaMemsetAsync(w.status, 0, sizeof(int32_t) * 64, st));
   const std::vector<double2> coef = bessel_coefficients(a, b, dt);
-  if (!g_vac_timer.beg) {
-    GTB_CUDA_TRY(cudaEventCreate(&g_vac_timer.beg));
-    GTB_CUDA_TRY(cudaEventCreate(&g_vac_timer.end));
-  }
-  g_vac_timer.armed = false;
   for (int64_t r0 = 0; r0 < n_vec; r0 += R_batch) {
     const int R = (int)std::min<int64_t>(R_batch, n_vec - r0);
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan, dplan;  // evolution passes (no bra) and moment passes (dot with psiL)
-    if (!(orb && make_plan_orb(H, R, orb, false, &plan) && make_plan_orb(H, R, orb, true, &dplan))) {
-      rc = make_plan(H, R, false, &plan);
+    const bool direct = (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0;
+    if (!(orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS) && make_plan_orb(H, R, orb, false, direct, &plan) &&
+          make_plan_orb(H, R, orb, true, direct, &dplan))) {
+      rc = make_plan(H, R, false, opt, &plan);
       if (rc != GTB_OK) return rc;
-      rc = make_plan(H, R, true, &dplan);
+      rc = make_plan(H, R, true, opt, &dplan);
       if (rc != GTB_OK) return rc;
     }
     double *psiL = w.buf[0], *psiR = w.buf[1], *sa_ = w.buf[2], *sb_ = w.buf[3];
@@ -329,7 +322,7 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
           reinterpret_cast<double2*>(cur), reinterpret_cast<const double2*>(psiL), w.partial);
       GTB_LAUNCHED();
       const bool timed = last_batch && j == n_steps - 1;
-      if (timed) GTB_CUDA_TRY(cudaEventRecord(g_vac_timer.beg, st));
+      if (timed && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
       StepArgs sa{H->cols, H->vals, H->diag, n, H->width, dplan.T, cur, io, 1.0 / a, b,
                   w.partial + kMaxGrid, psiL};
       for (int k = 1; k < M; ++k) {  // io <- chi_k, slot k = (Re<psiL|chi_{k-1}>, Re<psiL|chi_k>)
@@ -341,10 +334,9 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
         GTB_LAUNCHED();
         std::swap(cur, io);
       }
-      if (timed) {
-        GTB_CUDA_TRY(cudaEventRecord(g_vac_timer.end, st));
-        g_vac_timer.passes = M - 1;
-        g_vac_timer.armed = M > 1;
+      if (timed && ev_end) {
+        GTB_CUDA_TRY(cudaEventRecord(ev_end, st));
+        if (opt->loop_passes) *opt->loop_passes = M - 1;
       }
       launch_reduce_partials(w.partial, kMaxGrid, dplan.grid, w.sums + (size_t)j * M, M, st);
       GTB_LAUNCHED();
@@ -355,16 +347,6 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
   finish_vac_kernel<<<(int)((total + kBlock - 1) / kBlock), kBlock, 0, st>>>(w.sums, total, norm, C,
                                                                              w.status);
   GTB_LAUNCHED();
-  return GTB_OK;
-}
-
-extern "C" int gtb_vac_last_loop_ms(double* ms, int32_t* passes) {
-  if (!ms || !passes || !g_vac_timer.armed) return GTB_ERR_INVALID_ARG;
-  GTB_CUDA_TRY(cudaEventSynchronize(g_vac_timer.end));
-  float t = 0.f;
-  GTB_CUDA_TRY(cudaEventElapsedTime(&t, g_vac_timer.beg, g_vac_timer.end));
-  *ms = (double)t;
-  *passes = g_vac_timer.passes;
   return GTB_OK;
 }
 

@@ -71,18 +71,35 @@ def test_argument_validation_needs_no_gpu():
 
     ell = gtb._Ell(100, 3, 256, 256, None)
     mu = C.c_void_p(256)
-    def km(a=8.5, M=16, R=2, Rb=2, mode=0, ws_bytes=0):
+    def km(a=8.5, M=16, R=2, Rb=2, mode=0, ws_bytes=0, opt=None):
         return lib.gtb_kpm_moments(C.byref(ell), C.c_double(a), C.c_double(0.0), C.c_int32(M),
                                    C.c_int32(R), C.c_int32(Rb), C.c_uint64(1), C.c_int32(mode), mu,
-                                   fake, C.c_size_t(ws_bytes), None)
+                                   fake, C.c_size_t(ws_bytes), None, opt)
     assert km(a=0.0) == gtb.ERR_INVALID_ARG
     assert km(M=0) == gtb.ERR_INVALID_ARG
     assert km(R=0) == gtb.ERR_INVALID_ARG
     assert km(Rb=65) == gtb.ERR_INVALID_ARG
     assert km(mode=2) == gtb.ERR_INVALID_ARG
     assert km() == gtb.ERR_WORKSPACE
+    assert km(mode=gtb.MODE_ORB4 | gtb.MODE_ORB9) == gtb.ERR_INVALID_ARG
+    for bad in (gtb.options(kernel=9), gtb.options(tile_stages=9), gtb.options(flags=1 << 20)):
+        assert km(opt=C.byref(bad)) == gtb.ERR_INVALID_ARG
+    half = gtb.options()
+    half.loop_begin = 256                                       # an event pair must be complete
+    assert km(opt=C.byref(half)) == gtb.ERR_INVALID_ARG
+    assert km(opt=C.byref(gtb.options(kernel=gtb.KERNEL_ROW))) == gtb.ERR_WORKSPACE
     assert lib.gtb_dos(None, 4, C.c_double(1.0), C.c_double(0.0), 1, None, 4, C.c_double(1.0),
                        None, None) == gtb.ERR_INVALID_ARG
+
+
+def test_library_does_not_read_the_environment():
+    """Kernel selection goes through gtb_kpm_options (include/gtb.h), never through getenv (the
+    statically linked CUDA runtime imports getenv itself, so the sources are what is checked)."""
+    csrc = os.path.join(ROOT, "paper_2509_06525_b200", "csrc")
+    for f in os.listdir(csrc):
+        if f.endswith((".cu", ".cuh")):
+            text = open(os.path.join(csrc, f)).read()
+            assert "getenv" not in text and "environ" not in text, f
 
 
 def test_product_does_not_reach_the_oracle():

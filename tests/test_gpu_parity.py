@@ -208,14 +208,14 @@ def test_single_step_and_sums_match_oracle_rows():
 
 
 # K7 has two implementations: the register path and the TMA-staged tile path.
-# GTB_K7_TILE forces one or the other, GTB_K7_STAGES the depth of the shared-memory ring.
+# gtb_kpm_options.kernel pins one or the other, tile_stages the depth of the shared-memory ring.
 @pytest.mark.parametrize("key,nx,ny,kw,R", [("c2", 37, 23, {}, 8), ("c3", 33, 31, {}, 4),
                                              ("c2b", 41, 29, {}, 2), ("c4", 48, 21, {"stripe": 6}, 8),
                                              ("c5", 57, 43, {}, 2), ("c5", 57, 43, {}, 4)])
-@pytest.mark.parametrize("tile,stages", [(0, 0), (1, 1), (1, 2), (1, 3), (1, 5)])
-def test_both_k7_paths_match_oracle_rows(monkeypatch, key, nx, ny, kw, R, tile, stages):
-    monkeypatch.setenv("GTB_K7_TILE", str(tile))
-    monkeypatch.setenv("GTB_K7_STAGES", str(max(stages, 1)))
+@pytest.mark.parametrize("kernel,stages", [(gtb.KERNEL_AUTO, 0), (gtb.KERNEL_ROW, 0), (gtb.KERNEL_TILE, 1),
+                                           (gtb.KERNEL_TILE, 2), (gtb.KERNEL_TILE, 3), (gtb.KERNEL_TILE, 5)])
+def test_both_k7_paths_match_oracle_rows(key, nx, ny, kw, R, kernel, stages):
+    opt = gtb.options(kernel=kernel, tile_stages=stages)
     w, inp = _small(key, nx, ny, kw)
     Ho = _oracle_H(w, inp, with_diag=w.use_diag)
     Hg = _gpu_H(w, inp, with_diag=w.use_diag)
@@ -227,50 +227,37 @@ def test_both_k7_paths_match_oracle_rows(monkeypatch, key, nx, ny, kw, R, tile, 
     phi2 = oracle.kpm_step_rows(Ho, a, b, False, phi0, phi1, rows)
     g0 = _dev(phi0)
     g1 = torch.empty_like(g0)
-    s = gtb.kpm_step(Hg, a, b, True, g0, g1).cpu().numpy()
+    s = gtb.kpm_step(Hg, a, b, True, g0, g1, opt=opt).cpu().numpy()
     assert np.abs(g1.cpu().numpy() - phi1).max() <= 1e-14
     assert s[0] == pytest.approx(n * R, rel=1e-14)
-    s = gtb.kpm_step(Hg, a, b, False, g1, g0).cpu().numpy()
+    s = gtb.kpm_step(Hg, a, b, False, g1, g0, opt=opt).cpu().numpy()
     assert np.abs(g0.cpu().numpy() - phi2).max() <= 1e-14
     assert s[0] == pytest.approx((phi1 * phi1).sum(), rel=1e-13)
     assert s[1] == pytest.approx((phi2 * phi1).sum(), rel=1e-12, abs=1e-9)
     M = 65
     ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
-    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5, opt=opt).cpu().numpy()
     assert np.abs(got - ref).max() <= 1e-12
 
 
-# K7s: two steps per launch through L2 (temporal blocking).  Forced on here (by default it is
-# taken only when the working set exceeds L2); chunk size, slack and lattice shapes chosen so that
-# the halo spans one chunk, several chunks, and the whole ring (ny = 2: the y-neighbour is n/2 away).
-@pytest.mark.parametrize("key,nx,ny,kw,R", [("c5", 57, 43, {}, 2), ("c1", 24, 24, {}, 4),
-                                             ("c4", 48, 21, {"stripe": 6}, 8), ("c5", 300, 2, {}, 2),
-                                             ("c5", 256, 3, {}, 4)])
-@pytest.mark.parametrize("chunk,slack", [(64, 0), (128, 2368), (256, 7), (512, 592), (1024, 3)])
-@pytest.mark.parametrize("M", [64, 65])
-def test_two_step_sweep_matches_oracle(monkeypatch, key, nx, ny, kw, R, chunk, slack, M):
-    monkeypatch.setenv("GTB_K7_SWEEP", "1")
-    monkeypatch.setenv("GTB_K7_CHUNK", str(chunk))
-    monkeypatch.setenv("GTB_K7_SLACK", str(slack))
-    w, inp = _small(key, nx, ny, kw)
-    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
-    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
-    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
-    ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
-    ws = gtb.workspace(gtb.kpm_workspace_bytes(Ho.n, M, R))
-    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5, ws=ws, check=True).cpu().numpy()
-    assert np.abs(got - ref).max() <= 1e-12
-    monkeypatch.setenv("GTB_K7_SWEEP", "0")
-    one = gtb.kpm_moments(Hg, a, b, M, R, R, 5, ws=ws, check=True).cpu().numpy()
-    assert np.abs(got - one).max() <= 1e-13          # same vectors, another summation order
+def test_a_pinned_kernel_that_cannot_take_the_matrix_is_an_error():
+    """gtb_kpm_options: no silent detour (include/gtb.h)."""
+    w, inp = _small("c2", 37, 23, {})
+    Hg = _gpu_H(w, inp, with_diag=True)                       # K = 20
+    with pytest.raises(gtb.GtbError):
+        gtb.kpm_moments(Hg, 20.0, 0.0, 8, 2, 2, 5, opt=gtb.options(kernel=gtb.KERNEL_ROW_X2))
+    with pytest.raises(gtb.GtbError):
+        gtb.kpm_moments(Hg, 20.0, 0.0, 8, 3, 3, 5, opt=gtb.options(kernel=gtb.KERNEL_TILE))   # R = 3
+    with pytest.raises(gtb.GtbError):
+        gtb.kpm_moments(Hg, 20.0, 0.0, 8, 2, 2, 5, opt=gtb.options(kernel=7))
 
 
-# K7p: small systems run all passes in one cooperative launch (default); GTB_K7_SMALL=0 takes the
-# per-pass launches.  Both must agree with the oracle and with each other.
+# K7p: small systems run all passes in one cooperative launch (default); GTB_OPT_PER_PASS_LAUNCH takes
+# the per-pass launches.  Both must agree with the oracle and with each other.
 @pytest.mark.parametrize("key,nx,ny,kw,R", [("c1", 24, 24, {}, 4), ("c2", 37, 23, {}, 8), ("c3", 33, 31, {}, 2),
                                              ("c4", 48, 21, {"stripe": 6}, 8), ("c5", 57, 43, {}, 2)])
 @pytest.mark.parametrize("M", [2, 3, 64, 257])
-def test_single_launch_path_matches_oracle_and_per_pass_path(monkeypatch, key, nx, ny, kw, R, M):
+def test_single_launch_path_matches_oracle_and_per_pass_path(key, nx, ny, kw, R, M):
     w, inp = _small(key, nx, ny, kw)
     Ho = _oracle_H(w, inp, with_diag=w.use_diag)
     Hg = _gpu_H(w, inp, with_diag=w.use_diag)
@@ -280,58 +267,12 @@ def test_single_launch_path_matches_oracle_and_per_pass_path(monkeypatch, key, n
     got = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True).cpu().numpy()
     used = gtb.launch_count() - l0
     assert np.abs(got - ref).max() <= 1e-12
-    monkeypatch.setenv("GTB_K7_SMALL", "0")
     l0 = gtb.launch_count()
-    per_pass = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True).cpu().numpy()
+    per_pass = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True,
+                               opt=gtb.options(flags=gtb.OPT_PER_PASS_LAUNCH)).cpu().numpy()
     assert np.abs(got - per_pass).max() <= 1e-13
     if M >= 64:
         assert used < (gtb.launch_count() - l0) // 4      # the single-launch path really was taken
-
-
-# K7g: row groups (4 consecutive rows share their gathered neighbours).  The grouped arrays are checked
-# against the union built here from the oracle's ELL, the moments against the oracle's.
-@pytest.mark.parametrize("key,nx,ny,kw", SMALL)
-def test_row_groups_and_grouped_moments(key, nx, ny, kw):
-    w, inp = _small(key, nx, ny, kw)
-    Ho = _oracle_H(w, inp, with_diag=w.use_diag)
-    Hg = _gpu_H(w, inp, with_diag=w.use_diag)
-    G = gtb.group_rows(Hg)
-    n, ng = Ho.n, Ho.n // 4
-    gc, gv = G.cols.cpu().numpy(), G.vals.cpu().numpy()
-    assert gc.shape == (G.width, ng) and gv.shape == (G.width, ng, 4)
-    worst = 0
-    for g in range(0, ng, max(1, ng // 97)):                # sampled groups, incl. the first
-        rows = np.arange(4 * g, 4 * g + 4)
-        union = sorted({int(c) for r in rows for c in Ho.cols[:, r] if c != r})
-        worst = max(worst, len(union))
-        assert gc[:len(union), g].tolist() == union and (gc[len(union):, g] == 4 * g).all()
-        for mu, r in enumerate(rows):
-            want = {int(c): v for c, v in zip(Ho.cols[:, r], Ho.vals[:, r]) if c != r}
-            got = gv[:, g, mu]
-            assert (got[len(union):] == 0).all()
-            for u, c in enumerate(union):
-                ref = want.get(c, 0.0)
-                assert abs(got[u] - ref) <= ULP4 * max(abs(ref), 1e-300) or got[u] == ref
-    assert worst <= G.width
-    a, b = (w.a, w.b) if w.a is not None else _scale(Ho)
-    for R, M in ((2, 33), (4, 64), (8, 65)):
-        ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
-        got = gtb.kpm_moments(G, a, b, M, R, R, 5, mode=gtb.MODE_GROUP4, check=True).cpu().numpy()
-        assert np.abs(got - ref).max() <= 1e-12
-    exact = gtb.kpm_moments(G, a, b, 16, mode=1 | gtb.MODE_GROUP4, R_batch=8).cpu().numpy()
-    plain = gtb.kpm_moments(Hg, a, b, 16, mode=1, R_batch=8).cpu().numpy()
-    assert np.abs(exact - plain).max() <= 1e-13
-    with pytest.raises(gtb.GtbError):                      # the grouped layout has no scalar reading
-        gtb.kpm_moments(G, a, b, 8, 3, 3, 5, mode=gtb.MODE_GROUP4)
-
-
-def test_row_groups_need_a_multiple_of_four_rows():
-    w, inp = _small("c2b", 23, 17, {})
-    n = inp.pos.shape[0] - 1
-    args = (inp.box, (0, 0, 0), w.cutoff, w.onsite, w.t0, w.r0, w.beta)
-    Hg = gtb.build_hamiltonian(_dev(inp.pos[:n]), _dev(inp.species[:n]), *args, _dev(inp.onsite_shift[:n]))
-    with pytest.raises(gtb.GtbError):
-        gtb.group_rows(Hg)
 
 
 # K7x2 (narrow rows: two elements in flight per thread) against the oracle's rows and against K7, on sizes
@@ -339,9 +280,8 @@ def test_row_groups_need_a_multiple_of_four_rows():
 @pytest.mark.parametrize("key,nx,ny,kw,R,width", [("c5", 57, 43, {}, 2, None), ("c5", 57, 43, {}, 8, 4),
                                                    ("c4", 48, 21, {"stripe": 6}, 8, None),
                                                    ("c1", 24, 24, {}, 4, 4), ("c5", 301, 127, {}, 2, None)])
-def test_two_elements_in_flight_path(monkeypatch, key, nx, ny, kw, R, width):
-    monkeypatch.setenv("GTB_K7_SMALL", "0")
-    monkeypatch.setenv("GTB_K7_TILE", "0")
+def test_two_elements_in_flight_path(key, nx, ny, kw, R, width):
+    opts = {"1": gtb.options(kernel=gtb.KERNEL_ROW_X2), "0": gtb.options(kernel=gtb.KERNEL_ROW)}
     w, inp = _small(key, nx, ny, kw)
     Ho = _oracle_H(w, inp, width=width, with_diag=w.use_diag)
     Hg = _gpu_H(w, inp, width=width, with_diag=w.use_diag)
@@ -353,19 +293,16 @@ def test_two_elements_in_flight_path(monkeypatch, key, nx, ny, kw, R, width):
     phi2 = oracle.kpm_step_rows(Ho, a, b, False, phi0, phi1, rows)
     out = {}
     for x2 in ("1", "0"):
-        monkeypatch.setenv("GTB_K7_X2", x2)
         g1, g0 = _dev(phi1), _dev(phi0)
-        s = gtb.kpm_step(Hg, a, b, False, g1, g0).cpu().numpy()       # g0 <- phi_2
+        s = gtb.kpm_step(Hg, a, b, False, g1, g0, opt=opts[x2]).cpu().numpy()       # g0 <- phi_2
         out[x2] = g0.cpu().numpy()
         assert np.abs(out[x2][rows] - phi2).max() <= 1e-14
         assert s[0] == pytest.approx((phi1 * phi1).sum(), rel=1e-13)
     assert (out["1"] == out["0"]).all()                               # same arithmetic per element
     M = 33
     ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0) if n < 20000 else None
-    monkeypatch.setenv("GTB_K7_X2", "1")
-    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
-    monkeypatch.setenv("GTB_K7_X2", "0")
-    old = gtb.kpm_moments(Hg, a, b, M, R, R, 5).cpu().numpy()
+    got = gtb.kpm_moments(Hg, a, b, M, R, R, 5, opt=opts["1"]).cpu().numpy()
+    old = gtb.kpm_moments(Hg, a, b, M, R, R, 5, opt=opts["0"]).cpu().numpy()
     assert np.abs(got - old).max() <= 1e-13
     if ref is not None:
         assert np.abs(got - ref).max() <= 1e-12
