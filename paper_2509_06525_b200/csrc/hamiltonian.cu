@@ -7,6 +7,7 @@
 // raw differences of the unwrapped coordinates, minimum image by rint, r2 summed left
 // to right in fp64 WITHOUT fused multiply-add (the *_rn intrinsics below forbid contraction), and
 // a strict r2 < cutoff^2 test -- this is what makes the column indices bit-reproducible.
+#include <algorithm>
 #include <cmath>
 
 #include "common.cuh"
@@ -374,7 +375,9 @@ __global__ void gershgorin_final_kernel(const double* partial, int blocks, doubl
 }
 
 // ---- host side -------------------------------------------------------------------------
-int64_t cell_cap(int64_t n) { return 2 * n + 1024; }
+// cell indices are int32: the cap never exceeds INT32_MAX - 64 (beyond n ~ 1.07e9 atoms the grid is
+// simply coarser than two cells per atom)
+int64_t cell_cap(int64_t n) { return std::min<int64_t>(2 * n + 1024, (int64_t)INT32_MAX - 64); }
 
 struct BuildWs {
   int32_t* cell_of;

@@ -143,6 +143,18 @@ def make_inputs(w: Workload, seed: int = SEED_LATTICE) -> Inputs:
     return Inputs(pos, species, box, pbc, shift, w)
 
 
+def inputs_digest(inp: Inputs) -> str:
+    """SHA-256 of the generated arrays: stored in the full-size goldens (tests/golden/) so that a test
+    notices if the generators ever produce a different lattice."""
+    import hashlib
+    h = hashlib.sha256()
+    h.update(np.ascontiguousarray(inp.pos).tobytes())
+    h.update(np.ascontiguousarray(inp.species).tobytes())
+    if inp.onsite_shift is not None:
+        h.update(np.ascontiguousarray(inp.onsite_shift).tobytes())
+    return h.hexdigest()
+
+
 def energy_grid(w: Workload, a: float, b: float) -> np.ndarray:
     """E_j = E_min + j (E_max - E_min)/(G-1), endpoints included (C6)."""
     lo = w.e_min if w.e_min is not None else b - a

@@ -22,7 +22,6 @@ so that the test notices if the generators ever produce different lattices.
 """
 from __future__ import annotations
 
-import hashlib
 import os
 import sys
 import time
@@ -41,15 +40,6 @@ DOUBLING = {"c3", "c3b", "c5"}      # configs whose full-depth run uses the orac
 M_CHECK = 48
 
 
-def inputs_digest(inp) -> str:
-    h = hashlib.sha256()
-    h.update(np.ascontiguousarray(inp.pos).tobytes())
-    h.update(np.ascontiguousarray(inp.species).tobytes())
-    if inp.onsite_shift is not None:
-        h.update(np.ascontiguousarray(inp.onsite_shift).tobytes())
-    return h.hexdigest()
-
-
 def make(key: str) -> None:
     w = W.CONFIGS[key]
     t0 = time.time()
@@ -61,7 +51,7 @@ def make(key: str) -> None:
     else:                                   # reading A8
         lo, hi = oracle.spectral_bounds(H)
         a, b = 1.01 * (hi - lo) / 2.0, (hi + lo) / 2.0
-    digest = inputs_digest(inp)
+    digest = W.inputs_digest(inp)
     print(f"[{key}] N={H.n} K={H.width} a={a!r} b={b!r} built in {time.time() - t0:.0f} s", flush=True)
     algo = 1 if key in DOUBLING else 0
     check = ""
