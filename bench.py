@@ -35,6 +35,8 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
 KERNEL = "auto"                 # set by --kernel: pins the fused-pass kernel through gtb_kpm_options
+REP = "scalar"                  # set by --rep (spd only): scalar ELL expansion, stored 9x9 blocks, or bonds (matrix-free)
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x clocks.max.sm
 HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
 ORBITALS = "pz"                 # set by --orbitals: "pz" (one orbital per atom), "sp" (4) or "spd" (9)
 ORB_COUNT = {"pz": 1, "sp": 4, "spd": 9}
@@ -110,6 +112,8 @@ class ClockSampler:
 
 def _workload(args) -> W.Workload:
     w = W.CONFIGS[args.workload]
+    if args.cutoff:
+        w = W.replace(w, cutoff=args.cutoff, name=f"{w.name}-rc{args.cutoff:g}")
     if args.nx or args.ny:
         w = w.scaled(args.nx or w.nx, args.ny or w.ny)
     if args.moments:
@@ -283,11 +287,25 @@ def run_ours(args):
             H = gtb.sk_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns],
                                    W.SK_ONSITE_P[:ns], W.sk_table(ns), r0=1.42, beta=w.beta,
                                    onsite_shift=shift)
-        elif ORBITALS == "spd":
+        elif ORBITALS == "spd" and REP == "scalar":
             ns = len(w.onsite)
             H = gtb.spd_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
                                     W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42, beta=w.beta,
                                     onsite_shift=shift)
+        elif ORBITALS == "spd":      # bond form (matrix-free) or stored 9x9 blocks on the same neighbour lists
+            ns = len(w.onsite)
+            Hm = gtb.spd_bonds(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
+                               W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42, beta=w.beta, onsite_shift=shift)
+            H = Hm if REP == "bonds" else gtb.spd_blocks(Hm)
+            rmode = gtb.MODE_BOND9 if REP == "bonds" else gtb.MODE_BLOCK9
+            lo, hi = gtb.spd_bounds(H, rmode).tolist()
+            a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+            gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode=rmode, ws=ws_kpm, mu=mu, opt=opt)
+            if "E" not in state:
+                state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
+            rho = gtb.dos(mu, a, b, state["E"])
+            state["H"], state["a"], state["b"], state["rho"] = H, a, b, rho
+            return rho
         if w.a is None or ORBITALS != "pz" or HOPPING == "mlp":
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
@@ -350,10 +368,18 @@ def run_ours(args):
     e2e = replicas.whole_job_value(units, ms_e2e)
     # roofline of the dominant kernel (the fused pass K7): algorithmic bytes per launch
     # = N * (12 K + 8 [diag] + 48 R), over its mean launch duration
-    orb4 = ORBITALS != "pz" and w.R in (2, 4, 8)
+    orb4 = ORBITALS != "pz" and w.R in (2, 4, 8) and not (ORBITALS == "spd" and REP != "scalar")
     B = ORB_COUNT[ORBITALS]
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
-    if orb4:   # per orbital row: K blocks of (4 B column + 8 B^2 B values) shared by B rows, + diag + vectors
+    flops_per_launch = None
+    rep9 = ORBITALS == "spd" and REP != "scalar"
+    if rep9 and REP == "blocks":   # per ATOM: K x (column + 81 values) + 9 onsite + 9 orbital rows of vectors; / 9 per row
+        per_atom = (H.width * (4 + 648) + 72 + 9 * 48 * w.R) / 9.0
+    elif rep9:                     # per ATOM: K columns + own record + shift + vectors (each neighbour record once: in the 32)
+        per_atom = (4 * H.width + 32 + 8 + 9 * 48 * w.R) / 9.0
+        # closed-form action: 64 FMA per real component and pair + ~50 FMA-equivalents of geometry, + the epilogue
+        flops_per_launch = float(n) * (H.width * (2 * 64 * 2 * w.R + 100) + 9 * 2 * w.R * 8)
+    elif orb4:   # per orbital row: K blocks of (4 B column + 8 B^2 B values) shared by B rows, + diag + vectors
         per_atom = (H.width // B) * (4 + 8 * B * B) // B + (8 if H.diag is not None else 0) + 48 * w.R
     bytes_per_launch = float(n_orb) * per_atom
     k7_ms = loop_ms / max(loop_passes, 1)
@@ -363,7 +389,12 @@ def run_ours(args):
     vec = w.R in (2, 4, 8)
     tile = KERNEL == "tile" or (KERNEL == "auto" and H.width > 4 and n % 4 == 0 and vec)
     x2 = KERNEL == "row_x2" or (KERNEL == "auto" and H.width <= 4 and vec)
-    k7_name = ("cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
+    if rep9:
+        small = False
+    k7_name = ("cheb_bond9_kernel (K7m: fused Chebyshev pass, 9x9 pair action rebuilt from the bond vector)"
+               if rep9 and REP == "bonds" else
+               "cheb_block9_kernel (K7bb: fused Chebyshev pass on stored 9x9 blocks [K][81][n])" if rep9 else
+               "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
                ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)" if tile else
                "cheb_step_x2_kernel (K7x2: fused Chebyshev pass, two elements in flight per thread)" if x2 else
@@ -371,20 +402,34 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": k7_name,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                "traffic": _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS, w.name)
+                "traffic": _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS +
+                                        ("" if REP == "scalar" else "-" + REP), w.name)
                 if KERNEL == "auto" else None,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "bytes_per_atom_pass": per_atom,
                 "ms_per_launch": k7_ms, "launches_timed": loop_passes,
                 "share_of_step": loop_ms / ms}
+    if flops_per_launch is not None:   # the matrix-free pass has two roofs: report against the lower one
+        t_hbm = bytes_per_launch / (peak * 1e9)
+        t_alu = flops_per_launch / (FP64_PEAK_TFLOPS * 1e12)
+        tf = flops_per_launch / (k7_ms * 1e-3) / 1e12
+        roofline["hbm_frac"] = achieved / peak
+        roofline["alu"] = {"achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+                           "algorithmic_flops_per_launch": flops_per_launch,
+                           "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz"}
+        if t_alu > t_hbm:
+            roofline.update(bound="alu", achieved=tf, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
+                            frac=tf / FP64_PEAK_TFLOPS, peak_source=roofline["alu"]["peak_source"])
+            roofline.pop("frac_of_8TBs_nominal", None)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128 vectors)",
             "data": "synthetic",
             "config": {"workload": w.name, "atoms": n, "orbitals_per_atom": n_orb // n,
-                       "ell_width": H.width, "moments": w.M,
+                       "ell_width": H.width, "representation": REP if ORBITALS == "spd" else "ell",
+                       "cutoff_A": w.cutoff, "moments": w.M,
                        "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (
-                           (2 * n_orb * w.R * 16 + H.nbytes()) / 1e9),
+                           (2 * n_orb * w.R * 16 + (H.nbytes() if not rep9 else H.cols.numel() * 4 + H.vals.numel() * 8)) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "seconds_per_full_dos": ms / args.steps * 1e-3,
             "recursion_updates_per_s": float(n_orb) * w.M * w.R / ((loop_ms / args.steps + k7_ms) * 1e-3),
@@ -556,11 +601,16 @@ def main():
                    help="analytic: t(r) of the configs; mlp: descriptor + MLPs of Eq. 2 with synthetic weights (NEXT-3)")
     p.add_argument("--kernel", default="auto", choices=["auto", "row", "row_x2", "tile"],
                    help="pin the fused-pass kernel (gtb_kpm_options.kernel); auto: picked from the matrix shape")
+    p.add_argument("--rep", default="bonds", choices=["scalar", "blocks", "bonds"],
+                   help="--orbitals spd: scalar ELL expansion (K7b9), stored 9x9 blocks (K7bb) or bonds = matrix-free (K7m)")
+    p.add_argument("--cutoff", type=float, default=0.0, help="override the neighbour cutoff in Angstrom "
+                   "(3.0 on the pristine lattice = third-nearest neighbours, K = 12: Fig. 4a)")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS, HOPPING, KERNEL
+    global ORBITALS, HOPPING, KERNEL, REP
     KERNEL = args.kernel
+    REP = args.rep
     ORBITALS = args.orbitals
     HOPPING = args.hopping
     if args.hopping == "mlp" and (args.orbitals != "pz" or args.quantity == "vac"):

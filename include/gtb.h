@@ -98,6 +98,8 @@ enum {
 #define GTB_OPT_PER_PASS_LAUNCH 1 /* never fold a small system's passes into one cooperative launch (K7p) */
 #define GTB_OPT_SCALAR_BLOCKS 2   /* ignore GTB_MODE_ORB4 / ORB9: run the scalar kernels on the expanded H */
 #define GTB_OPT_BLOCK_DIRECT 4    /* K7b9: strided block loads instead of the shared-memory hand-off      */
+#define GTB_OPT_SEPARATE_AXPY 8   /* gtb_vac_moments: one accumulation launch per Chebyshev-Bessel term
+                                     instead of the accumulation fused into the propagation pass (same bits) */
 typedef struct gtb_kpm_options {
   int32_t kernel;       /* GTB_KERNEL_*; a kernel that cannot take (H, R_batch) -> GTB_ERR_INVALID_ARG  */
   int32_t tile_stages;  /* K7t ring depth, 1..8; 0 = default (2)                                       */
@@ -161,6 +163,8 @@ int gtb_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n, doubl
  *         R_batch at a time (each pass of H serves R_batch vectors).
  * mode 1: exact trace over all n basis vectors e_i (R_total and seed ignored),
  *         R_batch of them per pass.
+ * mode | GTB_MODE_BLOCK9 / GTB_MODE_BOND9: H is the block / bond form of an s,p,d Hamiltonian (see
+ *         gtb_spd_bonds below); H->n counts atoms, the vectors have 9 H->n rows.
  * mode | GTB_MODE_ORB4 (or GTB_MODE_ORB9): the caller promises that H is the orbital-blocked matrix
  *         written by gtb_sk_hamiltonian (4 orbitals per atom; gtb_spd_hamiltonian: 9); the fused pass
  *         then works on whole 4x4 (9x9) blocks (one gather of the neighbour's orbitals per block).  Same results; ignored
@@ -181,10 +185,12 @@ int gtb_kpm_status(const void* ws, void* stream);
  *   first == 0:  out = (H phi_cur - b phi_cur)*(2/a) - phi_io      (phi_io read, then overwritten)
  * sums (DEVICE [2]) = { sum_{i,r} |phi_cur|^2 ,  sum_{i,r} Re(conj(out) phi_cur) }.
  * phi_cur, phi_io: DEVICE [n][R][2], 32-byte aligned, must not overlap.
+ * mode: 0, or one of GTB_MODE_ORB4 / ORB9 / BLOCK9 / BOND9 with the meaning they have in gtb_kpm_moments
+ * (BLOCK9 / BOND9: n = 9 H->n vector rows).
  * Workspace: gtb_kpm_workspace_bytes(n, 2, R). */
 int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
-                 const double* phi_cur, double* phi_io, double* sums, void* ws, size_t ws_bytes,
-                 void* stream, const gtb_kpm_options* opt);
+                 const double* phi_cur, double* phi_io, double* sums, int32_t mode, void* ws,
+                 size_t ws_bytes, void* stream, const gtb_kpm_options* opt);
 
 /* ---- density of states (Eq. 4; north_star (4); reading C6) ---- */
 /* ASYNC.  rho(E_j) = scale*[g_0 mu_0 + 2 sum_{n=1}^{M-1} g_n mu_n T_n(x_j)] / (pi a sqrt(1-x_j^2)),
@@ -321,6 +327,42 @@ size_t gtb_spd_workspace_bytes(void);
 int gtb_spd_hamiltonian(const gtb_ell* nbr, const double* pos, const int32_t* species,
                         const double box[3], const int32_t pbc[3], const gtb_spd_model* model,
                         gtb_ell* H, int32_t* status, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- s,p,d at the paper's scale: block and bond representations (Fig. 4a :192) ----
+ * The scalar ELL of gtb_spd_hamiltonian costs 972 K bytes per atom (81 K column copies + 81 K values) and
+ * stops near 10^7 atoms.  Two other representations of the SAME operator, each with its own fused pass:
+ *
+ * bonds (GTB_MODE_BOND9, matrix-free): the pass rebuilds every pair's 9x9 action from the bond vector and
+ *   the species pair's ten integrals in registers (closed form of reading S4 summed over the bond frame:
+ *   csrc/spd9.cu).  H costs 4 K + 40 bytes per atom: 10^8 atoms x 9 orbitals with a
+ *   third-neighbour cutoff fit one 180 GB B200.
+ *     Hm->n = atoms, Hm->width = K and Hm->cols = the neighbour lists of `nbr` (shared, not copied),
+ *     Hm->vals = a caller-allocated DEVICE block of gtb_spd_bonds_bytes(n) bytes (256-byte aligned) that
+ *     receives the parameter tables and one record (x, y, z, species) + onsite shift per atom;
+ *     Hm->diag is ignored (the onsite energies of the model are always applied).
+ *   The model's same-l integrals (ss, pp, dd) must be symmetric in the species pair (GTB_ERR_INVALID_ARG
+ *   otherwise: no symmetric H exists); the mixed-l ones (sp, sd, pd) may differ between (A, B) and (B, A).
+ *   SYNC on the parameter upload, then ASYNC.  *status (DEVICE int32) non-zero: species out of range.
+ *
+ * blocks (GTB_MODE_BLOCK9): the pairs' blocks stored once, every load coalesced:
+ *     Hb->n = atoms, Hb->width = K, Hb->cols = Hm->cols (shared), Hb->vals = double [K][81][n]
+ *     (entry 9 nu + mu of block k of atom i at ((k*81 + 9 nu + mu) * n + i); padding slots: zeros),
+ *     Hb->diag = double [9][n] (onsite energy of orbital mu of atom i at mu*n + i) or NULL.
+ *   gtb_spd_blocks fills them from the bond form.  ASYNC.  652 K + 72 bytes per atom.
+ *
+ * Both go to gtb_kpm_moments(H, ..., mode | GTB_MODE_BLOCK9 / GTB_MODE_BOND9, ...) with R_batch in
+ * {2, 4, 8}; the vectors have 9 n rows (orbital 9 i + mu, as in the scalar form), so the workspace is
+ * gtb_kpm_workspace_bytes(9 n, M, R_batch) and the moments are normalised by 9 n R.  Same moments as the
+ * scalar form up to rounding (another summation order inside a block).
+ * gtb_spd_bounds: ASYNC, the Gershgorin interval of the orbital matrix from either form (lo_hi DEVICE [2];
+ * mode = GTB_MODE_BLOCK9 or GTB_MODE_BOND9; workspace gtb_spd_bounds_workspace_bytes()). */
+size_t gtb_spd_bonds_bytes(int64_t n_atoms);
+int gtb_spd_bonds(const gtb_ell* nbr, const double* pos, const int32_t* species, const double box[3],
+                  const int32_t pbc[3], const gtb_spd_model* model, gtb_ell* Hm, int32_t* status,
+                  void* stream);
+int gtb_spd_blocks(const gtb_ell* Hm, gtb_ell* Hb, void* stream);
+size_t gtb_spd_bounds_workspace_bytes(void);
+int gtb_spd_bounds(const gtb_ell* H, int32_t mode, double* lo_hi, void* ws, size_t ws_bytes, void* stream);
 
 /* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
  *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):

@@ -151,6 +151,17 @@ def random_phase_fill(seed: int, r0: int, R: int, n: int) -> np.ndarray:
     return phi
 
 
+def random_phase_rows(seed: int, r0: int, R: int, rows) -> np.ndarray:
+    """Rows `rows` of random_phase_fill(seed, r0, R, n): [len(rows)][R][2]."""
+    rows = np.ascontiguousarray(rows, dtype=np.int64).reshape(-1)
+    phi = np.zeros((rows.shape[0], R, 2))
+    st = lib().gtbo_random_phase_rows(C.c_uint64(seed & (2**64 - 1)), C.c_int32(r0), C.c_int32(R),
+                                      C.c_void_p(rows.ctypes.data), C.c_int64(rows.shape[0]),
+                                      C.c_void_p(phi.ctypes.data))
+    _check(st, "random_phase_rows")
+    return phi
+
+
 def kpm_moments(H: Ell, a: float, b: float, M: int, R: int = 1, seed: int = 0, mode: int = 0,
                 algo: int = 0, return_im: bool = False):
     mu = np.zeros(M)
@@ -341,6 +352,34 @@ def spd_hamiltonian(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, onsite
     _check(lib().gtbo_spd_hamiltonian(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
                                       C.byref(model), C.byref(hc)), "spd_hamiltonian")
     return H
+
+
+def spd_step_atoms(nbr: Ell, pos, species, box, pbc, onsite_s, onsite_p, onsite_d, sk, a: float, b: float,
+                   first: bool, atoms, x_own, x_nbr, prev=None, r0: float = 1.0, beta: float = 0.0,
+                   onsite_shift=None) -> np.ndarray:
+    """One Chebyshev step of the s,p,d orbital matrix on the listed atoms without materialising H:
+    x_own [q][9][R][2], x_nbr [q][K][9][R][2], prev like x_own -> out [q][9][R][2]."""
+    pos, species, box, pbc = _f64(pos), _i32(species), _f64(box), _i32(pbc)
+    es, ep, ed = (_f64(x).reshape(-1) for x in (onsite_s, onsite_p, onsite_d))
+    sk = _f64(sk).reshape(-1)
+    ns = es.shape[0]
+    assert sk.shape[0] == ns * ns * 10
+    shift = _f64(onsite_shift) if onsite_shift is not None else None
+    atoms = np.ascontiguousarray(atoms, dtype=np.int64).reshape(-1)
+    x_own, x_nbr = _f64(x_own), _f64(x_nbr)
+    q, R = atoms.shape[0], x_own.shape[2]
+    assert x_own.shape == (q, 9, R, 2) and x_nbr.shape == (q, nbr.width, 9, R, 2)
+    prev = _f64(prev) if prev is not None else None
+    out = np.zeros((q, 9, R, 2))
+    model = _SpdModel(ns, es.ctypes.data, ep.ctypes.data, ed.ctypes.data, sk.ctypes.data, r0, beta,
+                      shift.ctypes.data if shift is not None else None)
+    nc = nbr._c()
+    _check(lib().gtbo_spd_step_atoms(C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc), C.byref(model),
+                                     C.c_double(a), C.c_double(b), C.c_int32(int(first)), C.c_int32(R),
+                                     _p(atoms), C.c_int64(q), _p(x_own), _p(x_nbr),
+                                     C.c_void_p(prev.ctypes.data if prev is not None else None), _p(out)),
+           "spd_step_atoms")
+    return out
 
 
 def mlp_sk_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, weights,

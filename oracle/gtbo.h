@@ -88,6 +88,9 @@ uint64_t gtbo_mix64(uint64_t z);                         /* splitmix64 output */
 uint64_t gtbo_hash(uint64_t seed, uint32_t r, uint64_t i); /* h(seed, r, i)   */
 double gtbo_uniform(uint64_t seed, uint32_t r, uint64_t i); /* (h>>11)*2^-53  */
 /* phi[i][k] = exp(i*theta), theta = fl(2*pi*u(seed, r0+k, i)), k = 0..R-1    */
+/* rows[q] of the vectors gtbo_random_phase_fill would write: phi [n_rows][R][2]. */
+int gtbo_random_phase_rows(uint64_t seed, int32_t r0, int32_t R, const int64_t* rows, int64_t n_rows,
+                           double* phi);
 int gtbo_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int64_t n,
                            double* phi);
 
@@ -184,6 +187,13 @@ typedef struct gtbo_spd_model {
   const double* onsite_shift; /* [n] or NULL */
 } gtbo_spd_model;
 /* H: caller-allocated scalar ELL over 9n orbitals, width 9*nbr->width, diag [9n] or NULL. */
+/* One Chebyshev step of the s,p,d orbital matrix on sampled atoms without materialising H (for sizes
+ * whose scalar ELL does not fit the host); vectors given sparsely, see gtbo_spd.cpp. */
+int gtbo_spd_step_atoms(const gtbo_ell* nbr, const double* pos, const int32_t* species,
+                        const double box[3], const int32_t pbc[3], const gtbo_spd_model* model,
+                        double a, double b, int32_t first, int32_t R, const int64_t* atoms,
+                        int64_t n_rows, const double* x_own, const double* x_nbr, const double* prev,
+                        double* out);
 int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* species,
                          const double box[3], const int32_t pbc[3],
                          const gtbo_spd_model* model, gtbo_ell* H);

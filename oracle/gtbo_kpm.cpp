@@ -162,6 +162,22 @@ extern "C" int gtbo_random_phase_fill(uint64_t seed, int32_t r0, int32_t R, int6
   return GTBO_OK;
 }
 
+// the rows `rows[q]` of the vectors gtbo_random_phase_fill would write (for sampled checks at sizes whose
+// full vectors do not fit the host): phi[q][k] = exp(i theta(seed, r0 + k, rows[q]))
+extern "C" int gtbo_random_phase_rows(uint64_t seed, int32_t r0, int32_t R, const int64_t* rows,
+                                      int64_t n_rows, double* phi) {
+  if (!phi || !rows || R <= 0 || n_rows < 0 || r0 < 0) return GTBO_ERR_INVALID_ARG;
+  for (int64_t q = 0; q < n_rows; ++q)
+    for (int32_t k = 0; k < R; ++k) {
+      if (rows[q] < 0) return GTBO_ERR_INVALID_ARG;
+      const double u = gtbo_uniform(seed, (uint32_t)(r0 + k), (uint64_t)rows[q]);
+      const double theta = 6.283185307179586 * u;
+      phi[((size_t)q * R + k) * 2 + 0] = std::cos(theta);
+      phi[((size_t)q * R + k) * 2 + 1] = std::sin(theta);
+    }
+  return GTBO_OK;
+}
+
 extern "C" int gtbo_kpm_moments(const gtbo_ell* H, double a, double b, int32_t M,
                                 int32_t R, uint64_t seed, int32_t mode, int32_t algo,
                                 double* mu, double* im_max) {

@@ -80,6 +80,38 @@ double integral(const double* V, int l, int lp, int m) {
   return am == 0 ? V[7] : (am == 1 ? V[8] : V[9]);   // d-d
 }
 
+// the 9x9 hopping block E[a][b] of the pair (i, j), j != i: the construction of the file header
+void pair_block(const double* pos, const double box[3], const int32_t pbc[3], const gtbo_spd_model* model,
+                int64_t i, int64_t j, int si, int sj, double E[kOrb][kOrb]) {
+  const int ns = model->n_species;
+  double d[3];
+  for (int a = 0; a < 3; ++a) {
+    d[a] = pos[3 * j + a] - pos[3 * i + a];
+    if (pbc[a]) d[a] = d[a] - box[a] * std::rint(d[a] / box[a]);
+  }
+  const double r = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
+  const double u[3] = {d[0] / r, d[1] / r, d[2] / r};
+  const double f = model->beta == 0.0 ? 1.0 : std::exp(-model->beta * (r / model->r0 - 1.0));
+  // V: integrals of the pair (s_i, s_j), used for l_a <= l_b; Vt: those of (s_j, s_i), used for
+  // l_a > l_b -- PAPER.md:88, H_ij^{l l'} = (-1)^{l+l'} H_ji^{l' l}: the (l_a > l_b) element of the
+  // (i, j) block is the (l_b, l_a) element of the (j, i) block, whose lower-l orbital sits on j.
+  double V[10], Vt[10];
+  for (int q = 0; q < 10; ++q) {
+    V[q] = model->sk[((size_t)si * ns + sj) * 10 + q] * f;
+    Vt[q] = model->sk[((size_t)sj * ns + si) * 10 + q] * f;
+  }
+  double c[kOrb][5];
+  frame_coefficients(u, c);
+  for (int a = 0; a < kOrb; ++a)
+    for (int b = 0; b < kOrb; ++b) {
+      const int la = kL[a], lb = kL[b];
+      const int lo = la < lb ? la : lb, hi = la < lb ? lb : la;
+      double s = 0.0;
+      for (int m = 0; m < 5; ++m) s += c[a][m] * integral(la > lb ? Vt : V, lo, hi, m) * c[b][m];
+      E[a][b] = (la > lb && ((la + lb) & 1)) ? -s : s;
+    }
+}
+
 }  // namespace
 
 extern "C" int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* species,
@@ -99,32 +131,7 @@ extern "C" int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, cons
       if (j != i) {
         const int sj = species[j];
         if (sj < 0 || sj >= ns) return GTBO_ERR_INVALID_ARG;
-        double d[3];
-        for (int a = 0; a < 3; ++a) {
-          d[a] = pos[3 * j + a] - pos[3 * i + a];
-          if (pbc[a]) d[a] = d[a] - box[a] * std::rint(d[a] / box[a]);
-        }
-        const double r = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
-        const double u[3] = {d[0] / r, d[1] / r, d[2] / r};
-        const double f = model->beta == 0.0 ? 1.0 : std::exp(-model->beta * (r / model->r0 - 1.0));
-        // V: integrals of the pair (s_i, s_j), used for l_a <= l_b; Vt: those of (s_j, s_i), used for
-        // l_a > l_b -- PAPER.md:88, H_ij^{l l'} = (-1)^{l+l'} H_ji^{l' l}: the (l_a > l_b) element of the
-        // (i, j) block is the (l_b, l_a) element of the (j, i) block, whose lower-l orbital sits on j.
-        double V[10], Vt[10];
-        for (int q = 0; q < 10; ++q) {
-          V[q] = model->sk[((size_t)si * ns + sj) * 10 + q] * f;
-          Vt[q] = model->sk[((size_t)sj * ns + si) * 10 + q] * f;
-        }
-        double c[kOrb][5];
-        frame_coefficients(u, c);
-        for (int a = 0; a < kOrb; ++a)
-          for (int b = 0; b < kOrb; ++b) {
-            const int la = kL[a], lb = kL[b];
-            const int lo = la < lb ? la : lb, hi = la < lb ? lb : la;
-            double s = 0.0;
-            for (int m = 0; m < 5; ++m) s += c[a][m] * integral(la > lb ? Vt : V, lo, hi, m) * c[b][m];
-            E[a][b] = (la > lb && ((la + lb) & 1)) ? -s : s;
-          }
+        pair_block(pos, box, pbc, model, i, j, si, sj, E);
       }
       for (int mu = 0; mu < kOrb; ++mu)
         for (int nu = 0; nu < kOrb; ++nu) {
@@ -139,6 +146,56 @@ extern "C" int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, cons
         H->diag[kOrb * i + a] = (kL[a] == 0 ? model->onsite_s[si] : kL[a] == 1 ? model->onsite_p[si]
                                                                                : model->onsite_d[si]) + shift;
     }
+  }
+  return GTBO_OK;
+}
+
+// One Chebyshev step of the orbital matrix on SAMPLED atoms, without materialising H (at 10^8 atoms the
+// scalar ELL of gtbo_spd_hamiltonian would need 10^12 bytes): for every listed atom i the blocks of its
+// pairs are built exactly as above and applied to the neighbours' orbital rows,
+//   out[q][mu] = ((H x)_{9 i + mu} - b x_{9 i + mu}) * (first ? 1/a : 2/a)  [- prev_{9 i + mu} unless first],
+// row sum in slot order 9 k + nu, then the onsite term: the order of gtbo_kpm_step_rows on the scalar ELL.
+// The vectors are given SPARSELY: x_own [n_rows][9][R][2] (rows of the listed atoms), x_nbr
+// [n_rows][K][9][R][2] (rows of their neighbours, slot by slot; padding slots ignored), prev like x_own.
+extern "C" int gtbo_spd_step_atoms(const gtbo_ell* nbr, const double* pos, const int32_t* species,
+                                   const double box[3], const int32_t pbc[3], const gtbo_spd_model* model,
+                                   double a, double b, int32_t first, int32_t R, const int64_t* atoms,
+                                   int64_t n_rows, const double* x_own, const double* x_nbr,
+                                   const double* prev, double* out) {
+  if (!nbr || !pos || !species || !box || !pbc || !model || !atoms || !x_own || !x_nbr || !out ||
+      (!first && !prev) || R <= 0 || model->n_species <= 0)
+    return GTBO_ERR_INVALID_ARG;
+  const int64_t n = nbr->n;
+  const int32_t K = nbr->width;
+  const int ns = model->n_species;
+  for (int64_t q = 0; q < n_rows; ++q) {
+    const int64_t i = atoms[q];
+    if (i < 0 || i >= n) return GTBO_ERR_INVALID_ARG;
+    const int si = species[i];
+    if (si < 0 || si >= ns) return GTBO_ERR_INVALID_ARG;
+    const double shift = model->onsite_shift ? model->onsite_shift[i] : 0.0;
+    for (int mu = 0; mu < kOrb; ++mu)
+      for (int32_t r = 0; r < R; ++r)
+        for (int c = 0; c < 2; ++c) {
+          double acc = 0.0;
+          for (int32_t k = 0; k < K; ++k) {
+            const int64_t j = nbr->cols[(size_t)k * n + i];
+            if (j == i) continue;
+            const int sj = species[j];
+            if (sj < 0 || sj >= ns) return GTBO_ERR_INVALID_ARG;
+            double E[kOrb][kOrb];
+            pair_block(pos, box, pbc, model, i, j, si, sj, E);
+            for (int nu = 0; nu < kOrb; ++nu)
+              acc = acc + E[mu][nu] * x_nbr[((((size_t)q * K + k) * kOrb + nu) * R + r) * 2 + c];
+          }
+          const double own = x_own[(((size_t)q * kOrb + mu) * R + r) * 2 + c];
+          const double eps = (kL[mu] == 0 ? model->onsite_s[si] : kL[mu] == 1 ? model->onsite_p[si]
+                                                                              : model->onsite_d[si]) + shift;
+          acc = acc + eps * own;
+          double v = (acc - b * own) * ((first ? 1.0 : 2.0) / a);
+          if (!first) v = v - prev[(((size_t)q * kOrb + mu) * R + r) * 2 + c];
+          out[(((size_t)q * kOrb + mu) * R + r) * 2 + c] = v;
+        }
   }
   return GTBO_OK;
 }

@@ -33,13 +33,16 @@ EXPORTS = (
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_conductivity",
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
-    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian",
+    "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_spd_bonds_bytes", "gtb_spd_bonds",
+    "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
 KERNEL_AUTO, KERNEL_ROW, KERNEL_ROW_X2, KERNEL_TILE = 0, 1, 2, 3      # gtb_kpm_options.kernel
-OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT = 1, 2, 4     # gtb_kpm_options.flags
+OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT, OPT_SEPARATE_AXPY = 1, 2, 4, 8   # gtb_kpm_options.flags
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
+MODE_BLOCK9 = 64            # ... the block form written by spd_blocks (H.n = atoms)
+MODE_BOND9 = 128            # ... the bond form written by spd_bonds (matrix-free)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
 
@@ -299,7 +302,8 @@ def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
     if mu is None:
         mu = torch.empty(M, dtype=torch.float64, device=dev)
     if ws is None:
-        ws = workspace(kpm_workspace_bytes(H.n, M, R_batch), dev)
+        rows = 9 * H.n if mode & (MODE_BLOCK9 | MODE_BOND9) else H.n
+        ws = workspace(kpm_workspace_bytes(rows, M, R_batch), dev)
     hc = H._c()
     st = lib().gtb_kpm_moments(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(M),
                                C.c_int32(R_total), C.c_int32(R_batch),
@@ -316,18 +320,19 @@ def kpm_status(ws: torch.Tensor) -> None:
 
 
 def kpm_step(H: Ell, a: float, b: float, first: bool, phi_cur: torch.Tensor, phi_io: torch.Tensor,
-             ws: Optional[torch.Tensor] = None, opt: Optional[_Options] = None) -> torch.Tensor:
+             ws: Optional[torch.Tensor] = None, opt: Optional[_Options] = None,
+             mode: int = 0) -> torch.Tensor:
     """One fused pass; phi_io is overwritten with phi_{n+1}.  Returns the two sums (device [2])."""
     phi_cur = _dev(phi_cur, torch.float64, "phi_cur")
     phi_io = _dev(phi_io, torch.float64, "phi_io")
     R = phi_cur.shape[1]
     sums = torch.empty(2, dtype=torch.float64, device=phi_cur.device)
     if ws is None:
-        ws = workspace(kpm_workspace_bytes(H.n, 2, R), phi_cur.device)
+        ws = workspace(kpm_workspace_bytes(phi_cur.shape[0], 2, R), phi_cur.device)
     hc = H._c()
     st = lib().gtb_kpm_step(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(int(first)),
-                            C.c_int32(R), _ptr(phi_cur), _ptr(phi_io), _ptr(sums), _ptr(ws),
-                            C.c_size_t(ws.numel()), _stream(), _opt(opt))
+                            C.c_int32(R), _ptr(phi_cur), _ptr(phi_io), _ptr(sums), C.c_int32(mode),
+                            _ptr(ws), C.c_size_t(ws.numel()), _stream(), _opt(opt))
     _check(st, "kpm_step")
     return sums
 
@@ -576,6 +581,57 @@ def mlp_sk_hamiltonian(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, 
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "mlp_sk_hamiltonian", "species index out of range")
     return H
+
+
+def spd_bonds(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, onsite_s, onsite_p, onsite_d, sk,
+              r0: float = 1.0, beta: float = 0.0, onsite_shift: Optional[torch.Tensor] = None) -> Ell:
+    """The bond (matrix-free) form of the s,p,d Hamiltonian for kpm_moments(..., mode=MODE_BOND9): the
+    neighbour lists of `nbr` (shared) and a device block of parameter tables + atom records in `vals`."""
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    es, ep, ed = (np.ascontiguousarray(x, dtype=np.float64).reshape(-1) for x in (onsite_s, onsite_p, onsite_d))
+    ns = es.shape[0]
+    sk_h = _host_f64(sk, ns * ns * 10)
+    if onsite_shift is not None:
+        onsite_shift = _dev(onsite_shift, torch.float64, "onsite_shift")
+    dev = pos.device
+    lib().gtb_spd_bonds_bytes.restype = C.c_size_t
+    nbytes = int(lib().gtb_spd_bonds_bytes(C.c_int64(nbr.n)))
+    blob = torch.empty(nbytes // 8, dtype=torch.float64, device=dev)
+    Hm = Ell(nbr.n, nbr.width, nbr.cols, blob, None)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    model = _SpdModel(ns, es.ctypes.data, ep.ctypes.data, ed.ctypes.data, sk_h.ctypes.data, r0, beta,
+                      onsite_shift.data_ptr() if onsite_shift is not None else None)
+    nc, hc = nbr._c(), Hm._c()
+    st = lib().gtb_spd_bonds(C.byref(nc), _ptr(pos), _ptr(species), C.c_void_p(box_h.ctypes.data),
+                             C.c_void_p(pbc_h.ctypes.data), C.byref(model), C.byref(hc), _ptr(status), _stream())
+    _check(st, "spd_bonds")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "spd_bonds", "species index out of range")
+    return Hm
+
+
+def spd_blocks(Hm: Ell, with_diag: bool = True) -> Ell:
+    """The block form (cols [K][n] shared, blocks [K][81][n], onsite [9][n]) for mode=MODE_BLOCK9."""
+    dev = Hm.vals.device
+    Hb = Ell(Hm.n, Hm.width, Hm.cols, torch.empty((max(Hm.width, 1), 81, Hm.n), dtype=torch.float64, device=dev),
+             torch.empty((9, Hm.n), dtype=torch.float64, device=dev) if with_diag else None)
+    mc, bc = Hm._c(), Hb._c()
+    _check(lib().gtb_spd_blocks(C.byref(mc), C.byref(bc), _stream()), "spd_blocks")
+    return Hb
+
+
+def spd_bounds(H: Ell, mode: int) -> torch.Tensor:
+    """Gershgorin interval (device [2]) of the orbital matrix held in block or bond form."""
+    out = torch.empty(2, dtype=torch.float64, device=H.vals.device)
+    lib().gtb_spd_bounds_workspace_bytes.restype = C.c_size_t
+    ws = workspace(int(lib().gtb_spd_bounds_workspace_bytes()), out.device)
+    hc = H._c()
+    _check(lib().gtb_spd_bounds(C.byref(hc), C.c_int32(mode), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()),
+                                _stream()), "spd_bounds")
+    return out
 
 
 # ---------------------------------------------------------------- Fig. 4b post-processing

@@ -23,6 +23,8 @@ struct StepArgs {
   double b;
   double2* partial;       // [gridDim.x]: (sum |phi_n|^2, sum Re conj(phi_{n+1}) phi_n), or with
   const double* dot_with; // dot_with = L:  (sum Re conj(L) phi_n, sum Re conj(L) phi_{n+1})
+  double* axpy_acc;       // propagation passes (plan mode 2): axpy_acc += (axpy_cr + i axpy_ci) * phi_{n+1},
+  double axpy_cr, axpy_ci;  // fused into the pass; no dot products are taken
 };
 
 using StepFn = void (*)(const StepArgs);
@@ -38,9 +40,10 @@ struct StepPlan {
   int block = 0;   // threads per CTA of the staged kernel (0: the default of K7t)
 };
 
-// dot = false: the DOS pass (dot products with phi_n itself); dot = true: with StepArgs::dot_with.
+// dot = 0: the DOS pass (dot products with phi_n itself); 1: with StepArgs::dot_with; 2: no dot products,
+// the Chebyshev-Bessel accumulation StepArgs::axpy_acc += c * phi_{n+1} fused into the pass instead.
 // opt (may be NULL) pins a kernel; GTB_ERR_INVALID_ARG when the pinned kernel cannot take (H, R).
-int make_plan(const gtb_ell* H, int R, bool dot, const gtb_kpm_options* opt, StepPlan* p);
+int make_plan(const gtb_ell* H, int R, int dot, const gtb_kpm_options* opt, StepPlan* p);
 int check_options(const gtb_kpm_options* opt);
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st);
 // K7b plan for an orbital-blocked matrix (B = 4: gtb_sk_hamiltonian's, B = 9: gtb_spd_hamiltonian's);

@@ -67,8 +67,9 @@ __global__ void __launch_bounds__(kBlock) basis_fill_kernel(int64_t r0, int32_t 
 // K6 / K7.  Thread e handles element e of phi viewed as an array of Vec<VW>: row = e / T, vector
 // group t = e % T, so a warp touches one contiguous 32*VW*8-byte span of phi_{n-1}/phi_{n+1}, and
 // every gather of a row's neighbour is T consecutive threads reading R*16 contiguous bytes.
-template <int VW, int LOG2T, bool kFirst, bool kDiag, int CH, bool kDotL>
+template <int VW, int LOG2T, bool kFirst, bool kDiag, int CH, int kMode>
 __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
+  constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   const int64_t n = a.n;
   const int T = LOG2T >= 0 ? (1 << LOG2T) : a.T;
   const int64_t total = n * T;
@@ -90,6 +91,7 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
     const Vec<VW> own = load_gather<VW>(a.phi_cur + e * VW);
     Vec<VW> with;
     if (kDotL) with = load_stream<VW>(a.dot_with + e * VW);
+    if (kAxpy) with = load_stream<VW>(a.axpy_acc + e * VW);
     if (CH == 0) {
 #pragma unroll 4
       for (int k = 0; k < width; ++k) {
@@ -131,10 +133,16 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
     for (int q = 0; q < VW; ++q) {
       y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
       if (!kFirst) y.v[q] -= prev.v[q];
-      s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
-      s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+      if (!kAxpy) {
+        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+      }
     }
     store_stream<VW>(a.phi_io + e * VW, y);
+    if (kAxpy) {
+      axpy_into<VW>(with, y, a.axpy_cr, a.axpy_ci);
+      store_stream<VW>(a.axpy_acc + e * VW, with);
+    }
   }
   __shared__ double red[kBlock / 32][2];
   s1 = warp_sum(s1);
@@ -164,8 +172,9 @@ __global__ void __launch_bounds__(kBlock) cheb_step_kernel(const StepArgs a) {
 // and the two stores.  W (3 or 4) is a compile-time bound on the row width, so everything is unrolled and
 // lives in registers (64 registers: still 4 blocks per SM).  Same arithmetic order per element as K7.
 // Config 5: 2.20 -> 1.99 ms per pass.
-template <int LOG2T, bool kDiag, int W, bool kDotL>
+template <int LOG2T, bool kDiag, int W, int kMode>
 __global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) {
+  constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
   constexpr int NE = 2;
@@ -194,6 +203,7 @@ __global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) 
       prev[r] = load_stream<VW>(a.phi_io + e[r] * VW);
       own[r] = load_gather<VW>(a.phi_cur + e[r] * VW);
       if (kDotL) with[r] = load_stream<VW>(a.dot_with + e[r] * VW);
+      if (kAxpy) with[r] = load_stream<VW>(a.axpy_acc + e[r] * VW);
 #pragma unroll
       for (int k = 0; k < W; ++k) {
         const bool ok = k < width;
@@ -227,10 +237,16 @@ __global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) 
 #pragma unroll
         for (int q = 0; q < VW; ++q) {
           y.v[q] = (acc[r].v[q] - b * own[r].v[q]) * scale - prev[r].v[q];
-          s1 = fma(own[r].v[q], kDotL ? with[r].v[q] : own[r].v[q], s1);
-          s2 = fma(y.v[q], kDotL ? with[r].v[q] : own[r].v[q], s2);
+          if (!kAxpy) {
+            s1 = fma(own[r].v[q], kDotL ? with[r].v[q] : own[r].v[q], s1);
+            s2 = fma(y.v[q], kDotL ? with[r].v[q] : own[r].v[q], s2);
+          }
         }
         store_stream<VW>(a.phi_io + e[r] * VW, y);
+        if (kAxpy) {
+          axpy_into<VW>(with[r], y, a.axpy_cr, a.axpy_ci);
+          store_stream<VW>(a.axpy_acc + e[r] * VW, with[r]);
+        }
       }
     }
   }
@@ -253,14 +269,14 @@ __global__ void __launch_bounds__(kBlock) cheb_step_x2_kernel(const StepArgs a) 
   }
 }
 
-template <int LOG2T, int W, bool DOT>
+template <int LOG2T, int W, int DOT>
 StepFn pick_x2(bool diag) {
   return diag ? cheb_step_x2_kernel<LOG2T, true, W, DOT> : cheb_step_x2_kernel<LOG2T, false, W, DOT>;
 }
 template <int LOG2T>
-StepFn pick_x2(bool diag, int width, bool dot) {
-  if (width <= 3) return dot ? pick_x2<LOG2T, 3, true>(diag) : pick_x2<LOG2T, 3, false>(diag);
-  return dot ? pick_x2<LOG2T, 4, true>(diag) : pick_x2<LOG2T, 4, false>(diag);
+StepFn pick_x2(bool diag, int width, int mode) {
+  if (width <= 3) return mode == 2 ? pick_x2<LOG2T, 3, 2>(diag) : mode == 1 ? pick_x2<LOG2T, 3, 1>(diag) : pick_x2<LOG2T, 3, 0>(diag);
+  return mode == 2 ? pick_x2<LOG2T, 4, 2>(diag) : mode == 1 ? pick_x2<LOG2T, 4, 1>(diag) : pick_x2<LOG2T, 4, 0>(diag);
 }
 
 // ---- K7t: the same pass with the Hamiltonian stream staged by TMA ------------------------------
@@ -312,8 +328,9 @@ __host__ __device__ inline uint32_t tile_stage_bytes(int width, int TR, bool dia
 #endif
 constexpr int kTileBlock = GTB_TILE_BLOCK;  // threads per CTA of K7t
 
-template <int LOG2T, bool kFirst, bool kDiag, int CH, bool kDotL>
+template <int LOG2T, bool kFirst, bool kDiag, int CH, int kMode>
 __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
+  constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
   constexpr int TR = kTileBlock / T;  // rows per tile: one thread per 256-bit element
@@ -345,7 +362,7 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
     const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
     if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
     __syncwarp();
-    for (int j = lane; j < 2 * width + (kDotL ? 4 : 3); j += 32) {
+    for (int j = lane; j < 2 * width + (kDotL || kAxpy ? 4 : 3); j += 32) {
       if (j < width) {
         bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
       } else if (j < 2 * width) {
@@ -359,6 +376,7 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
         if (!kFirst) bulk_prefetch_l2(a.phi_io + row0 * (T * VW), rows * (T * VW * 8));
       } else {
         if (kDotL) bulk_prefetch_l2(a.dot_with + row0 * (T * VW), rows * (T * VW * 8));
+        if (kAxpy) bulk_prefetch_l2(a.axpy_acc + row0 * (T * VW), rows * (T * VW * 8));
       }
     }
   };
@@ -413,15 +431,22 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
     if (wid == 0 && i + nstages < my_tiles) issue(i + nstages);
     if (live) {
       if (kDotL) with = load_stream<VW>(a.dot_with + e * VW);  // prefetched into L2 by the producer
+      if (kAxpy) with = load_stream<VW>(a.axpy_acc + e * VW);
       Vec<VW> y;
 #pragma unroll
       for (int q = 0; q < VW; ++q) {
         y.v[q] = (acc.v[q] - b * own.v[q]) * scale;
         if (!kFirst) y.v[q] -= prev.v[q];
-        s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
-        s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+        if (!kAxpy) {
+          s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+          s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+        }
       }
       store_stream<VW>(a.phi_io + e * VW, y);
+      if (kAxpy) {
+        axpy_into<VW>(with, y, a.axpy_cr, a.axpy_ci);
+        store_stream<VW>(a.axpy_acc + e * VW, with);
+      }
     }
   }
   __shared__ double red[kTileBlock / 32][2];
@@ -584,25 +609,25 @@ __global__ void copy_sums_kernel(const double2* sums, double* out2) {
 }
 
 // ---- host side ---------------------------------------------------------------------------
-template <int VW, int LOG2T, int CH, bool DOT>
+template <int VW, int LOG2T, int CH, int DOT>
 void pick_ch(bool diag, StepPlan* p) {
   p->first = diag ? cheb_step_kernel<VW, LOG2T, true, true, CH, DOT> : cheb_step_kernel<VW, LOG2T, true, false, CH, DOT>;
   p->next = diag ? cheb_step_kernel<VW, LOG2T, false, true, CH, DOT> : cheb_step_kernel<VW, LOG2T, false, false, CH, DOT>;
 }
 
 template <int VW, int LOG2T>
-void pick(bool diag, int ch, bool dot, StepPlan* p) {
-  if (ch == 0) { if (dot) pick_ch<VW, LOG2T, 0, true>(diag, p); else pick_ch<VW, LOG2T, 0, false>(diag, p); }
-  else { if (dot) pick_ch<VW, LOG2T, 8, true>(diag, p); else pick_ch<VW, LOG2T, 8, false>(diag, p); }
+void pick(bool diag, int ch, int mode, StepPlan* p) {
+  if (ch == 0) { if (mode == 2) pick_ch<VW, LOG2T, 0, 2>(diag, p); else if (mode == 1) pick_ch<VW, LOG2T, 0, 1>(diag, p); else pick_ch<VW, LOG2T, 0, 0>(diag, p); }
+  else { if (mode == 2) pick_ch<VW, LOG2T, 8, 2>(diag, p); else if (mode == 1) pick_ch<VW, LOG2T, 8, 1>(diag, p); else pick_ch<VW, LOG2T, 8, 0>(diag, p); }
 }
 
-template <int LOG2T, int CH, bool DOT>
+template <int LOG2T, int CH, int DOT>
 void pick_tile_ch(bool diag, StepPlan* p) {
   p->tfirst = diag ? cheb_tile_kernel<LOG2T, true, true, CH, DOT> : cheb_tile_kernel<LOG2T, true, false, CH, DOT>;
   p->tnext = diag ? cheb_tile_kernel<LOG2T, false, true, CH, DOT> : cheb_tile_kernel<LOG2T, false, false, CH, DOT>;
 }
 
-template <int LOG2T, bool DOT>
+template <int LOG2T, int DOT>
 void pick_tile_dot(bool diag, int ch, StepPlan* p) {
   switch (ch) {
     case 3: pick_tile_ch<LOG2T, 3, DOT>(diag, p); break;
@@ -614,9 +639,10 @@ void pick_tile_dot(bool diag, int ch, StepPlan* p) {
 }
 
 template <int LOG2T>
-void pick_tile(bool diag, int ch, bool dot, StepPlan* p) {
-  if (dot) pick_tile_dot<LOG2T, true>(diag, ch, p);
-  else pick_tile_dot<LOG2T, false>(diag, ch, p);
+void pick_tile(bool diag, int ch, int mode, StepPlan* p) {
+  if (mode == 2) pick_tile_dot<LOG2T, 2>(diag, ch, p);
+  else if (mode == 1) pick_tile_dot<LOG2T, 1>(diag, ch, p);
+  else pick_tile_dot<LOG2T, 0>(diag, ch, p);
 }
 
 // gathers kept in flight per thread: the chunk that pads `width` least (ties: the larger)
@@ -636,7 +662,8 @@ int tile_chunk(int width) {
 
 // Picks the kernels and the launch shape of the fused pass for (H, R).  opt (may be NULL) pins a
 // kernel; a pinned kernel that cannot take this matrix is GTB_ERR_INVALID_ARG, never a silent detour.
-int make_plan(const gtb_ell* H, int R, bool dot, const gtb_kpm_options* opt, StepPlan* p) {
+int make_plan(const gtb_ell* H, int R, int dot, const gtb_kpm_options* opt, StepPlan* p) {
+  if (dot < 0 || dot > 2) return GTB_ERR_INVALID_ARG;
   const int64_t n = H->n;
   const int width = H->width;
   const bool diag = H->diag != nullptr;
@@ -706,7 +733,7 @@ void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t
   if (p.stages > 0)
     (first ? p.tfirst : p.tnext)<<<p.grid, p.block ? p.block : kTileBlock, p.smem, st>>>(sa, p.stages);
   else
-    (first ? p.first : p.next)<<<p.grid, kBlock, 0, st>>>(sa);
+    (first ? p.first : p.next)<<<p.grid, p.block ? p.block : kBlock, p.smem, st>>>(sa);
 }
 
 void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st) {
@@ -738,7 +765,8 @@ int check_options(const gtb_kpm_options* opt) {
   if (!opt) return GTB_OK;
   if (opt->kernel < GTB_KERNEL_AUTO || opt->kernel > GTB_KERNEL_TILE || opt->tile_stages < 0 ||
       opt->tile_stages > 8 ||
-      (opt->flags & ~(GTB_OPT_PER_PASS_LAUNCH | GTB_OPT_SCALAR_BLOCKS | GTB_OPT_BLOCK_DIRECT)) ||
+      (opt->flags & ~(GTB_OPT_PER_PASS_LAUNCH | GTB_OPT_SCALAR_BLOCKS | GTB_OPT_BLOCK_DIRECT |
+                      GTB_OPT_SEPARATE_AXPY)) ||
       ((opt->loop_begin == nullptr) != (opt->loop_end == nullptr)))
     return GTB_ERR_INVALID_ARG;
   return GTB_OK;
@@ -912,24 +940,42 @@ extern "C" int gtb_kpm_status(const void* ws, void* stream) {
 }
 
 extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
-                            const double* phi_cur, double* phi_io, double* sums, void* ws,
-                            size_t ws_bytes, void* stream, const gtb_kpm_options* opt) {
+                            const double* phi_cur, double* phi_io, double* sums, int32_t mode_flags,
+                            void* ws, size_t ws_bytes, void* stream, const gtb_kpm_options* opt) {
   int rc = check_ell(H);
   if (rc != GTB_OK) return rc;
   rc = check_options(opt);
   if (rc != GTB_OK) return rc;
+  const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
+  const int rep = (mode_flags & GTB_MODE_BLOCK9) ? 1 : (mode_flags & GTB_MODE_BOND9) ? 2 : 0;
+  if ((mode_flags & ~(GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9)) ||
+      (orb != 0) + (rep != 0) > 1 || ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)) ||
+      ((mode_flags & GTB_MODE_BLOCK9) && (mode_flags & GTB_MODE_BOND9)))
+    return GTB_ERR_INVALID_ARG;
   if (!phi_cur || !phi_io || !sums || !(a > 0.0) || R <= 0 || R > 64 ||
       (reinterpret_cast<uintptr_t>(phi_cur) & 31u) || (reinterpret_cast<uintptr_t>(phi_io) & 31u))
     return GTB_ERR_INVALID_ARG;
-  rc = check_ws(ws, ws_bytes, gtb_kpm_workspace_bytes(H->n, 2, R));
+  const int64_t n = rep ? 9 * H->n : H->n;   // vector rows
+  if (n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
+  rc = check_ws(ws, ws_bytes, gtb_kpm_workspace_bytes(n, 2, R));
   if (rc != GTB_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const KpmWs w = carve_kpm(ws, H->n, 2, R);
+  const KpmWs w = carve_kpm(ws, n, 2, R);
   StepPlan plan;
-  rc = make_plan(H, R, false, opt, &plan);
-  if (rc != GTB_OK) return rc;
+  const int opt_flags = opt ? opt->flags : 0;
+  bool blocked = false;
+  if (rep) {
+    if (!make_plan_rep9(H, R, rep, false, &plan)) return GTB_ERR_INVALID_ARG;
+    blocked = true;
+  } else if (orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS)) {
+    blocked = make_plan_orb(H, R, orb, false, (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0, &plan);
+  }
+  if (!blocked) {
+    rc = make_plan(H, R, false, opt, &plan);
+    if (rc != GTB_OK) return rc;
+  }
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
-  StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width, plan.T, phi_cur, phi_io,
+  StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, phi_cur, phi_io,
               (first ? 1.0 : 2.0) / a, b, w.partial};
   launch_step(plan, first != 0, sa, st);
   GTB_LAUNCHED();

@@ -262,6 +262,3 @@ bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, bool direct, StepPl
 
 }  // namespace gtb
 
-namespace gtb {
-bool make_plan_rep9(const gtb_ell*, int, int, bool, StepPlan*) { return false; }
-}  // namespace gtb

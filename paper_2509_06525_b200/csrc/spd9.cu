@@ -1,0 +1,659 @@
+// s,p,d Slater-Koster Hamiltonians at the paper's scale (PAPER.md:96 "s, p, d orbital basis", :106 "over
+// 100 million atoms (approximately 1 billion orbitals)", Fig. 4a :192): two representations of the same
+// operator that gtb_spd_hamiltonian writes as a scalar ELL matrix, and the fused Chebyshev pass on each.
+//
+//   blocks (GTB_MODE_BLOCK9, K7bb):  cols int32 [K][n], blocks double [K][81][n] (entry 9 nu + mu, atom
+//       fastest: a warp's loads of one entry are one contiguous run), onsite double [9][n].  652 K bytes
+//       per atom instead of the scalar form's 972 K, no dead column copies, every load coalesced.
+//   bonds  (GTB_MODE_BOND9, K7m):    cols int32 [K][n] and one record (x, y, z, species) per atom; the pass
+//       rebuilds each pair's action from the bond vector and the species pair's integrals in registers:
+//       H costs 4 K + 40 bytes per atom, so 10^8 atoms x 9 orbitals fit one 180 GB B200.
+//
+// The two-centre integrals are diagonal in the bond frame (reading S4).  Summing the
+// frame out in closed form gives, with u = (l, m, n) the bond direction, D_a = u^T A_a u and G_a = A_a u
+// for the five d orbitals (A_a the quadratic forms of reading S4):
+//   E_ss = V_ss;   E_{s,pb} = V_sp u_b;   E_{s,db} = V_sd D_b;
+//   E_{pa,s} = -V'_sp u_a;   E_{pa,pb} = V_ppp d_ab + (V_pps - V_ppp) u_a u_b;
+//   E_{pa,db} = (V_pds - k V_pdp) u_a D_b + k V_pdp G_{b,a},   k = 2/sqrt3;
+//   E_{da,s} = V'_sd D_a;   E_{da,pb} = -(V'_pds - k V'_pdp) D_a u_b - k V'_pdp G_{a,b};
+//   E_{da,db} = V_ddd d_ab + (V_dds - 4/3 V_ddp + 1/3 V_ddd) D_a D_b + 4/3 (V_ddp - V_ddd) G_a . G_b,
+// V of the pair (s_i, s_j), V' of (s_j, s_i) (the l_a > l_b elements belong to the (j, i)
+// block).  Applied to a vector these are 64 FMAs per real component instead of 81 for a stored block.
+#include <algorithm>
+#include <cmath>
+
+#include "vecload.cuh"
+
+namespace gtb {
+namespace {
+
+constexpr int kNc = 14;             // coefficient combinations per ordered species pair
+constexpr size_t kBondHeaderBytes = 8192;
+constexpr double kS3 = 1.7320508075688772;   // sqrt(3)
+constexpr double kK = 1.1547005383792517;    // 2 / sqrt(3)
+
+struct BondHeader {
+  double box[3];
+  double r0, beta;
+  int32_t pbc[3];
+  int32_t n_species;
+  int64_t n;
+  double onsite[3][GTB_MAX_SPECIES];                        // s, p, d
+  double coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES][kNc];      // see pair_coefficients
+};
+static_assert(sizeof(BondHeader) <= kBondHeaderBytes, "bond header");
+
+// the 14 combinations of the closed form above, from V = sk[si][sj], Vt = sk[sj][si]
+// (ss_s, sp_s, pp_s, pp_p, sd_s, pd_s, pd_p, dd_s, dd_p, dd_d)
+void pair_coefficients(const double* V, const double* Vt, double* c) {
+  c[0] = V[0];                                        // ss
+  c[1] = V[1];                                        // s <- p
+  c[2] = V[4];                                        // s <- d
+  c[3] = -Vt[1];                                      // p <- s
+  c[4] = V[3];                                        // p <- p: delta
+  c[5] = V[2] - V[3];                                 //          u u^T
+  c[6] = V[5] - kK * V[6];                            // p <- d: u D^T
+  c[7] = kK * V[6];                                   //          G^T
+  c[8] = Vt[4];                                       // d <- s
+  c[9] = -(Vt[5] - kK * Vt[6]);                       // d <- p: D u^T
+  c[10] = -kK * Vt[6];                                //          G
+  c[11] = V[9];                                       // d <- d: delta
+  c[12] = V[7] - 4.0 / 3.0 * V[8] + 1.0 / 3.0 * V[9]; //          D D^T
+  c[13] = 4.0 / 3.0 * (V[8] - V[9]);                  //          G G^T
+}
+
+struct Geometry {
+  double l, m, n;   // bond direction
+  double f;         // exp(-beta (r/r0 - 1))
+};
+
+// bond i -> j with the minimum image; the same evaluation order as the assembly kernels
+__device__ __forceinline__ Geometry bond_geometry(const double pi[3], const double pj[3],
+                                                  const double* box, const int32_t* pbc, double r0,
+                                                  double beta) {
+  double d[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    d[a] = __dsub_rn(pj[a], pi[a]);
+    if (pbc[a]) d[a] = __dsub_rn(d[a], __dmul_rn(box[a], rint(__ddiv_rn(d[a], box[a]))));
+  }
+  const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+  const double r = sqrt(r2);
+  const double inv = 1.0 / r;
+  Geometry g;
+  g.l = d[0] * inv;
+  g.m = d[1] * inv;
+  g.n = d[2] * inv;
+  g.f = beta == 0.0 ? 1.0 : exp(-beta * (r / r0 - 1.0));
+  return g;
+}
+
+// D_a = u^T A_a u, order xy, yz, zx, x2-y2, z2
+__device__ __forceinline__ void angular_d(const Geometry& g, double D[5]) {
+  D[0] = kS3 * g.l * g.m;
+  D[1] = kS3 * g.m * g.n;
+  D[2] = kS3 * g.n * g.l;
+  D[3] = 0.5 * kS3 * (g.l * g.l - g.m * g.m);
+  D[4] = g.n * g.n - 0.5 * (g.l * g.l + g.m * g.m);
+}
+
+// G_a = A_a u
+__device__ __forceinline__ void angular_g(const Geometry& g, double G[5][3]) {
+  const double h = 0.5 * kS3;
+  G[0][0] = h * g.m; G[0][1] = h * g.l; G[0][2] = 0.0;
+  G[1][0] = 0.0; G[1][1] = h * g.n; G[1][2] = h * g.m;
+  G[2][0] = h * g.n; G[2][1] = 0.0; G[2][2] = h * g.l;
+  G[3][0] = h * g.l; G[3][1] = -h * g.m; G[3][2] = 0.0;
+  G[4][0] = -0.5 * g.l; G[4][1] = -0.5 * g.m; G[4][2] = g.n;
+}
+
+// the explicit 9x9 block E[mu][nu] of the pair (closed form in the file header); c already holds f
+__device__ void pair_block(const Geometry& g, const double* c, double E[9][9]) {
+  const double u[3] = {g.l, g.m, g.n};
+  double D[5], G[5][3];
+  angular_d(g, D);
+  angular_g(g, G);
+  E[0][0] = c[0];
+  for (int b = 0; b < 3; ++b) {
+    E[0][1 + b] = c[1] * u[b];
+    E[1 + b][0] = c[3] * u[b];
+    for (int a = 0; a < 3; ++a) E[1 + a][1 + b] = (a == b ? c[4] : 0.0) + c[5] * u[a] * u[b];
+  }
+  for (int b = 0; b < 5; ++b) {
+    E[0][4 + b] = c[2] * D[b];
+    E[4 + b][0] = c[8] * D[b];
+    for (int a = 0; a < 3; ++a) {
+      E[1 + a][4 + b] = c[6] * u[a] * D[b] + c[7] * G[b][a];
+      E[4 + b][1 + a] = c[9] * D[b] * u[a] + c[10] * G[b][a];
+    }
+    for (int a = 0; a < 5; ++a)
+      E[4 + a][4 + b] = (a == b ? c[11] : 0.0) + c[12] * D[a] * D[b] +
+                        c[13] * (G[a][0] * G[b][0] + G[a][1] * G[b][1] + G[a][2] * G[b][2]);
+  }
+}
+
+__device__ __forceinline__ uint32_t smem_u32_of(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+__device__ __forceinline__ Vec<4> ld_rec(const double* p) {   // 32-byte atom record, read-only path
+  return load_gather<4>(p);
+}
+
+// ---- assembly ---------------------------------------------------------------------------------------
+// bond records: posw[i] = (x, y, z, species), shift[i]
+__global__ void __launch_bounds__(kBlock) bond_record_kernel(int64_t n, const double* __restrict__ pos,
+                                                             const int32_t* __restrict__ species,
+                                                             const double* __restrict__ shift_in,
+                                                             int32_t n_species, double* __restrict__ posw,
+                                                             double* __restrict__ shift,
+                                                             int32_t* __restrict__ status) {
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kBlock) {
+    const int s = species[i];
+    if (s < 0 || s >= n_species) atomicOr(status, 1);
+    posw[4 * i + 0] = pos[3 * i + 0];
+    posw[4 * i + 1] = pos[3 * i + 1];
+    posw[4 * i + 2] = pos[3 * i + 2];
+    posw[4 * i + 3] = (double)min(max(s, 0), n_species - 1);
+    shift[i] = shift_in ? shift_in[i] : 0.0;
+  }
+}
+
+// one thread per (atom, neighbour slot): the block of the pair into blocks[k][9 nu + mu][i]
+__global__ void __launch_bounds__(128) block9_assemble_kernel(const int32_t* __restrict__ cols, int64_t n,
+                                                              int32_t K, const double* __restrict__ bond,
+                                                              double* __restrict__ blocks) {
+  const BondHeader& h = *reinterpret_cast<const BondHeader*>(bond);
+  const double* posw = bond + kBondHeaderBytes / 8;
+  const int64_t total = n * K;
+  for (int64_t e = (int64_t)blockIdx.x * 128 + threadIdx.x; e < total; e += (int64_t)gridDim.x * 128) {
+    const int64_t k = e / n;
+    const int64_t i = e - k * n;
+    const int64_t j = cols[e];
+    double E[9][9];
+    if (j == i) {   // padding slot
+      for (int mu = 0; mu < 9; ++mu)
+        for (int nu = 0; nu < 9; ++nu) E[mu][nu] = 0.0;
+    } else {
+      const Vec<4> pi = ld_rec(posw + 4 * i), pj = ld_rec(posw + 4 * j);
+      const Geometry g = bond_geometry(pi.v, pj.v, h.box, h.pbc, h.r0, h.beta);
+      const double* c0 = h.coef[(int)pi.v[3] * h.n_species + (int)pj.v[3]];
+      double c[kNc];
+      for (int q = 0; q < kNc; ++q) c[q] = c0[q] * g.f;
+      pair_block(g, c, E);
+    }
+    double* out = blocks + (size_t)k * 81 * n + i;
+    for (int nu = 0; nu < 9; ++nu)
+      for (int mu = 0; mu < 9; ++mu) out[(size_t)(9 * nu + mu) * n] = E[mu][nu];
+  }
+}
+
+// onsite[mu][i] = eps_{l(mu)}[s_i] + shift_i
+__global__ void __launch_bounds__(kBlock) onsite9_kernel(int64_t n, const double* __restrict__ bond,
+                                                         double* __restrict__ onsite) {
+  const BondHeader& h = *reinterpret_cast<const BondHeader*>(bond);
+  const double* posw = bond + kBondHeaderBytes / 8;
+  const double* shift = posw + 4 * n;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kBlock) {
+    const int s = (int)posw[4 * i + 3];
+    const double sh = shift[i];
+    for (int mu = 0; mu < 9; ++mu) onsite[(size_t)mu * n + i] = h.onsite[mu == 0 ? 0 : (mu < 4 ? 1 : 2)][s] + sh;
+  }
+}
+
+// Gershgorin interval of the orbital matrix from either representation (rows = atoms x 9):
+// kBond: blocks rebuilt from the bond records; else read from the stored blocks
+template <bool kBond>
+__global__ void __launch_bounds__(128) bounds9_kernel(const int32_t* __restrict__ cols, int64_t n, int32_t K,
+                                                      const double* __restrict__ bond_or_blocks,
+                                                      const double* __restrict__ onsite,
+                                                      double* __restrict__ partial) {
+  double lo = INFINITY, hi = -INFINITY;
+  for (int64_t i = (int64_t)blockIdx.x * 128 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 128) {
+    double off[9];
+    for (int mu = 0; mu < 9; ++mu) off[mu] = 0.0;
+    double eps[9];
+    if (kBond) {
+      const BondHeader& h = *reinterpret_cast<const BondHeader*>(bond_or_blocks);
+      const double* posw = bond_or_blocks + kBondHeaderBytes / 8;
+      const Vec<4> pi = ld_rec(posw + 4 * i);
+      for (int k = 0; k < K; ++k) {
+        const int64_t j = cols[(size_t)k * n + i];
+        if (j == i) continue;
+        const Vec<4> pj = ld_rec(posw + 4 * j);
+        const Geometry g = bond_geometry(pi.v, pj.v, h.box, h.pbc, h.r0, h.beta);
+        const double* c0 = h.coef[(int)pi.v[3] * h.n_species + (int)pj.v[3]];
+        double c[kNc];
+        for (int q = 0; q < kNc; ++q) c[q] = c0[q] * g.f;
+        double E[9][9];
+        pair_block(g, c, E);
+        for (int mu = 0; mu < 9; ++mu)
+          for (int nu = 0; nu < 9; ++nu) off[mu] += fabs(E[mu][nu]);
+      }
+      const double sh = posw[4 * n + i];
+      for (int mu = 0; mu < 9; ++mu) eps[mu] = h.onsite[mu == 0 ? 0 : (mu < 4 ? 1 : 2)][(int)pi.v[3]] + sh;
+    } else {
+      for (int k = 0; k < K; ++k)
+        for (int nu = 0; nu < 9; ++nu)
+          for (int mu = 0; mu < 9; ++mu)
+            off[mu] += fabs(bond_or_blocks[((size_t)k * 81 + 9 * nu + mu) * n + i]);
+      for (int mu = 0; mu < 9; ++mu) eps[mu] = onsite ? onsite[(size_t)mu * n + i] : 0.0;
+    }
+    for (int mu = 0; mu < 9; ++mu) {
+      lo = fmin(lo, eps[mu] - off[mu]);
+      hi = fmax(hi, eps[mu] + off[mu]);
+    }
+  }
+  __shared__ double s[4][2];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  lo = warp_min(lo);
+  hi = warp_max(hi);
+  if (lane == 0) {
+    s[wid][0] = lo;
+    s[wid][1] = hi;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 4; ++w) {
+      lo = fmin(lo, s[w][0]);
+      hi = fmax(hi, s[w][1]);
+    }
+    partial[2 * blockIdx.x + 0] = lo;
+    partial[2 * blockIdx.x + 1] = hi;
+  }
+}
+
+__global__ void bounds9_final_kernel(const double* partial, int blocks, double* lo_hi) {
+  if (threadIdx.x == 0) {
+    double lo = partial[0], hi = partial[1];
+    for (int b = 1; b < blocks; ++b) {
+      lo = fmin(lo, partial[2 * b]);
+      hi = fmax(hi, partial[2 * b + 1]);
+    }
+    lo_hi[0] = lo;
+    lo_hi[1] = hi;
+  }
+}
+
+// ---- the fused pass, shared epilogue -------------------------------------------------------------------
+// phi rows are orbital rows 9 i + mu, as everywhere else; thread = (atom i, one 256-bit element t)
+template <int LOG2T, bool kFirst, bool kDotL>
+__device__ __forceinline__ void epilogue9(const StepArgs& a, int64_t i, int64_t t, const Vec<4> (&acc)[9],
+                                          const double (&eps)[9], double& s1, double& s2) {
+  constexpr int VW = 4;
+  constexpr int64_t kOrb = (int64_t)(1 << LOG2T) * VW;
+  const double scale = a.scale, b = a.b;
+#pragma unroll
+  for (int mu = 0; mu < 9; ++mu) {
+    const int64_t at = (9 * i + mu) * kOrb + t * VW;
+    const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
+    Vec<VW> prev, with;
+    if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
+    if (kDotL) with = load_stream<VW>(a.dot_with + at);
+    Vec<VW> y;
+#pragma unroll
+    for (int q = 0; q < VW; ++q) {
+      const double hx = fma(eps[mu], own.v[q], acc[mu].v[q]);
+      y.v[q] = (hx - b * own.v[q]) * scale;
+      if (!kFirst) y.v[q] -= prev.v[q];
+      s1 = fma(own.v[q], kDotL ? with.v[q] : own.v[q], s1);
+      s2 = fma(y.v[q], kDotL ? with.v[q] : own.v[q], s2);
+    }
+    store_stream<VW>(a.phi_io + at, y);
+  }
+}
+
+// ---- K7bb: stored blocks [K][81][n] ----------------------------------------------------------------------
+constexpr int kBlock9Threads = 256;
+
+template <int LOG2T, bool kFirst, bool kDotL>
+__global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int64_t kOrb = (int64_t)T * VW;
+  const int64_t n = a.n / 9;   // atoms
+  const int K = a.width;
+  const int64_t total = n * T;
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBlock9Threads + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBlock9Threads) {
+    const int64_t i = e >> LOG2T;
+    const int64_t t = e - i * T;
+    const double* xt = a.phi_cur + t * VW;
+    Vec<VW> acc[9];
+#pragma unroll
+    for (int mu = 0; mu < 9; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : 0;
+    for (int k = 0; k < K; ++k) {
+      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : 0;
+      const double* blk = a.vals + (size_t)k * 81 * n + i;
+      const double* xj = xt + 9 * j * kOrb;
+#pragma unroll 3
+      for (int nu = 0; nu < 9; ++nu) {
+        double hcol[9];
+#pragma unroll
+        for (int mu = 0; mu < 9; ++mu) hcol[mu] = ld_stream_f64(blk + (size_t)(9 * nu + mu) * n);
+        const Vec<VW> x = load_gather<VW>(xj + nu * kOrb);
+#pragma unroll
+        for (int mu = 0; mu < 9; ++mu)
+#pragma unroll
+          for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(hcol[mu], x.v[q], acc[mu].v[q]);
+      }
+      j = jn;
+    }
+    double eps[9];
+#pragma unroll
+    for (int mu = 0; mu < 9; ++mu) eps[mu] = a.diag ? ld_stream_f64(a.diag + (size_t)mu * n + i) : 0.0;
+    epilogue9<LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
+  }
+  block_store_sums<kBlock9Threads>(s1, s2, a.partial + blockIdx.x);
+}
+
+// ---- K7m: matrix-free, from the bond records ---------------------------------------------------------------
+// Per (atom, neighbour) the thread needs the neighbour's record (32 B) and its 9 orbital elements (9 x 32 B),
+// all gathers.  They are fetched one neighbour AHEAD with cp.async into the thread's own shared-memory slots
+// (two stages, 16-byte planes so that consecutive threads hit consecutive banks), so the gather latency
+// overlaps the ~400 fp64 instructions of the current pair; the elements are then read back one complex
+// number at a time, which keeps the live registers to the 36 accumulators plus one pair's temporaries.
+constexpr int kBond9Threads = 128;
+constexpr int kBondSlots = 20;                                   // 16-byte planes per stage: 2 (record) + 18 (x)
+constexpr size_t kBond9Smem = 2 * kBondSlots * 16 * kBond9Threads;   // 80 KB: two blocks per SM
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+template <int LOG2T, bool kFirst, bool kDotL>
+__global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const StepArgs a) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int64_t kOrb = (int64_t)T * VW;
+  extern __shared__ __align__(16) unsigned char s_stage[];
+  __shared__ double s_coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES * kNc];
+  __shared__ double s_onsite[3][GTB_MAX_SPECIES];
+  const BondHeader& h = *reinterpret_cast<const BondHeader*>(a.vals);
+  const int ns = h.n_species;
+  for (int q = threadIdx.x; q < ns * ns * kNc; q += kBond9Threads) s_coef[q] = (&h.coef[0][0])[q];
+  for (int q = threadIdx.x; q < 3 * GTB_MAX_SPECIES; q += kBond9Threads) (&s_onsite[0][0])[q] = (&h.onsite[0][0])[q];
+  // periodic axes: d -= L rint(d / L), as a multiplication by 1/L (a neighbour's d / L is within
+  // cutoff / L < 1/2 of an integer, far from the ties where the two roundings could differ)
+  const double Lx = h.box[0], Ly = h.box[1], Lz = h.box[2];
+  const double iLx = h.pbc[0] ? 1.0 / Lx : 0.0, iLy = h.pbc[1] ? 1.0 / Ly : 0.0, iLz = h.pbc[2] ? 1.0 / Lz : 0.0;
+  const double r0 = h.r0, beta = h.beta;
+  __syncthreads();
+  const int64_t n = a.n / 9;   // atoms
+  const int K = a.width;
+  const int64_t total = n * T;
+  const double* posw = a.vals + kBondHeaderBytes / 8;
+  const double* shift = posw + 4 * n;
+  const uint32_t slot0 = smem_u32_of(s_stage) + threadIdx.x * 16;
+  auto slot = [&](int stage, int plane) { return slot0 + (uint32_t)((stage * kBondSlots + plane) * 16 * kBond9Threads); };
+  auto plane_ptr = [&](int stage, int plane) {
+    return reinterpret_cast<const double2*>(s_stage + ((size_t)(stage * kBondSlots + plane) * kBond9Threads + threadIdx.x) * 16);
+  };
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBond9Threads + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBond9Threads) {
+    const int64_t i = e >> LOG2T;
+    const int64_t t = e - i * T;
+    const double* xt = a.phi_cur + t * VW;
+    const Vec<4> pi = ld_rec(posw + 4 * i);
+    const int si = (int)pi.v[3];
+    Vec<VW> acc[9];
+#pragma unroll
+    for (int mu = 0; mu < 9; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    auto prefetch = [&](int64_t j, int stage) {
+      const double* rec = posw + 4 * j;
+      cp_async16(slot(stage, 0), rec);
+      cp_async16(slot(stage, 1), rec + 2);
+      const double* xj = xt + 9 * j * kOrb;
+#pragma unroll
+      for (int nu = 0; nu < 9; ++nu) {
+        cp_async16(slot(stage, 2 + 2 * nu), xj + nu * kOrb);
+        cp_async16(slot(stage, 3 + 2 * nu), xj + nu * kOrb + 2);
+      }
+      cp_async_commit();
+    };
+    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : i;
+    int64_t jn = K > 1 ? (int64_t)ld_stream_i32(a.cols + (size_t)n + i) : i;
+    if (K > 0) prefetch(j, 0);
+    for (int k = 0; k < K; ++k) {
+      const int st = k & 1;
+      const int64_t jnn = k + 2 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 2) * n + i) : i;
+      if (k + 1 < K) {
+        prefetch(jn, st ^ 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
+      }
+      if (j != i) {   // padding slots carry the atom's own index
+        const double2 ra = *plane_ptr(st, 0), rb = *plane_ptr(st, 1);
+        double dx = __dsub_rn(ra.x, pi.v[0]), dy = __dsub_rn(ra.y, pi.v[1]), dz = __dsub_rn(rb.x, pi.v[2]);
+        dx = fma(-Lx, rint(dx * iLx), dx);
+        dy = fma(-Ly, rint(dy * iLy), dy);
+        dz = fma(-Lz, rint(dz * iLz), dz);
+        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const double inv = rsqrt(r2);
+        Geometry g;
+        g.l = dx * inv;
+        g.m = dy * inv;
+        g.n = dz * inv;
+        g.f = beta == 0.0 ? 1.0 : exp(-beta * (r2 * inv / r0 - 1.0));
+        const double* c0 = s_coef + (si * ns + (int)rb.y) * kNc;
+        double c[kNc];
+#pragma unroll
+        for (int q = 0; q < kNc; ++q) c[q] = c0[q] * g.f;
+        double D[5];
+        angular_d(g, D);
+        const double hl = 0.5 * kS3 * g.l, hm = 0.5 * kS3 * g.m, hn = 0.5 * kS3 * g.n;
+        const double l2 = 0.5 * g.l, m2 = 0.5 * g.m;
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {   // one complex number of the 256-bit element at a time
+          double2 x[9];
+#pragma unroll
+          for (int nu = 0; nu < 9; ++nu) x[nu] = *plane_ptr(st, 2 + 2 * nu + half);
+#pragma unroll
+          for (int ri = 0; ri < 2; ++ri) {
+            const int q = 2 * half + ri;
+            const double xs = ri ? x[0].y : x[0].x, px = ri ? x[1].y : x[1].x, py = ri ? x[2].y : x[2].x,
+                         pz = ri ? x[3].y : x[3].x;
+            const double d0 = ri ? x[4].y : x[4].x, d1 = ri ? x[5].y : x[5].x, d2 = ri ? x[6].y : x[6].x,
+                         d3 = ri ? x[7].y : x[7].x, d4 = ri ? x[8].y : x[8].x;
+            const double up = fma(g.l, px, fma(g.m, py, g.n * pz));                             // u . x_p
+            const double qd = fma(D[0], d0, fma(D[1], d1, fma(D[2], d2, fma(D[3], d3, D[4] * d4))));  // D . x_d
+            const double wx = fma(hm, d0, fma(hn, d2, fma(hl, d3, -l2 * d4)));                  // sum_b G_b x_d[b]
+            const double wy = fma(hl, d0, fma(hn, d1, fma(-hm, d3, -m2 * d4)));
+            const double wz = fma(hm, d1, fma(hl, d2, g.n * d4));
+            acc[0].v[q] += fma(c[0], xs, fma(c[1], up, c[2] * qd));
+            const double P = fma(c[3], xs, fma(c[5], up, c[6] * qd));
+            acc[1].v[q] += fma(c[4], px, fma(c[7], wx, g.l * P));
+            acc[2].v[q] += fma(c[4], py, fma(c[7], wy, g.m * P));
+            acc[3].v[q] += fma(c[4], pz, fma(c[7], wz, g.n * P));
+            const double Q = fma(c[8], xs, fma(c[9], up, c[12] * qd));
+            const double vx = fma(c[10], px, c[13] * wx), vy = fma(c[10], py, c[13] * wy),
+                         vz = fma(c[10], pz, c[13] * wz);
+            acc[4].v[q] += fma(c[11], d0, fma(D[0], Q, fma(hm, vx, hl * vy)));
+            acc[5].v[q] += fma(c[11], d1, fma(D[1], Q, fma(hn, vy, hm * vz)));
+            acc[6].v[q] += fma(c[11], d2, fma(D[2], Q, fma(hn, vx, hl * vz)));
+            acc[7].v[q] += fma(c[11], d3, fma(D[3], Q, fma(hl, vx, -hm * vy)));
+            acc[8].v[q] += fma(c[11], d4, fma(D[4], Q, fma(-l2, vx, fma(-m2, vy, g.n * vz))));
+          }
+        }
+      }
+      j = jn;
+      jn = jnn;
+    }
+    const double sh = ld_stream_f64(shift + i);
+    double eps[9];
+    eps[0] = s_onsite[0][si] + sh;
+#pragma unroll
+    for (int mu = 1; mu < 4; ++mu) eps[mu] = s_onsite[1][si] + sh;
+#pragma unroll
+    for (int mu = 4; mu < 9; ++mu) eps[mu] = s_onsite[2][si] + sh;
+    epilogue9<LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
+  }
+  block_store_sums<kBond9Threads>(s1, s2, a.partial + blockIdx.x);
+}
+
+template <int LOG2T, bool DOT>
+void pick_rep9(int rep, StepPlan* p) {
+  if (rep == 1) {
+    p->first = cheb_block9_kernel<LOG2T, true, DOT>;
+    p->next = cheb_block9_kernel<LOG2T, false, DOT>;
+    p->block = kBlock9Threads;
+    p->smem = 0;
+  } else {
+    p->first = cheb_bond9_kernel<LOG2T, true, DOT>;
+    p->next = cheb_bond9_kernel<LOG2T, false, DOT>;
+    p->block = kBond9Threads;
+    p->smem = kBond9Smem;
+  }
+}
+
+int grid_of(int64_t total, int threads) {
+  return (int)std::max<int64_t>(1, std::min<int64_t>((total + threads - 1) / threads, kMaxGrid));
+}
+
+int check_spd_model(const gtb_spd_model* m) {
+  if (!m || !m->onsite_s || !m->onsite_p || !m->onsite_d || !m->sk || m->n_species < 1 ||
+      m->n_species > GTB_MAX_SPECIES)
+    return GTB_ERR_INVALID_ARG;
+  // same-l integrals belong to both orderings of the pair: an asymmetric entry has no symmetric H
+  for (int s = 0; s < m->n_species; ++s)
+    for (int t = 0; t < s; ++t)
+      for (int q : {0, 2, 3, 7, 8, 9})
+        if (m->sk[((size_t)s * m->n_species + t) * 10 + q] != m->sk[((size_t)t * m->n_species + s) * 10 + q])
+          return GTB_ERR_INVALID_ARG;
+  return GTB_OK;
+}
+
+}  // namespace
+
+bool make_plan_rep9(const gtb_ell* H, int R, int rep, bool dot, StepPlan* p) {
+  if ((rep != 1 && rep != 2) || (R != 2 && R != 4 && R != 8) || H->width < 0 || !H->vals ||
+      (H->width > 0 && !H->cols) || (reinterpret_cast<uintptr_t>(H->vals) & 31u))
+    return false;
+  if (R == 2) { if (dot) pick_rep9<0, true>(rep, p); else pick_rep9<0, false>(rep, p); p->T = 1; }
+  else if (R == 4) { if (dot) pick_rep9<1, true>(rep, p); else pick_rep9<1, false>(rep, p); p->T = 2; }
+  else { if (dot) pick_rep9<2, true>(rep, p); else pick_rep9<2, false>(rep, p); p->T = 4; }
+  p->vw = 4;
+  p->stages = 0;
+  int dev = 0, sms = kSmCount, per_sm = 0;
+  if (p->smem > 0 &&
+      (cudaFuncSetAttribute(p->first, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem) != cudaSuccess ||
+       cudaFuncSetAttribute(p->next, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem) != cudaSuccess))
+    return false;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->next, p->block, p->smem) != cudaSuccess)
+    return false;
+  per_sm = std::max(1, per_sm);
+  const int64_t total = H->n * p->T;
+  p->grid = (int)std::max<int64_t>(1, std::min<int64_t>((total + p->block - 1) / p->block, (int64_t)sms * per_sm));
+  p->grid = std::min(p->grid, kMaxGrid);
+  return true;
+}
+
+}  // namespace gtb
+
+using namespace gtb;
+
+extern "C" size_t gtb_spd_bonds_bytes(int64_t n) {
+  if (n <= 0) return 0;
+  return align_up(kBondHeaderBytes + (size_t)n * 40);
+}
+
+extern "C" int gtb_spd_bonds(const gtb_ell* nbr, const double* pos, const int32_t* species,
+                             const double box[3], const int32_t pbc[3], const gtb_spd_model* model,
+                             gtb_ell* Hm, int32_t* status, void* stream) {
+  int rc = check_ell(nbr);
+  if (rc != GTB_OK) return rc;
+  rc = check_spd_model(model);
+  if (rc != GTB_OK) return rc;
+  if (!pos || !species || !box || !pbc || !Hm || !status || Hm->n != nbr->n || Hm->width != nbr->width ||
+      Hm->cols != nbr->cols || !Hm->vals || (reinterpret_cast<uintptr_t>(Hm->vals) & 255u))
+    return GTB_ERR_INVALID_ARG;
+  if (9 * nbr->n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
+  for (int a = 0; a < 3; ++a)
+    if (pbc[a] && !(box[a] > 0.0)) return GTB_ERR_INVALID_ARG;
+  BondHeader h{};
+  const int ns = model->n_species;
+  for (int a = 0; a < 3; ++a) {
+    h.box[a] = box[a];
+    h.pbc[a] = pbc[a];
+  }
+  h.r0 = model->r0;
+  h.beta = model->beta;
+  h.n_species = ns;
+  h.n = nbr->n;
+  for (int s = 0; s < ns; ++s) {
+    h.onsite[0][s] = model->onsite_s[s];
+    h.onsite[1][s] = model->onsite_p[s];
+    h.onsite[2][s] = model->onsite_d[s];
+    for (int t = 0; t < ns; ++t)
+      pair_coefficients(model->sk + ((size_t)s * ns + t) * 10, model->sk + ((size_t)t * ns + s) * 10,
+                        h.coef[s * ns + t]);
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int64_t n = nbr->n;
+  // the header goes up from pageable memory: the copy has left the host buffer when the call returns
+  GTB_CUDA_TRY(cudaMemcpyAsync(Hm->vals, &h, sizeof(h), cudaMemcpyHostToDevice, st));
+  GTB_CUDA_TRY(cudaStreamSynchronize(st));
+  GTB_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int32_t), st));
+  double* posw = Hm->vals + kBondHeaderBytes / 8;
+  bond_record_kernel<<<grid_of(n, kBlock), kBlock, 0, st>>>(n, pos, species, model->onsite_shift, ns, posw,
+                                                            posw + 4 * n, status);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}
+
+extern "C" int gtb_spd_blocks(const gtb_ell* Hm, gtb_ell* Hb, void* stream) {
+  int rc = check_ell(Hm);
+  if (rc != GTB_OK) return rc;
+  if (!Hb || Hb->n != Hm->n || Hb->width != Hm->width || Hb->cols != Hm->cols ||
+      (Hb->width > 0 && !Hb->vals) || (reinterpret_cast<uintptr_t>(Hb->vals) & 31u))
+    return GTB_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int64_t n = Hm->n;
+  if (Hm->width > 0) {
+    block9_assemble_kernel<<<grid_of(n * Hm->width, 128), 128, 0, st>>>(Hm->cols, n, Hm->width, Hm->vals,
+                                                                        Hb->vals);
+    GTB_LAUNCHED();
+  }
+  if (Hb->diag) {
+    onsite9_kernel<<<grid_of(n, kBlock), kBlock, 0, st>>>(n, Hm->vals, Hb->diag);
+    GTB_LAUNCHED();
+  }
+  return GTB_OK;
+}
+
+extern "C" size_t gtb_spd_bounds_workspace_bytes(void) { return align_up(sizeof(double) * 2 * kMaxGrid); }
+
+extern "C" int gtb_spd_bounds(const gtb_ell* H, int32_t mode, double* lo_hi, void* ws, size_t ws_bytes,
+                              void* stream) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if ((mode != GTB_MODE_BLOCK9 && mode != GTB_MODE_BOND9) || !lo_hi || !H->vals) return GTB_ERR_INVALID_ARG;
+  rc = check_ws(ws, ws_bytes, gtb_spd_bounds_workspace_bytes());
+  if (rc != GTB_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  double* partial = static_cast<double*>(ws);
+  const int grid = grid_of(H->n, 128);
+  if (mode == GTB_MODE_BOND9)
+    bounds9_kernel<true><<<grid, 128, 0, st>>>(H->cols, H->n, H->width, H->vals, nullptr, partial);
+  else
+    bounds9_kernel<false><<<grid, 128, 0, st>>>(H->cols, H->n, H->width, H->vals, H->diag, partial);
+  GTB_LAUNCHED();
+  bounds9_final_kernel<<<1, 32, 0, st>>>(partial, grid, lo_hi);
+  GTB_LAUNCHED();
+  return GTB_OK;
+}

@@ -143,8 +143,9 @@ std::vector<double2> bessel_coefficients(double a, double b, double dt) {
 }
 
 // state <- U(dt) state.  Buffers: *state (in), *s1, *s2 scratch; on return *state points at the
-// result and *s1, *s2 at the two free buffers.
-int evolve_in_place(const gtb_ell* H, const StepPlan& plan, double a, double b,
+// result and *s1, *s2 at the two free buffers.  fused: `plan` is a mode-2 plan (make_plan(..., 2, ...)):
+// the accumulation acc += c_m t_m runs inside the pass that produces t_m; else one caxpy launch per term.
+int evolve_in_place(const gtb_ell* H, const StepPlan& plan, bool fused, double a, double b,
                     const std::vector<double2>& c, int R, double** state, double** s1, double** s2,
                     double2* scratch_partial, cudaStream_t st) {
   const int64_t total = H->n * R;
@@ -163,11 +164,16 @@ int evolve_in_place(const gtb_ell* H, const StepPlan& plan, double a, double b,
     sa.phi_cur = cur;
     sa.phi_io = io;
     sa.scale = (m == 1 ? 1.0 : 2.0) / a;
-    launch_step(plan, m == 1, sa, st);  // io <- t_m
+    sa.axpy_acc = acc;
+    sa.axpy_cr = c[m].x;
+    sa.axpy_ci = c[m].y;
+    launch_step(plan, m == 1, sa, st);  // io <- t_m  (fused: and acc += c_m t_m)
     GTB_LAUNCHED();
-    caxpy_kernel<<<g, kBlock, 0, st>>>(total, c[m].x, c[m].y, reinterpret_cast<const double2*>(io),
-                                       reinterpret_cast<double2*>(acc), 0);
-    GTB_LAUNCHED();
+    if (!fused) {
+      caxpy_kernel<<<g, kBlock, 0, st>>>(total, c[m].x, c[m].y, reinterpret_cast<const double2*>(io),
+                                         reinterpret_cast<double2*>(acc), 0);
+      GTB_LAUNCHED();
+    }
     std::swap(cur, io);  // cur = t_m, io = t_{m-1} (overwritten by t_{m+1} next)
   }
   *state = acc;
@@ -242,14 +248,14 @@ extern "C" int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const VacWs w = carve_vac(ws, H->n, 2, 1, R);
   StepPlan plan;
-  rc = make_plan(H, R, false, nullptr, &plan);
+  rc = make_plan(H, R, 2, nullptr, &plan);
   if (rc != GTB_OK) return rc;
   const std::vector<double2> c = bessel_coefficients(a, b, dt);
   if (terms) *terms = (int32_t)c.size();
   const size_t bytes = sizeof(double) * (size_t)H->n * R * 2;
   double *state = w.buf[0], *s1 = w.buf[1], *s2 = w.buf[2];
   GTB_CUDA_TRY(cudaMemcpyAsync(state, phi, bytes, cudaMemcpyDeviceToDevice, st));
-  rc = evolve_in_place(H, plan, a, b, c, R, &state, &s1, &s2, w.partial, st);
+  rc = evolve_in_place(H, plan, true, a, b, c, R, &state, &s1, &s2, w.partial, st);
   if (rc != GTB_OK) return rc;
   GTB_CUDA_TRY(cudaMemcpyAsync(phi, state, bytes, cudaMemcpyDeviceToDevice, st));
   return GTB_OK;
@@ -294,11 +300,13 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan, dplan;  // evolution passes (no bra) and moment passes (dot with psiL)
     const bool direct = (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0;
+    bool fused = false;   // the blocked passes (K7b, K7b9) keep the separate accumulation kernel
     if (!(orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS) && make_plan_orb(H, R, orb, false, direct, &plan) &&
           make_plan_orb(H, R, orb, true, direct, &dplan))) {
-      rc = make_plan(H, R, false, opt, &plan);
+      fused = !(opt_flags & GTB_OPT_SEPARATE_AXPY);
+      rc = make_plan(H, R, fused ? 2 : 0, opt, &plan);
       if (rc != GTB_OK) return rc;
-      rc = make_plan(H, R, true, opt, &dplan);
+      rc = make_plan(H, R, 1, opt, &dplan);
       if (rc != GTB_OK) return rc;
     }
     double *psiL = w.buf[0], *psiR = w.buf[1], *sa_ = w.buf[2], *sb_ = w.buf[3];
@@ -310,9 +318,9 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     GTB_LAUNCHED();
     for (int j = 0; j < n_steps; ++j) {
       if (j > 0) {
-        rc = evolve_in_place(H, plan, a, b, coef, R, &psiL, &sa_, &sb_, w.partial, st);
+        rc = evolve_in_place(H, plan, fused, a, b, coef, R, &psiL, &sa_, &sb_, w.partial, st);
         if (rc != GTB_OK) return rc;
-        rc = evolve_in_place(H, plan, a, b, coef, R, &psiR, &sa_, &sb_, w.partial, st);
+        rc = evolve_in_place(H, plan, fused, a, b, coef, R, &psiR, &sa_, &sb_, w.partial, st);
         if (rc != GTB_OK) return rc;
       }
       double* cur = sa_;  // chi_0 = V psiR, partial slot 0 = Re<psiL|chi_0>

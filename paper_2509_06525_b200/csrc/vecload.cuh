@@ -74,6 +74,16 @@ __device__ __forceinline__ double ld_stream_f64(const double* p) {
   return v;
 }
 
+// acc += c * y on the complex numbers of a vector element (c = cr + i ci); the arithmetic of caxpy_kernel
+template <int VW>
+__device__ __forceinline__ void axpy_into(Vec<VW>& acc, const Vec<VW>& y, double cr, double ci) {
+#pragma unroll
+  for (int p = 0; p < VW / 2; ++p) {
+    acc.v[2 * p] = fma(cr, y.v[2 * p], fma(-ci, y.v[2 * p + 1], acc.v[2 * p]));
+    acc.v[2 * p + 1] = fma(cr, y.v[2 * p + 1], fma(ci, y.v[2 * p], acc.v[2 * p + 1]));
+  }
+}
+
 // block sums of the two dot products -> one double2 per block
 template <int kThreads>
 __device__ __forceinline__ void block_store_sums(double s1, double s2, double2* out) {

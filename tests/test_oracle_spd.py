@@ -170,3 +170,39 @@ def test_asymmetric_table_keeps_h_symmetric_and_the_doubling_identities_valid():
     m0 = oracle.kpm_moments(H, a, b, 24, 2, 7, mode=0, algo=0)
     m1 = oracle.kpm_moments(H, a, b, 24, 2, 7, mode=0, algo=1)
     assert np.abs(m0 - m1).max() <= 1e-12
+
+
+# ---------------------------------------------------------------------------------- P40
+def test_sampled_atom_step_equals_the_step_on_the_assembled_matrix():
+    """spd_step_atoms (H never materialised, vectors given sparsely; used at 10^8 atoms) against two
+    separately pinned functions: spd_hamiltonian (P31-P35, P39) + kpm_step_rows (dense product pin), on a
+    two-species disordered lattice, first and later steps, every atom; and random_phase_rows against
+    random_phase_fill."""
+    w = W.CONFIGS["c4"].scaled(6, 4, stripe=3)
+    inp = W.make_inputs(w)
+    species = (inp.species > 0).astype(np.int32)
+    shift = 0.01 * np.arange(len(species), dtype=float)
+    es, ep, ed, sk = [-8.0, -5.5], [0.3, -1.1], [6.5, 4.0], _asym_table()
+    nbr = oracle.build_hamiltonian(inp.pos, species, inp.box, inp.pbc, 2.65, [0.0, 0.0], np.ones((2, 2)),
+                                   with_diag=False)
+    H = oracle.spd_hamiltonian(nbr, inp.pos, species, inp.box, inp.pbc, es, ep, ed, sk, r0=1.42, beta=1.5,
+                               onsite_shift=shift)
+    n, K, R = nbr.n, nbr.width, 2
+    a, b = 31.0, -0.7
+    phi0 = oracle.random_phase_fill(5, 0, R, 9 * n)
+    rows = np.array([0, 7, 9 * n - 1, 40])
+    assert np.array_equal(oracle.random_phase_rows(5, 0, R, rows), phi0[rows])
+    all_rows = np.arange(9 * n)
+    phi1 = oracle.kpm_step_rows(H, a, b, True, None, phi0, all_rows)
+    phi2 = oracle.kpm_step_rows(H, a, b, False, phi0, phi1, all_rows)
+    atoms = np.arange(n)
+    def sparse(x):
+        xo = x.reshape(n, 9, R, 2)
+        return xo[atoms], xo[nbr.cols[:, atoms].T]          # [q][9][R][2], [q][K][9][R][2]
+    o0, n0 = sparse(phi0)
+    args = (nbr, inp.pos, species, inp.box, inp.pbc, es, ep, ed, sk, a, b)
+    got1 = oracle.spd_step_atoms(*args, True, atoms, o0, n0, r0=1.42, beta=1.5, onsite_shift=shift)
+    assert np.abs(got1.reshape(-1, R, 2) - phi1).max() <= 1e-15
+    o1, n1 = sparse(phi1)
+    got2 = oracle.spd_step_atoms(*args, False, atoms, o1, n1, prev=o0, r0=1.42, beta=1.5, onsite_shift=shift)
+    assert np.abs(got2.reshape(-1, R, 2) - phi2).max() <= 1e-15
