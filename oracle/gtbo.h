@@ -114,7 +114,7 @@ int gtbo_kpm_step_rows(const gtbo_ell* H, double a, double b, int32_t first,
                        const int64_t* rows, int64_t n_rows, double* out);
 
 /* --- C6: Jackson-damped DOS (Eq. 4) -------------------------- */
-/* kernel 0 = none (g_n = 1), 1 = Jackson.  rho = 0 where |(E-b)/a| >= 1.    */
+/* kernel 0 = none (g_n = 1), 1 = Jackson.  rho = 0 where |(E-b)/a| >= 1 - 8 eps (reading A13b). */
 int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
              const double* energies, int32_t G, double scale, double* rho);
 /* g[n], n = 0..M-1 (exported so the kernel itself can be pinned).           */

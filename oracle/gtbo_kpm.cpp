@@ -268,7 +268,9 @@ extern "C" int gtbo_jackson(int32_t M, double* g) {
 }
 
 // rho(E) = scale [g_0 mu_0 + 2 sum_{n>=1} g_n mu_n T_n(x)] / (pi a sqrt(1-x^2)),
-// x = (E-b)/a, T_n(x) = cos(n arccos x); rho = 0 for |x| >= 1.
+// x = (E-b)/a, T_n(x) = cos(n arccos x); rho = 0 for |x| >= 1 - 8 eps (reading A13b: a grid end
+// point b +- a evaluates to x = +-1 or an ulp or two inside by rounding alone; there 1/sqrt(1-x^2) ~ 1e8
+// multiplies a sum that cancels to rounding noise, so the point is treated as the end point it is).
 extern "C" int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t kernel,
                         const double* energies, int32_t G, double scale, double* rho) {
   if (!mu || !energies || !rho || M <= 0 || G < 0 || !(a > 0.0) ||
@@ -280,7 +282,7 @@ extern "C" int gtbo_dos(const double* mu, int32_t M, double a, double b, int32_t
 #pragma omp parallel for schedule(static)
   for (int32_t j = 0; j < G; ++j) {
     const double x = (energies[j] - b) / a;
-    if (!(std::fabs(x) < 1.0)) {
+    if (!(std::fabs(x) < 1.0 - 8.0 * 2.220446049250313e-16)) {
       rho[j] = 0.0;
       continue;
     }

@@ -40,6 +40,34 @@ DOUBLING = {"c3", "c3b", "c5"}      # configs whose full-depth run uses the orac
 M_CHECK = 48
 
 
+def remake_dos(key: str) -> None:
+    """--dos-only: rewrite <cfg>_dos_G<G>.txt from the stored moments (oracle.dos alone; used after reading
+    A13b changed the value at grid points within 8 eps of |x| = 1, which leaves the moments untouched)."""
+    w = W.CONFIGS[key]
+    head, mu = [], []
+    with open(os.path.join(HERE, f"{key}_moments_M{w.M}.txt")) as f:
+        for line in f:
+            t = line.split()
+            if line.startswith("#") and not line.startswith("# n "):
+                head.append(line.rstrip("\n"))
+            elif t and t[0] in ("a", "b", "inputs_sha256"):
+                head.append(line.rstrip("\n"))
+            elif t and t[0] == "mu":
+                mu.append(float.fromhex(t[2]))
+    vals = {l.split()[0]: l.split()[1] for l in head if not l.startswith("#")}
+    a, b = float.fromhex(vals["a"]), float.fromhex(vals["b"])
+    mu = np.array(mu)
+    assert mu.shape == (w.M,)
+    E = W.energy_grid(w, a, b)
+    rho = oracle.dos(mu, a, b, E)
+    with open(os.path.join(HERE, f"{key}_dos_G{E.shape[0]}.txt"), "w") as f:
+        f.write("\n".join(head) + "\n# j  E_j  rho(E_j)   (oracle.dos of the stored moments, Jackson kernel, scale 1;"
+                " reading A13b)\n")
+        for j, (e, r) in enumerate(zip(E, rho)):
+            f.write(f"rho {j} {float(e).hex()} {float(r).hex()}\n")
+    print(f"[{key}] DOS rewritten from the stored moments", flush=True)
+
+
 def make(key: str) -> None:
     w = W.CONFIGS[key]
     t0 = time.time()
@@ -91,6 +119,8 @@ def make(key: str) -> None:
 
 
 if __name__ == "__main__":
-    keys = sys.argv[1:] or ["c4", "c2b", "c2", "c3", "c5"]
+    args = sys.argv[1:]
+    dos_only = "--dos-only" in args
+    keys = [k for k in args if not k.startswith("--")] or ["c4", "c2b", "c2", "c3", "c5"]
     for k in keys:
-        make(k)
+        (remake_dos if dos_only else make)(k)

@@ -92,3 +92,27 @@ def test_graphene_dos_features(golden):
     # growing towards the van Hove peaks
     assert rho[1900:2101].max() < 0.05 * rho[k]
     assert rho[2000 + 150] < rho[2000 + 300] < rho[2000 + 450] < rho[2000 + 600]
+
+
+def test_grid_end_points_within_rounding_of_the_band_edge_are_outside():
+    """Reading A13b: rho = 0 for |x| >= 1 - 8 eps.  A grid end point E = b +- a evaluates to x = +-1 or an
+    ulp or two inside by rounding alone; the weight 1/(pi a sqrt(1 - x^2)) is ~1e8 there.  With mu = (1, 0, 0, ...)
+    and no damping the reconstruction IS that weight (closed form), so the rule is visible on its own:
+    zero at 1, 1 - eps, 1 - 4 eps (both signs), the closed form from 1 - 16 eps inwards."""
+    eps = 2.0**-52
+    a, b = 13.151754450485727, -0.017020550974913284          # config 2's scale
+    mu = np.zeros(8)
+    mu[0] = 1.0
+    for sgn in (1.0, -1.0):
+        xs_out = sgn * np.array([1.0, 1.0 - eps / 2, 1.0 - eps, 1.0 - 4 * eps, 1.0 - 8 * eps, 1.0 + eps, 1.5])
+        xs_in = sgn * np.array([1.0 - 16 * eps, 1.0 - 1e-12, 0.999, 0.3])
+        assert (oracle.dos(mu, 1.0, 0.0, xs_out, kernel=0) == 0.0).all()
+        got = oracle.dos(mu, 1.0, 0.0, xs_in, kernel=0)
+        want = 1.0 / (np.pi * np.sqrt((1.0 - xs_in) * (1.0 + xs_in)))
+        assert np.abs(got / want - 1.0).max() <= 1e-9
+    # config 2's own grid: the last point comes out one ulp inside the edge and is an end point
+    E = np.linspace(b - a, b + a, 4001)
+    x = (E - b) / a
+    assert abs(x[-1]) < 1.0 and abs(x[0]) >= 1.0
+    rho = oracle.dos(mu, a, b, E, kernel=0)
+    assert rho[0] == 0.0 and rho[-1] == 0.0 and rho[1] > 0.0 and rho[-2] > 0.0
