@@ -194,7 +194,8 @@ int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,
 
 /* ---- density of states (Eq. 4; north_star (4); reading C6) ---- */
 /* ASYNC.  rho(E_j) = scale*[g_0 mu_0 + 2 sum_{n=1}^{M-1} g_n mu_n T_n(x_j)] / (pi a sqrt(1-x_j^2)),
- * x_j = (E_j - b)/a, and rho = 0 where |x_j| >= 1.
+ * x_j = (E_j - b)/a, and rho = 0 where |x_j| >= 1 - 8 eps, eps = 2^-52 (the end points b +- a of a grid, up
+ * to the rounding of x_j: reading A13b).
  * kernel 0: g_n = 1;  kernel 1 (Jackson):
  *   g_n = [(M-n+1) cos(pi n/(M+1)) + sin(pi n/(M+1)) cot(pi/(M+1))]/(M+1).
  * mu, energies, rho: DEVICE. */

@@ -51,7 +51,7 @@ void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t
 bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, bool direct, StepPlan* p);
 // s,p,d Hamiltonian held as 9x9 blocks (rep = 1: gtb_spd_blocks) or as bonds (rep = 2: gtb_spd_bonds);
 // H->n counts atoms, the vectors have 9 H->n rows.  false when R is not 2, 4 or 8.
-bool make_plan_rep9(const gtb_ell* H, int R, int rep, bool dot, StepPlan* p);
+bool make_plan_rep9(const gtb_ell* H, int R, int rep, StepPlan* p);
 
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);

@@ -3,7 +3,9 @@
 // Eq. 4 of the paper (printed garbled, read rho(E) = (2/Omega) Tr delta(E - H)) in
 // its kernel-polynomial form (BASELINE.json:north_star (4); reading C6 in DESIGN.md):
 //   rho(E) = scale * [g_0 mu_0 + 2 sum_{n>=1} g_n mu_n T_n(x)] / (pi a sqrt(1 - x^2)),  x = (E-b)/a,
-// zero for |x| >= 1.  The Chebyshev sum is evaluated by the Clenshaw recurrence
+// zero for |x| >= 1 - 8 eps (reading A13b: a grid end point E = b +- a comes out of fl((fl(b +- a) - b)/a)
+// as +-1 or one or two ulps inside, where 1/sqrt(1 - x^2) ~ 10^8 only amplifies the rounding noise of the
+// cancelling sum; such points are the end points and get rho = 0 on both sides).  The Chebyshev sum is evaluated by the Clenshaw recurrence
 //   b_n = c_n + 2 x b_{n+1} - b_{n+2},  sum = c_0 + x b_1 - b_2,
 // one thread per energy point, with the damped coefficients c_n = 2 g_n mu_n staged through shared
 // memory in chunks from the highest order down.
@@ -52,7 +54,7 @@ dos_kernel(const double* __restrict__ mu, int32_t M, double a, double b, int32_t
   }
   if (j < G) {
     double r = 0.0;
-    if (fabs(x) < 1.0) {
+    if (fabs(x) < 1.0 - 8.0 * 2.220446049250313e-16) {   // reading A13b
       const double c0 = (kernel == 1 ? jackson_g(0, M) : 1.0) * mu[0];
       const double sum = fma(x, b1, c0) - b2;
       r = scale * sum / (3.14159265358979323846 * a * sqrt((1.0 - x) * (1.0 + x)));

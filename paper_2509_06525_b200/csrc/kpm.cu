@@ -858,7 +858,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     StepPlan plan;
     bool blocked = false;
     if (rep) {  // block / bond representation: no scalar reading exists
-      if (!make_plan_rep9(H, R, rep, false, &plan)) return GTB_ERR_INVALID_ARG;
+      if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
       blocked = true;
     } else if (orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS)) {
       blocked = make_plan_orb(H, R, orb, false, (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0, &plan);
@@ -965,7 +965,7 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   const int opt_flags = opt ? opt->flags : 0;
   bool blocked = false;
   if (rep) {
-    if (!make_plan_rep9(H, R, rep, false, &plan)) return GTB_ERR_INVALID_ARG;
+    if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
     blocked = true;
   } else if (orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS)) {
     blocked = make_plan_orb(H, R, orb, false, (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0, &plan);

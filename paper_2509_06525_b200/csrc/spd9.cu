@@ -132,10 +132,6 @@ __device__ void pair_block(const Geometry& g, const double* c, double E[9][9]) {
   }
 }
 
-__device__ __forceinline__ uint32_t smem_u32_of(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-
 __device__ __forceinline__ Vec<4> ld_rec(const double* p) {   // 32-byte atom record, read-only path
   return load_gather<4>(p);
 }
@@ -276,16 +272,25 @@ __global__ void bounds9_final_kernel(const double* partial, int blocks, double* 
 }
 
 // ---- the fused pass, shared epilogue -------------------------------------------------------------------
-// phi rows are orbital rows 9 i + mu, as everywhere else; thread = (atom i, one 256-bit element t)
+// thread = (atom i, one 256-bit element t); the vectors are orbital rows 9 i + mu, [9 n][R][2], as everywhere.
+// (An orbital-major layout [9][n][R][2] for the library's own vectors was built and measured: the gathers of
+// consecutive atoms do not share cache lines on these lattices -- same-sublattice atoms are 4 apart -- and
+// nine separate row streams per array cost more than they save: 2.44 -> 3.20 ms at K = 3, 6.27 -> 6.92 ms
+// at K = 12 for 1.02e7 atoms, R = 2; removed.)
+template <int LOG2T>
+__device__ __forceinline__ int64_t vec_off(int64_t i, int mu) {   // in 256-bit elements, before t
+  return (9 * i + mu) << LOG2T;
+}
+
 template <int LOG2T, bool kFirst, bool kDotL>
-__device__ __forceinline__ void epilogue9(const StepArgs& a, int64_t i, int64_t t, const Vec<4> (&acc)[9],
-                                          const double (&eps)[9], double& s1, double& s2) {
+__device__ __forceinline__ void epilogue9(const StepArgs& a, int64_t i, int64_t t,
+                                          const Vec<4> (&acc)[9], const double (&eps)[9], double& s1,
+                                          double& s2) {
   constexpr int VW = 4;
-  constexpr int64_t kOrb = (int64_t)(1 << LOG2T) * VW;
   const double scale = a.scale, b = a.b;
 #pragma unroll
   for (int mu = 0; mu < 9; ++mu) {
-    const int64_t at = (9 * i + mu) * kOrb + t * VW;
+    const int64_t at = (vec_off<LOG2T>(i, mu) + t) * VW;
     const Vec<VW> own = load_gather<VW>(a.phi_cur + at);
     Vec<VW> prev, with;
     if (!kFirst) prev = load_stream<VW>(a.phi_io + at);
@@ -310,7 +315,6 @@ template <int LOG2T, bool kFirst, bool kDotL>
 __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const StepArgs a) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
-  constexpr int64_t kOrb = (int64_t)T * VW;
   const int64_t n = a.n / 9;   // atoms
   const int K = a.width;
   const int64_t total = n * T;
@@ -329,13 +333,12 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
     for (int k = 0; k < K; ++k) {
       const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : 0;
       const double* blk = a.vals + (size_t)k * 81 * n + i;
-      const double* xj = xt + 9 * j * kOrb;
 #pragma unroll 3
       for (int nu = 0; nu < 9; ++nu) {
         double hcol[9];
 #pragma unroll
         for (int mu = 0; mu < 9; ++mu) hcol[mu] = ld_stream_f64(blk + (size_t)(9 * nu + mu) * n);
-        const Vec<VW> x = load_gather<VW>(xj + nu * kOrb);
+        const Vec<VW> x = load_gather<VW>(xt + vec_off<LOG2T>(j, nu) * VW);
 #pragma unroll
         for (int mu = 0; mu < 9; ++mu)
 #pragma unroll
@@ -352,30 +355,17 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
 }
 
 // ---- K7m: matrix-free, from the bond records ---------------------------------------------------------------
-// Per (atom, neighbour) the thread needs the neighbour's record (32 B) and its 9 orbital elements (9 x 32 B),
-// all gathers.  They are fetched one neighbour AHEAD with cp.async into the thread's own shared-memory slots
-// (two stages, 16-byte planes so that consecutive threads hit consecutive banks), so the gather latency
-// overlaps the ~400 fp64 instructions of the current pair; the elements are then read back one complex
-// number at a time, which keeps the live registers to the 36 accumulators plus one pair's temporaries.
+// Per (atom, neighbour): one column index, the neighbour's record (32 B) and its 9 orbital elements as
+// 256-bit gathers (issued before the geometry, whose ~100 dependent fp64 instructions cover their latency),
+// then 64 FMAs per real component.  (Staging the gathers through shared memory with cp.async one neighbour
+// ahead measured 20 % SLOWER: the pass is bound by L1 wavefronts -- one per 32-byte gather of a lane --
+// not by latency: ncu of that variant, l1tex data pipe 94 %, fp64 pipe 25 %.)
 constexpr int kBond9Threads = 128;
-constexpr int kBondSlots = 20;                                   // 16-byte planes per stage: 2 (record) + 18 (x)
-constexpr size_t kBond9Smem = 2 * kBondSlots * 16 * kBond9Threads;   // 80 KB: two blocks per SM
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-}
 
 template <int LOG2T, bool kFirst, bool kDotL>
 __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const StepArgs a) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
-  constexpr int64_t kOrb = (int64_t)T * VW;
-  extern __shared__ __align__(16) unsigned char s_stage[];
   __shared__ double s_coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES * kNc];
   __shared__ double s_onsite[3][GTB_MAX_SPECIES];
   const BondHeader& h = *reinterpret_cast<const BondHeader*>(a.vals);
@@ -393,11 +383,6 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
   const int64_t total = n * T;
   const double* posw = a.vals + kBondHeaderBytes / 8;
   const double* shift = posw + 4 * n;
-  const uint32_t slot0 = smem_u32_of(s_stage) + threadIdx.x * 16;
-  auto slot = [&](int stage, int plane) { return slot0 + (uint32_t)((stage * kBondSlots + plane) * 16 * kBond9Threads); };
-  auto plane_ptr = [&](int stage, int plane) {
-    return reinterpret_cast<const double2*>(s_stage + ((size_t)(stage * kBondSlots + plane) * kBond9Threads + threadIdx.x) * 16);
-  };
   double s1 = 0.0, s2 = 0.0;
   for (int64_t e = (int64_t)blockIdx.x * kBond9Threads + threadIdx.x; e < total;
        e += (int64_t)gridDim.x * kBond9Threads) {
@@ -411,33 +396,15 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
     for (int mu = 0; mu < 9; ++mu)
 #pragma unroll
       for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
-    auto prefetch = [&](int64_t j, int stage) {
-      const double* rec = posw + 4 * j;
-      cp_async16(slot(stage, 0), rec);
-      cp_async16(slot(stage, 1), rec + 2);
-      const double* xj = xt + 9 * j * kOrb;
-#pragma unroll
-      for (int nu = 0; nu < 9; ++nu) {
-        cp_async16(slot(stage, 2 + 2 * nu), xj + nu * kOrb);
-        cp_async16(slot(stage, 3 + 2 * nu), xj + nu * kOrb + 2);
-      }
-      cp_async_commit();
-    };
     int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : i;
-    int64_t jn = K > 1 ? (int64_t)ld_stream_i32(a.cols + (size_t)n + i) : i;
-    if (K > 0) prefetch(j, 0);
     for (int k = 0; k < K; ++k) {
-      const int st = k & 1;
-      const int64_t jnn = k + 2 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 2) * n + i) : i;
-      if (k + 1 < K) {
-        prefetch(jn, st ^ 1);
-        cp_async_wait<1>();
-      } else {
-        cp_async_wait<0>();
-      }
+      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : i;
       if (j != i) {   // padding slots carry the atom's own index
-        const double2 ra = *plane_ptr(st, 0), rb = *plane_ptr(st, 1);
-        double dx = __dsub_rn(ra.x, pi.v[0]), dy = __dsub_rn(ra.y, pi.v[1]), dz = __dsub_rn(rb.x, pi.v[2]);
+        const Vec<4> pj = ld_rec(posw + 4 * j);
+        Vec<VW> x[9];
+#pragma unroll
+        for (int nu = 0; nu < 9; ++nu) x[nu] = load_gather<VW>(xt + vec_off<LOG2T>(j, nu) * VW);
+        double dx = __dsub_rn(pj.v[0], pi.v[0]), dy = __dsub_rn(pj.v[1], pi.v[1]), dz = __dsub_rn(pj.v[2], pi.v[2]);
         dx = fma(-Lx, rint(dx * iLx), dx);
         dy = fma(-Ly, rint(dy * iLy), dy);
         dz = fma(-Lz, rint(dz * iLz), dz);
@@ -448,7 +415,7 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
         g.m = dy * inv;
         g.n = dz * inv;
         g.f = beta == 0.0 ? 1.0 : exp(-beta * (r2 * inv / r0 - 1.0));
-        const double* c0 = s_coef + (si * ns + (int)rb.y) * kNc;
+        const double* c0 = s_coef + (si * ns + (int)pj.v[3]) * kNc;
         double c[kNc];
 #pragma unroll
         for (int q = 0; q < kNc; ++q) c[q] = c0[q] * g.f;
@@ -457,40 +424,30 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
         const double hl = 0.5 * kS3 * g.l, hm = 0.5 * kS3 * g.m, hn = 0.5 * kS3 * g.n;
         const double l2 = 0.5 * g.l, m2 = 0.5 * g.m;
 #pragma unroll
-        for (int half = 0; half < 2; ++half) {   // one complex number of the 256-bit element at a time
-          double2 x[9];
-#pragma unroll
-          for (int nu = 0; nu < 9; ++nu) x[nu] = *plane_ptr(st, 2 + 2 * nu + half);
-#pragma unroll
-          for (int ri = 0; ri < 2; ++ri) {
-            const int q = 2 * half + ri;
-            const double xs = ri ? x[0].y : x[0].x, px = ri ? x[1].y : x[1].x, py = ri ? x[2].y : x[2].x,
-                         pz = ri ? x[3].y : x[3].x;
-            const double d0 = ri ? x[4].y : x[4].x, d1 = ri ? x[5].y : x[5].x, d2 = ri ? x[6].y : x[6].x,
-                         d3 = ri ? x[7].y : x[7].x, d4 = ri ? x[8].y : x[8].x;
-            const double up = fma(g.l, px, fma(g.m, py, g.n * pz));                             // u . x_p
-            const double qd = fma(D[0], d0, fma(D[1], d1, fma(D[2], d2, fma(D[3], d3, D[4] * d4))));  // D . x_d
-            const double wx = fma(hm, d0, fma(hn, d2, fma(hl, d3, -l2 * d4)));                  // sum_b G_b x_d[b]
-            const double wy = fma(hl, d0, fma(hn, d1, fma(-hm, d3, -m2 * d4)));
-            const double wz = fma(hm, d1, fma(hl, d2, g.n * d4));
-            acc[0].v[q] += fma(c[0], xs, fma(c[1], up, c[2] * qd));
-            const double P = fma(c[3], xs, fma(c[5], up, c[6] * qd));
-            acc[1].v[q] += fma(c[4], px, fma(c[7], wx, g.l * P));
-            acc[2].v[q] += fma(c[4], py, fma(c[7], wy, g.m * P));
-            acc[3].v[q] += fma(c[4], pz, fma(c[7], wz, g.n * P));
-            const double Q = fma(c[8], xs, fma(c[9], up, c[12] * qd));
-            const double vx = fma(c[10], px, c[13] * wx), vy = fma(c[10], py, c[13] * wy),
-                         vz = fma(c[10], pz, c[13] * wz);
-            acc[4].v[q] += fma(c[11], d0, fma(D[0], Q, fma(hm, vx, hl * vy)));
-            acc[5].v[q] += fma(c[11], d1, fma(D[1], Q, fma(hn, vy, hm * vz)));
-            acc[6].v[q] += fma(c[11], d2, fma(D[2], Q, fma(hn, vx, hl * vz)));
-            acc[7].v[q] += fma(c[11], d3, fma(D[3], Q, fma(hl, vx, -hm * vy)));
-            acc[8].v[q] += fma(c[11], d4, fma(D[4], Q, fma(-l2, vx, fma(-m2, vy, g.n * vz))));
-          }
+        for (int q = 0; q < VW; ++q) {
+          const double xs = x[0].v[q], px = x[1].v[q], py = x[2].v[q], pz = x[3].v[q];
+          const double d0 = x[4].v[q], d1 = x[5].v[q], d2 = x[6].v[q], d3 = x[7].v[q], d4 = x[8].v[q];
+          const double up = fma(g.l, px, fma(g.m, py, g.n * pz));                             // u . x_p
+          const double qd = fma(D[0], d0, fma(D[1], d1, fma(D[2], d2, fma(D[3], d3, D[4] * d4))));  // D . x_d
+          const double wx = fma(hm, d0, fma(hn, d2, fma(hl, d3, -l2 * d4)));                  // sum_b G_b x_d[b]
+          const double wy = fma(hl, d0, fma(hn, d1, fma(-hm, d3, -m2 * d4)));
+          const double wz = fma(hm, d1, fma(hl, d2, g.n * d4));
+          acc[0].v[q] = fma(c[0], xs, fma(c[1], up, fma(c[2], qd, acc[0].v[q])));
+          const double P = fma(c[3], xs, fma(c[5], up, c[6] * qd));
+          acc[1].v[q] = fma(c[4], px, fma(c[7], wx, fma(g.l, P, acc[1].v[q])));
+          acc[2].v[q] = fma(c[4], py, fma(c[7], wy, fma(g.m, P, acc[2].v[q])));
+          acc[3].v[q] = fma(c[4], pz, fma(c[7], wz, fma(g.n, P, acc[3].v[q])));
+          const double Q = fma(c[8], xs, fma(c[9], up, c[12] * qd));
+          const double vx = fma(c[10], px, c[13] * wx), vy = fma(c[10], py, c[13] * wy),
+                       vz = fma(c[10], pz, c[13] * wz);
+          acc[4].v[q] = fma(c[11], d0, fma(D[0], Q, fma(hm, vx, fma(hl, vy, acc[4].v[q]))));
+          acc[5].v[q] = fma(c[11], d1, fma(D[1], Q, fma(hn, vy, fma(hm, vz, acc[5].v[q]))));
+          acc[6].v[q] = fma(c[11], d2, fma(D[2], Q, fma(hn, vx, fma(hl, vz, acc[6].v[q]))));
+          acc[7].v[q] = fma(c[11], d3, fma(D[3], Q, fma(hl, vx, fma(-hm, vy, acc[7].v[q]))));
+          acc[8].v[q] = fma(c[11], d4, fma(D[4], Q, fma(-l2, vx, fma(-m2, vy, fma(g.n, vz, acc[8].v[q])))));
         }
       }
       j = jn;
-      jn = jnn;
     }
     const double sh = ld_stream_f64(shift + i);
     double eps[9];
@@ -504,19 +461,18 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
   block_store_sums<kBond9Threads>(s1, s2, a.partial + blockIdx.x);
 }
 
-template <int LOG2T, bool DOT>
+template <int LOG2T>
 void pick_rep9(int rep, StepPlan* p) {
   if (rep == 1) {
-    p->first = cheb_block9_kernel<LOG2T, true, DOT>;
-    p->next = cheb_block9_kernel<LOG2T, false, DOT>;
+    p->first = cheb_block9_kernel<LOG2T, true, false>;
+    p->next = cheb_block9_kernel<LOG2T, false, false>;
     p->block = kBlock9Threads;
-    p->smem = 0;
   } else {
-    p->first = cheb_bond9_kernel<LOG2T, true, DOT>;
-    p->next = cheb_bond9_kernel<LOG2T, false, DOT>;
+    p->first = cheb_bond9_kernel<LOG2T, true, false>;
+    p->next = cheb_bond9_kernel<LOG2T, false, false>;
     p->block = kBond9Threads;
-    p->smem = kBond9Smem;
   }
+  p->smem = 0;
 }
 
 int grid_of(int64_t total, int threads) {
@@ -538,13 +494,13 @@ int check_spd_model(const gtb_spd_model* m) {
 
 }  // namespace
 
-bool make_plan_rep9(const gtb_ell* H, int R, int rep, bool dot, StepPlan* p) {
+bool make_plan_rep9(const gtb_ell* H, int R, int rep, StepPlan* p) {
   if ((rep != 1 && rep != 2) || (R != 2 && R != 4 && R != 8) || H->width < 0 || !H->vals ||
       (H->width > 0 && !H->cols) || (reinterpret_cast<uintptr_t>(H->vals) & 31u))
     return false;
-  if (R == 2) { if (dot) pick_rep9<0, true>(rep, p); else pick_rep9<0, false>(rep, p); p->T = 1; }
-  else if (R == 4) { if (dot) pick_rep9<1, true>(rep, p); else pick_rep9<1, false>(rep, p); p->T = 2; }
-  else { if (dot) pick_rep9<2, true>(rep, p); else pick_rep9<2, false>(rep, p); p->T = 4; }
+  if (R == 2) { pick_rep9<0>(rep, p); p->T = 1; }
+  else if (R == 4) { pick_rep9<1>(rep, p); p->T = 2; }
+  else { pick_rep9<2>(rep, p); p->T = 4; }
   p->vw = 4;
   p->stages = 0;
   int dev = 0, sms = kSmCount, per_sm = 0;
