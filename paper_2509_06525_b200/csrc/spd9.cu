@@ -282,11 +282,10 @@ __device__ __forceinline__ int64_t vec_off(int64_t i, int mu) {   // in 256-bit 
   return (9 * i + mu) << LOG2T;
 }
 
-template <int LOG2T, bool kFirst, bool kDotL>
+template <int VW, int LOG2T, bool kFirst, bool kDotL>
 __device__ __forceinline__ void epilogue9(const StepArgs& a, int64_t i, int64_t t,
-                                          const Vec<4> (&acc)[9], const double (&eps)[9], double& s1,
+                                          const Vec<VW> (&acc)[9], const double (&eps)[9], double& s1,
                                           double& s2) {
-  constexpr int VW = 4;
   const double scale = a.scale, b = a.b;
 #pragma unroll
   for (int mu = 0; mu < 9; ++mu) {
@@ -349,7 +348,7 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
     double eps[9];
 #pragma unroll
     for (int mu = 0; mu < 9; ++mu) eps[mu] = a.diag ? ld_stream_f64(a.diag + (size_t)mu * n + i) : 0.0;
-    epilogue9<LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
+    epilogue9<VW, LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
   }
   block_store_sums<kBlock9Threads>(s1, s2, a.partial + blockIdx.x);
 }
@@ -362,9 +361,12 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
 // not by latency: ncu of that variant, l1tex data pipe 94 %, fp64 pipe 25 %.)
 constexpr int kBond9Threads = 128;
 
-template <int LOG2T, bool kFirst, bool kDotL>
+// (Also measured and removed: one complex number per thread, 160 registers and 12 instead of 8 warps per
+// SM for a second copy of the geometry -- the same 6.24 ms at K = 12; an L2 prefetch of the rows two grid
+// strides ahead -- 5 % slower.  ncu at 10^8 atoms, K = 12: fp64 pipe 35 %, L1 data pipe 57 %, DRAM 24 % with
+// traffic = 1.006 x the algorithmic bytes, 5.3 stall cycles per issue on long_scoreboard.)
+template <int VW, int LOG2T, bool kFirst, bool kDotL>
 __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const StepArgs a) {
-  constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
   __shared__ double s_coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES * kNc];
   __shared__ double s_onsite[3][GTB_MAX_SPECIES];
@@ -456,20 +458,22 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
     for (int mu = 1; mu < 4; ++mu) eps[mu] = s_onsite[1][si] + sh;
 #pragma unroll
     for (int mu = 4; mu < 9; ++mu) eps[mu] = s_onsite[2][si] + sh;
-    epilogue9<LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
+    epilogue9<VW, LOG2T, kFirst, kDotL>(a, i, t, acc, eps, s1, s2);
   }
   block_store_sums<kBond9Threads>(s1, s2, a.partial + blockIdx.x);
 }
 
 template <int LOG2T>
 void pick_rep9(int rep, StepPlan* p) {
+  p->vw = 4;
+  p->T = 1 << LOG2T;
   if (rep == 1) {
     p->first = cheb_block9_kernel<LOG2T, true, false>;
     p->next = cheb_block9_kernel<LOG2T, false, false>;
     p->block = kBlock9Threads;
   } else {
-    p->first = cheb_bond9_kernel<LOG2T, true, false>;
-    p->next = cheb_bond9_kernel<LOG2T, false, false>;
+    p->first = cheb_bond9_kernel<4, LOG2T, true, false>;
+    p->next = cheb_bond9_kernel<4, LOG2T, false, false>;
     p->block = kBond9Threads;
   }
   p->smem = 0;
@@ -498,10 +502,9 @@ bool make_plan_rep9(const gtb_ell* H, int R, int rep, StepPlan* p) {
   if ((rep != 1 && rep != 2) || (R != 2 && R != 4 && R != 8) || H->width < 0 || !H->vals ||
       (H->width > 0 && !H->cols) || (reinterpret_cast<uintptr_t>(H->vals) & 31u))
     return false;
-  if (R == 2) { pick_rep9<0>(rep, p); p->T = 1; }
-  else if (R == 4) { pick_rep9<1>(rep, p); p->T = 2; }
-  else { pick_rep9<2>(rep, p); p->T = 4; }
-  p->vw = 4;
+  if (R == 2) pick_rep9<0>(rep, p);
+  else if (R == 4) pick_rep9<1>(rep, p);
+  else pick_rep9<2>(rep, p);
   p->stages = 0;
   int dev = 0, sms = kSmCount, per_sm = 0;
   if (p->smem > 0 &&

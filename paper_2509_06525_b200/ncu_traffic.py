@@ -28,6 +28,7 @@ def dram_bytes_per_launch(rows, kernel_substring: str):
             raise SystemExit(f"expected bytes (use --print-units base), got unit {units[col]!r}")
     vals = [float(r[rd].replace(",", "")) + float(r[wr].replace(",", ""))
             for r in rows[2:] if len(r) > max(rd, wr) and kernel_substring in r[name_col]]
+    vals = [v for v in vals if v == v]          # a launch the capture cut short reads nan
     if not vals:
         raise SystemExit(f"no launch of a kernel matching {kernel_substring!r} in the capture")
     return sum(vals) / len(vals), len(vals)
