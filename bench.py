@@ -35,6 +35,7 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
 KERNEL = "auto"                 # set by --kernel: pins the fused-pass kernel through gtb_kpm_options
+PACK = True                     # cleared by --no-pack: packed narrow rows (gtb_pack_ell, K7x2p) when the matrix fits
 REP = "scalar"                  # set by --rep (spd only): scalar ELL expansion, stored 9x9 blocks, or bonds (matrix-free)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x clocks.max.sm
 HOPPING = "analytic"            # set by --hopping: "analytic" t(r) or "mlp" (descriptor + MLPs of Eq. 2)
@@ -260,6 +261,8 @@ def run_ours(args):
     n_orb = ORB_COUNT[ORBITALS] * n                   # rows of H: the unit of the metric
     ws_kpm = gtb.workspace(gtb.kpm_workspace_bytes(n_orb, w.M, w.R), dev)
     ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n_orb), dev)
+    gtb.lib().gtb_pack_workspace_bytes.restype = __import__("ctypes").c_size_t
+    ws_pack = gtb.workspace(int(gtb.lib().gtb_pack_workspace_bytes()), dev)
     mu = torch.empty(w.M, dtype=torch.float64, device=dev)
     h_rho = torch.empty(w.n_energies, dtype=torch.float64).pin_memory()
     state = {}
@@ -312,7 +315,13 @@ def run_ours(args):
         else:
             a, b = w.a, w.b
         kmode = {"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0)
-        gtb.kpm_moments(H, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu, opt=opt)
+        Hk = H
+        state["packed"] = None
+        if PACK and KERNEL == "auto" and ORBITALS == "pz" and H.width <= 4 and w.R in (2, 4, 8) and n * (w.R // 2) > 148 * 8 * 256:
+            P = gtb.pack_ell(H, ws=ws_pack)          # part of the timed step; None: does not fit, plain path
+            if P is not None:
+                Hk, kmode, state["packed"] = P, gtb.MODE_PACKED, P
+        gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         rho = gtb.dos(mu, a, b, state["E"])
@@ -372,6 +381,10 @@ def run_ours(args):
     B = ORB_COUNT[ORBITALS]
     per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
     flops_per_launch = None
+    plain_per_atom = per_atom
+    packed = state.get("packed")
+    if packed is not None:   # one 16-byte word per row (+ the diagonal array when K = 4), + the vectors
+        per_atom = 16 + (8 if packed.diag is not None else 0) + 48 * w.R
     rep9 = ORBITALS == "spd" and REP != "scalar"
     if rep9 and REP == "blocks":   # per ATOM: K x (column + 81 values) + 9 onsite + 9 orbital rows of vectors; / 9 per row
         per_atom = (H.width * (4 + 648) + 72 + 9 * 48 * w.R) / 9.0
@@ -389,9 +402,12 @@ def run_ours(args):
     vec = w.R in (2, 4, 8)
     tile = KERNEL == "tile" or (KERNEL == "auto" and H.width > 4 and n % 4 == 0 and vec)
     x2 = KERNEL == "row_x2" or (KERNEL == "auto" and H.width <= 4 and vec)
-    if rep9:
+    if rep9 or packed is not None:
         small = False
-    k7_name = ("cheb_bond9_kernel (K7m: fused Chebyshev pass, 9x9 pair action rebuilt from the bond vector)"
+    k7_name = ("cheb_packed_kernel (K7x2p: fused Chebyshev pass on packed rows, 16-bit relative columns + value "
+               "dictionary of %d entries, two elements in flight per thread)" % packed.n_values
+               if packed is not None else
+               "cheb_bond9_kernel (K7m: fused Chebyshev pass, 9x9 pair action rebuilt from the bond vector)"
                if rep9 and REP == "bonds" else
                "cheb_block9_kernel (K7bb: fused Chebyshev pass on stored 9x9 blocks [K][81][n])" if rep9 else
                "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
@@ -402,12 +418,16 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": k7_name,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                "traffic": _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS +
+                "traffic": _ncu_traffic("dos-packed", w.name) if packed is not None else
+                _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS +
                                         ("" if REP == "scalar" else "-" + REP), w.name)
                 if KERNEL == "auto" else None,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "bytes_per_atom_pass": per_atom,
                 "ms_per_launch": k7_ms, "launches_timed": loop_passes,
                 "share_of_step": loop_ms / ms}
+    if packed is not None:   # NEXT-4: fewer bytes than the sec. 8(d) bound; both figures side by side
+        roofline["uncompressed_bytes_per_atom_pass"] = plain_per_atom
+        roofline["frac_on_uncompressed_bytes"] = float(n_orb) * plain_per_atom / (k7_ms * 1e-3) / 1e9 / peak
     if flops_per_launch is not None:   # the matrix-free pass has two roofs: report against the lower one
         t_hbm = bytes_per_launch / (peak * 1e9)
         t_alu = flops_per_launch / (FP64_PEAK_TFLOPS * 1e12)
@@ -425,7 +445,8 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128 vectors)",
             "data": "synthetic",
             "config": {"workload": w.name, "atoms": n, "orbitals_per_atom": n_orb // n,
-                       "ell_width": H.width, "representation": REP if ORBITALS == "spd" else "ell",
+                       "ell_width": H.width,
+                       "representation": REP if ORBITALS == "spd" else "packed rows" if packed is not None else "ell",
                        "cutoff_A": w.cutoff, "moments": w.M,
                        "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (
@@ -603,12 +624,14 @@ def main():
                    help="pin the fused-pass kernel (gtb_kpm_options.kernel); auto: picked from the matrix shape")
     p.add_argument("--rep", default="bonds", choices=["scalar", "blocks", "bonds"],
                    help="--orbitals spd: scalar ELL expansion (K7b9), stored 9x9 blocks (K7bb) or bonds = matrix-free (K7m)")
+    p.add_argument("--no-pack", action="store_true", help="keep narrow matrices on the plain ELL path (K7x2)")
     p.add_argument("--cutoff", type=float, default=0.0, help="override the neighbour cutoff in Angstrom "
                    "(3.0 on the pristine lattice = third-nearest neighbours, K = 12: Fig. 4a)")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS, HOPPING, KERNEL, REP
+    global ORBITALS, HOPPING, KERNEL, REP, PACK
+    PACK = not args.no_pack
     KERNEL = args.kernel
     REP = args.rep
     ORBITALS = args.orbitals

@@ -54,12 +54,15 @@ enum {
   GTB_ERR_WORKSPACE = -4,     /* workspace NULL, misaligned (256 B) or too small   */
   GTB_ERR_DIVERGED = -5,      /* non-finite moments: spectrum outside [b-a, b+a]   */
   GTB_ERR_CUDA = -6,          /* CUDA runtime error; see gtb_last_cuda_error()     */
-  GTB_ERR_INDEX_RANGE = -7    /* n too large for int32 indices                     */
+  GTB_ERR_INDEX_RANGE = -7,   /* n too large for int32 indices                     */
+  GTB_ERR_NOT_PACKABLE = -8   /* gtb_pack_ell: width > 4, a column offset beyond +-32767 rows or more than
+                                 65535 distinct values: stay on the plain ELL path       */
 };
 
 #define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian  (4 orbitals) */
 #define GTB_MODE_ORB9 32 /* ... from gtb_spd_hamiltonian (9 orbitals per atom)                           */
 #define GTB_MODE_BLOCK9 64  /* ... H holds the 9x9 blocks written by gtb_spd_blocks (H->n = atoms)          */
+#define GTB_MODE_PACKED 256 /* ... H holds the packed rows and value dictionary written by gtb_pack_ell     */
 #define GTB_MODE_BOND9 128  /* ... H holds the bond description written by gtb_spd_bonds (matrix-free)      */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
@@ -364,6 +367,24 @@ int gtb_spd_bonds(const gtb_ell* nbr, const double* pos, const int32_t* species,
 int gtb_spd_blocks(const gtb_ell* Hm, gtb_ell* Hb, void* stream);
 size_t gtb_spd_bounds_workspace_bytes(void);
 int gtb_spd_bounds(const gtb_ell* H, int32_t mode, double* lo_hi, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- compressed Hamiltonian stream for narrow rows ----
+ * For K <= 4 a row is packed into one 16-byte word: per slot a 16-bit column offset relative to the row
+ * (ring distance) and a 16-bit index into a dictionary of the distinct fp64 hopping values (lossless);
+ * with K <= 3 the fourth slot carries the dictionary index of the onsite energy.  H then costs 16 bytes per
+ * atom and pass instead of 12 K + 8 [diag]: config 5 132 -> 112, config 4 428 -> 400 bytes per atom.
+ *   P->n = H->n, P->width = H->width, P->cols = caller-allocated DEVICE block of gtb_packed_rows_bytes(n)
+ *   bytes (16-byte aligned) receiving the packed rows, P->vals = caller-allocated DEVICE block of
+ *   gtb_packed_dict_bytes() bytes receiving a 256-byte header and the dictionary; on return P->diag = NULL,
+ *   or H->diag when K = 4 (the diagonal array is then still read).
+ * SYNC.  GTB_ERR_NOT_PACKABLE when the matrix does not fit the format (any beta != 0 model: every hopping
+ * distinct); *n_values (HOST, may be NULL) receives the dictionary size.
+ * gtb_kpm_moments / gtb_kpm_step(P, ..., mode | GTB_MODE_PACKED) run K7x2p, the two-elements-in-flight
+ * pass reading this word: R_batch in {2, 4, 8}; same values in the same order, so bit-identical vectors. */
+size_t gtb_pack_workspace_bytes(void);
+size_t gtb_packed_rows_bytes(int64_t n);
+size_t gtb_packed_dict_bytes(void);
+int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_bytes, void* stream, int32_t* n_values);
 
 /* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
  *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):

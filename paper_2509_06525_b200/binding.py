@@ -20,7 +20,7 @@ from . import build as _build
 
 OK = 0
 ERR_INVALID_ARG, ERR_BOX_TOO_SMALL, ERR_ELL_OVERFLOW, ERR_WORKSPACE = -1, -2, -3, -4
-ERR_DIVERGED, ERR_CUDA, ERR_INDEX_RANGE = -5, -6, -7
+ERR_DIVERGED, ERR_CUDA, ERR_INDEX_RANGE, ERR_NOT_PACKABLE = -5, -6, -7, -8
 MAX_WIDTH = 64
 
 # every symbol include/gtb.h declares (tests check that the library exports each of them)
@@ -35,6 +35,7 @@ EXPORTS = (
     "gtb_sk_hamiltonian", "gtb_mlp_weight_count", "gtb_mlp_hamiltonian",
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_spd_bonds_bytes", "gtb_spd_bonds",
     "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
+    "gtb_pack_workspace_bytes", "gtb_packed_rows_bytes", "gtb_packed_dict_bytes", "gtb_pack_ell",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
@@ -43,6 +44,7 @@ OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT, OPT_SEPARATE_AXPY = 1,
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_BLOCK9 = 64            # ... the block form written by spd_blocks (H.n = atoms)
 MODE_BOND9 = 128            # ... the bond form written by spd_bonds (matrix-free)
+MODE_PACKED = 256           # ... the packed rows + value dictionary written by pack_ell (K <= 4)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
 
@@ -632,6 +634,33 @@ def spd_bounds(H: Ell, mode: int) -> torch.Tensor:
     _check(lib().gtb_spd_bounds(C.byref(hc), C.c_int32(mode), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()),
                                 _stream()), "spd_bounds")
     return out
+
+
+def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:
+    """The packed form of a narrow matrix (K <= 4) for mode=MODE_PACKED: `cols` holds the 16-byte packed rows
+    (int32 [n][4]), `vals` the header + value dictionary.  None when the matrix does not fit the format
+    (GTB_ERR_NOT_PACKABLE): stay on the plain path."""
+    L = lib()
+    for name in ("gtb_pack_workspace_bytes", "gtb_packed_dict_bytes"):
+        getattr(L, name).restype = C.c_size_t
+    L.gtb_packed_rows_bytes.restype = C.c_size_t
+    L.gtb_packed_rows_bytes.argtypes = [C.c_int64]
+    dev = H.vals.device
+    if ws is None:
+        ws = workspace(int(L.gtb_pack_workspace_bytes()), dev)
+    rows = torch.empty((int(L.gtb_packed_rows_bytes(H.n)) // 16, 4), dtype=torch.int32, device=dev)
+    blob = torch.empty(int(L.gtb_packed_dict_bytes()) // 8, dtype=torch.float64, device=dev)
+    P = Ell(H.n, H.width, rows, blob, None)
+    hc, pc = H._c(), P._c()
+    nv = C.c_int32(0)
+    st = L.gtb_pack_ell(C.byref(hc), C.byref(pc), _ptr(ws), C.c_size_t(ws.numel()), _stream(), C.byref(nv))
+    if st == ERR_NOT_PACKABLE:
+        return None
+    _check(st, "pack_ell")
+    if pc.diag:                      # K = 4 with a diagonal: the array is still read
+        P.diag = H.diag
+    P.n_values = int(nv.value)
+    return P
 
 
 # ---------------------------------------------------------------- Fig. 4b post-processing

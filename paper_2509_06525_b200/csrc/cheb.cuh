@@ -53,6 +53,9 @@ bool make_plan_orb(const gtb_ell* H, int R, int B, bool dot, bool direct, StepPl
 // H->n counts atoms, the vectors have 9 H->n rows.  false when R is not 2, 4 or 8.
 bool make_plan_rep9(const gtb_ell* H, int R, int rep, StepPlan* p);
 
+// packed narrow rows (gtb_pack_ell); mode as make_plan's dot; false when (P, R) does not fit
+bool make_plan_packed(const gtb_ell* P, int R, int mode, StepPlan* p);
+
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);
 // mode 0: random phases of (seed, r0..r0+R-1); mode 1: basis vectors e_{r0}..e_{r0+R-1}

@@ -828,11 +828,13 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
   if (rc != GTB_OK) return rc;
   rc = check_options(opt);
   if (rc != GTB_OK) return rc;
-  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9)) ||
+  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED)) ||
       ((mode_flags & GTB_MODE_ORB4) != 0) + ((mode_flags & GTB_MODE_ORB9) != 0) +
-              ((mode_flags & GTB_MODE_BLOCK9) != 0) + ((mode_flags & GTB_MODE_BOND9) != 0) > 1)
+              ((mode_flags & GTB_MODE_BLOCK9) != 0) + ((mode_flags & GTB_MODE_BOND9) != 0) +
+              ((mode_flags & GTB_MODE_PACKED) != 0) > 1)
     return GTB_ERR_INVALID_ARG;
   const int32_t mode = mode_flags & 1;
+  const bool packed = (mode_flags & GTB_MODE_PACKED) != 0;
   const int opt_flags = opt ? opt->flags : 0;
   const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   const int rep = (mode_flags & GTB_MODE_BLOCK9) ? 1 : (mode_flags & GTB_MODE_BOND9) ? 2 : 0;
@@ -857,7 +859,10 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     const bool last_batch = r0 + R_batch >= n_vec;
     StepPlan plan;
     bool blocked = false;
-    if (rep) {  // block / bond representation: no scalar reading exists
+    if (packed) {  // packed rows: no plain reading exists
+      if (!make_plan_packed(H, R, 0, &plan)) return GTB_ERR_INVALID_ARG;
+      blocked = true;
+    } else if (rep) {  // block / bond representation: no scalar reading exists
       if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
       blocked = true;
     } else if (orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS)) {
@@ -948,8 +953,9 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   if (rc != GTB_OK) return rc;
   const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   const int rep = (mode_flags & GTB_MODE_BLOCK9) ? 1 : (mode_flags & GTB_MODE_BOND9) ? 2 : 0;
-  if ((mode_flags & ~(GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9)) ||
-      (orb != 0) + (rep != 0) > 1 || ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)) ||
+  const bool packed = (mode_flags & GTB_MODE_PACKED) != 0;
+  if ((mode_flags & ~(GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED)) ||
+      (orb != 0) + (rep != 0) + (packed ? 1 : 0) > 1 || ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)) ||
       ((mode_flags & GTB_MODE_BLOCK9) && (mode_flags & GTB_MODE_BOND9)))
     return GTB_ERR_INVALID_ARG;
   if (!phi_cur || !phi_io || !sums || !(a > 0.0) || R <= 0 || R > 64 ||
@@ -964,7 +970,10 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   StepPlan plan;
   const int opt_flags = opt ? opt->flags : 0;
   bool blocked = false;
-  if (rep) {
+  if (packed) {
+    if (!make_plan_packed(H, R, 0, &plan)) return GTB_ERR_INVALID_ARG;
+    blocked = true;
+  } else if (rep) {
     if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
     blocked = true;
   } else if (orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS)) {

@@ -29,13 +29,14 @@ extern "C" const char* gtb_status_string(int status) {
     case GTB_ERR_DIVERGED: return "non-finite Chebyshev moments (spectrum outside [b-a, b+a])";
     case GTB_ERR_CUDA: return "CUDA runtime error";
     case GTB_ERR_INDEX_RANGE: return "too many atoms for int32 indices";
+    case GTB_ERR_NOT_PACKABLE: return "matrix does not fit the packed-row format (width, offsets or distinct values)";
     default: return "unknown status";
   }
 }
 
 extern "C" const char* gtb_last_cuda_error(void) { return gtb::g_cuda_error; }
 
-extern "C" int gtb_version(void) { return 100; }
+extern "C" int gtb_version(void) { return 200; }
 
 extern "C" int64_t gtb_launch_count(void) {
   return gtb::g_launches.load(std::memory_order_relaxed);

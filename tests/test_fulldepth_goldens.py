@@ -12,7 +12,7 @@ from paper_2509_06525_b200 import workloads as W
 from test_gpu_fulldepth import KEYS, _paths, read_fulldepth_golden
 
 
-REQUIRED = ("c4", "c2b", "c2", "c5")        # extended as make_fullsize_goldens.py finishes each config
+REQUIRED = ("c4", "c2b", "c2", "c5", "c3")        # extended as make_fullsize_goldens.py finishes each config
 
 
 def test_goldens_exist():

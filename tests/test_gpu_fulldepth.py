@@ -69,8 +69,12 @@ def _record(key, **kv):
             json.dump(kv, f)
 
 
-@pytest.mark.parametrize("key", [k for k in KEYS if all(os.path.exists(p) for p in _paths(k))])
-def test_full_size_full_depth_moments_and_dos_match_the_oracle(key):
+_HAVE = [k for k in KEYS if all(os.path.exists(p) for p in _paths(k))]
+
+
+@pytest.mark.parametrize("key,packed", [(k, False) for k in _HAVE] + [(k, True) for k in _HAVE if k in ("c4", "c5")])
+def test_full_size_full_depth_moments_and_dos_match_the_oracle(key, packed):
+    """packed: the same run through the packed-row format (gtb_pack_ell, K7x2p) -- what bench.py times at c5."""
     w = W.CONFIGS[key]
     g = read_fulldepth_golden(key)
     assert g["mu"].shape == (w.M,) and g["E"].shape == (w.n_energies,)
@@ -87,7 +91,11 @@ def test_full_size_full_depth_moments_and_dos_match_the_oracle(key):
         assert (a, b) == (w.a, w.b)
     assert np.array_equal(W.energy_grid(w, a, b), g["E"])
     ws = gtb.workspace(gtb.kpm_workspace_bytes(H.n, w.M, w.R))
-    mu = gtb.kpm_moments(H, a, b, w.M, w.R, w.R, w.seed, ws=ws, check=True)
+    Hk, kmode = H, 0
+    if packed:
+        Hk, kmode = gtb.pack_ell(H), gtb.MODE_PACKED
+        assert Hk is not None
+    mu = gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, w.seed, mode=kmode, ws=ws, check=True)
     dmu = float(np.abs(mu.cpu().numpy() - g["mu"]).max())
     E = _dev(g["E"])
     rho = gtb.dos(mu, a, b, E).cpu().numpy()
@@ -96,7 +104,7 @@ def test_full_size_full_depth_moments_and_dos_match_the_oracle(key):
     # K9 in isolation: the oracle's moments through the device DOS
     rho_k9 = gtb.dos(_dev(g["mu"]), a, b, E).cpu().numpy()
     dk9 = float(np.abs(rho_k9 - g["rho"]).max()) / peak
-    _record(key, N=H.n, K=H.width, M=w.M, R=w.R, max_dmu=dmu, max_drho_over_peak=drho, k9_only=dk9)
+    _record(key + ("_packed" if packed else ""), N=H.n, K=H.width, M=w.M, R=w.R, max_dmu=dmu, max_drho_over_peak=drho, k9_only=dk9)
     assert dmu <= 1e-9, dmu                  # north_star
     assert drho <= 1e-8, drho                # north_star
     assert dk9 <= 1e-11, dk9                 # DESIGN.md sec. 3 (Clenshaw vs cos(n acos x))
