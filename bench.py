@@ -504,9 +504,12 @@ def run_vac(args):
     d_pos, d_spec = h_pos.to(dev), h_spec.to(dev)
     d_shift = h_shift.to(dev) if h_shift is not None else None
     h2d = h_pos.numel() * 8 + h_spec.numel() * 4 + (h_shift.numel() * 8 if h_shift is not None else 0)
+    B = ORB_COUNT[ORBITALS]
+    n_rows = B * n                                    # rows of H: orbitals
     ws_build = gtb.workspace(gtb.build_workspace_bytes(n), dev)
-    ws_vac = gtb.workspace(gtb.vac_workspace_bytes(n, w.M, T, w.R), dev)
-    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n), dev)
+    ws_vac = gtb.workspace(gtb.vac_workspace_bytes(n_rows, w.M, T, w.R), dev)
+    ws_bounds = gtb.workspace(gtb.bounds_workspace_bytes(n_rows), dev)
+    vmode = {"sp": gtb.MODE_ORB4, "spd": gtb.MODE_ORB9}.get(ORBITALS, 0)
     Cm = torch.empty((T, w.M), dtype=torch.float64, device=dev)
     h_sigma = torch.empty((T, w.n_energies), dtype=torch.float64).pin_memory()
     state = {}
@@ -517,17 +520,28 @@ def run_vac(args):
     def step(pos, spec, shift):
         H = gtb.build_hamiltonian(pos, spec, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
                                   w.beta, shift, width=width, with_diag=w.use_diag, ws=ws_build)
-        if w.a is None:
+        vpos = pos
+        if ORBITALS != "pz":     # Slater-Koster blocks on the neighbour lists; every orbital sits at its atom
+            ns = len(w.onsite)
+            if ORBITALS == "sp":
+                H = gtb.sk_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
+                                       W.sk_table(ns), r0=1.42, beta=w.beta, onsite_shift=shift)
+            else:
+                H = gtb.spd_hamiltonian(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
+                                        W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42, beta=w.beta,
+                                        onsite_shift=shift)
+            vpos = pos.repeat_interleave(B, dim=0)
+        if w.a is None or ORBITALS != "pz":
             lo, hi = gtb.spectral_bounds(H, ws=ws_bounds).tolist()
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        vv = gtb.velocity_ell(H, pos, inp.box, inp.pbc, 0)
-        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, ws=ws_vac, out=Cm, opt=opt)
+        vv = gtb.velocity_ell(H, vpos, inp.box, inp.pbc, 0)
+        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, mode=vmode, ws=ws_vac, out=Cm, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         _, sigma = gtb.vac_conductivity(Cm, a, b, state["E"], VAC_DT)
-        state["H"] = H
+        state["H"], state["a"], state["b"], state["vv"] = H, a, b, vv
         return sigma
 
     def timed(fn, steps):
@@ -562,21 +576,65 @@ def run_vac(args):
     H = state["H"]
     e2e_step()
     ms_e2e, _, _, _ = timed(e2e_step, args.steps)
-    units = float(n) * w.M * w.R * T * args.steps
-    per_atom = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R) + 16 * w.R
-    bytes_per_launch = float(n) * per_atom
+    gtb.kpm_status(ws_vac)
+    units = float(n_rows) * w.M * w.R * T * args.steps
+    plain = W.algorithmic_bytes_per_atom_pass(H.width, H.diag is not None, w.R)
+    if vmode:    # blocked passes: K/B blocks of (4 B column + 8 B^2 B values) shared by B rows
+        plain = (H.width // B) * (4 + 8 * B * B) // B + (8 if H.diag is not None else 0) + 48 * w.R
+    per_atom = plain + 16 * w.R
+    bytes_per_launch = float(n_rows) * per_atom
     k_ms = loop_ms / max(loop_passes, 1)
     peak, peak_src = _peaks()
     achieved = bytes_per_launch / (k_ms * 1e-3) / 1e9
+    # the other kernels of a time point, timed on their own with CUDA events on the same stream: one
+    # propagation (gtb_evolve: terms - 1 passes with the Chebyshev-Bessel accumulation fused in, + the
+    # first term's accumulation launch + two vector copies of the stand-alone call) and one velocity_apply
+    a_, b_ = state["a"], state["b"]
+    phi = gtb.random_phase_fill(seed, 0, w.R, n_rows, device=dev)
+    ws_ev = gtb.workspace(gtb.evolve_workspace_bytes(n_rows, w.R), dev)
+    terms = gtb.evolve(H, a_, b_, VAC_DT, phi, ws=ws_ev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 5
+    e0.record()
+    for _ in range(reps):
+        gtb.evolve(H, a_, b_, VAC_DT, phi, ws=ws_ev)
+    e1.record()
+    e1.synchronize()
+    ev_ms = e0.elapsed_time(e1) / reps
+    e0.record()
+    for _ in range(reps):
+        y = gtb.velocity_apply(H, state["vv"], phi)
+    e1.record()
+    e1.synchronize()
+    va_ms = e0.elapsed_time(e1) / reps
+    step_ms = ms / args.steps
+    prop_bytes = float(n_rows) * (plain + 32 * w.R)          # + the accumulator read and written
+    va_bytes = float(n_rows) * (12 * H.width + 48 * w.R)     # columns, velocity values, x gathered once, y, bra
+    kernels = [
+        {"kernel": "moment pass (fused Chebyshev pass, dot products against the evolved bra)",
+         "ms_per_launch": k_ms, "launches_per_step": T * (w.M - 1), "GB/s": achieved, "frac": achieved / peak,
+         "share_of_step": k_ms * T * (w.M - 1) / step_ms},
+        {"kernel": "propagation pass (fused Chebyshev pass + Chebyshev-Bessel accumulation; %d terms per U(dt); "
+                   "timed as gtb_evolve / (terms - 1))" % terms,
+         "ms_per_launch": ev_ms / (terms - 1), "launches_per_step": 2 * (T - 1) * (terms - 1),
+         "GB/s": prop_bytes / (ev_ms / (terms - 1) * 1e-3) / 1e9,
+         "frac": prop_bytes / (ev_ms / (terms - 1) * 1e-3) / 1e9 / peak,
+         "share_of_step": 2 * (T - 1) * ev_ms / step_ms},
+        {"kernel": "velocity_apply_kernel (chi_0 = V psi_R with the C_0 dot product)",
+         "ms_per_launch": va_ms, "launches_per_step": T + 1, "GB/s": va_bytes / (va_ms * 1e-3) / 1e9,
+         "frac": va_bytes / (va_ms * 1e-3) / 1e9 / peak, "share_of_step": (T + 1) * va_ms / step_ms},
+    ]
+    accounted = sum(k["share_of_step"] for k in kernels)
     line = {"metric": METRIC, "value": replicas.whole_job_value(units, ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (complex128 vectors)", "data": "synthetic",
-            "config": {"workload": w.name, "quantity": "vac (Eq. 3)", "atoms": n, "ell_width": H.width,
+            "config": {"workload": w.name, "quantity": "vac (Eq. 3)", "atoms": n, "orbitals_per_atom": B,
+                       "ell_width": H.width,
                        "moments": w.M, "vectors": w.R, "time_steps": T, "dt_fs": 0.1,
                        "energies": w.n_energies, "passes_per_step": T * (w.M - 1),
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (
-                           (4 * n * w.R * 16 + 1.67 * H.nbytes()) / 1e9),
+                           (4 * n_rows * w.R * 16 + 1.67 * H.nbytes()) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "seconds_per_conductivity": ms / args.steps * 1e-3,
             "e2e": {"value": replicas.whole_job_value(units, ms_e2e), "unit": UNIT,
@@ -590,10 +648,11 @@ def run_vac(args):
                          "algorithmic_bytes_per_launch": bytes_per_launch,
                          "bytes_per_atom_pass": per_atom, "ms_per_launch": k_ms,
                          "launches_timed": loop_passes,
-                         "share_of_step": k_ms * T * (w.M - 1) * args.steps / ms},
+                         "share_of_step": k_ms * T * (w.M - 1) * args.steps / ms,
+                         "kernels": kernels, "share_accounted": accounted},
             "clocks": clk.summary()}
     if rank == 0:
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and ORBITALS == "pz":
             s, ns = _cpu_sample_vac(w, T)
             t, _ = _oracle_vac_step(s, W.make_inputs(s), ns, VAC_DT)
             line["cpu_baseline"] = {
@@ -638,8 +697,6 @@ def main():
     HOPPING = args.hopping
     if args.hopping == "mlp" and (args.orbitals != "pz" or args.quantity == "vac"):
         raise SystemExit("bench.py: --hopping mlp is wired for --orbitals pz --quantity dos")
-    if args.orbitals != "pz" and args.quantity == "vac":
-        raise SystemExit("bench.py: --orbitals sp/spd is wired for --quantity dos only")
     if args.quantity == "vac" and not args.moments:
         args.moments = 512
     if args.impl == "reference":
