@@ -35,6 +35,8 @@ from paper_2509_06525_b200 import workloads as W  # noqa: E402
 METRIC = "atom-Chebyshev-moment updates/sec (fp64 complex)"
 UNIT = "atom*moment*vector updates/s"
 KERNEL = "auto"                 # set by --kernel: pins the fused-pass kernel through gtb_kpm_options
+STAGES = 0                      # set by --stages: ring depth of the staged passes (0 = the library's default)
+WINDOW = True                   # cleared by --no-window: windowed tiles (gtb_window_ell, K7w) for wide rows
 PACK = True                     # cleared by --no-pack: packed narrow rows (gtb_pack_ell, K7x2p) when the matrix fits
 REP = "scalar"                  # set by --rep (spd only): scalar ELL expansion, stored 9x9 blocks, or bonds (matrix-free)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x clocks.max.sm
@@ -271,7 +273,7 @@ def run_ours(args):
 
     timer = gtb.LoopTimer()
     opt = gtb.options(kernel={"auto": gtb.KERNEL_AUTO, "row": gtb.KERNEL_ROW, "row_x2": gtb.KERNEL_ROW_X2,
-                              "tile": gtb.KERNEL_TILE}[KERNEL], timer=timer)
+                              "tile": gtb.KERNEL_TILE}[KERNEL], tile_stages=STAGES, timer=timer)
 
     def step(pos, spec, shift):
         # the width is a property of (lattice, cutoff) found once above (gtb_neighbor_width): the
@@ -321,6 +323,11 @@ def run_ours(args):
             P = gtb.pack_ell(H, ws=ws_pack)          # part of the timed step; None: does not fit, plain path
             if P is not None:
                 Hk, kmode, state["packed"] = P, gtb.MODE_PACKED, P
+        state["windowed"] = None
+        if WINDOW and KERNEL == "auto" and ORBITALS == "pz" and H.width >= 16 and w.R in (2, 4, 8):   # K = 11: K7t is as fast
+            Wd = gtb.window_ell(H, w.R)              # part of the timed step; None: no locality, K7t stays
+            if Wd is not None:
+                Hk, kmode, state["windowed"] = Wd, gtb.MODE_WINDOW, Wd
         gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
@@ -402,11 +409,14 @@ def run_ours(args):
     vec = w.R in (2, 4, 8)
     tile = KERNEL == "tile" or (KERNEL == "auto" and H.width > 4 and n % 4 == 0 and vec)
     x2 = KERNEL == "row_x2" or (KERNEL == "auto" and H.width <= 4 and vec)
-    if rep9 or packed is not None:
+    windowed = state.get("windowed")
+    if rep9 or packed is not None or windowed is not None:
         small = False
     k7_name = ("cheb_packed_kernel (K7x2p: fused Chebyshev pass on packed rows, 16-bit relative columns + value "
                "dictionary of %d entries, two elements in flight per thread)" % packed.n_values
                if packed is not None else
+               "cheb_window_kernel (K7w: fused Chebyshev pass on windowed tiles, phi_n gathered from shared memory; "
+               "largest window %d blocks)" % windowed.blocks if windowed is not None else
                "cheb_bond9_kernel (K7m: fused Chebyshev pass, 9x9 pair action rebuilt from the bond vector)"
                if rep9 and REP == "bonds" else
                "cheb_block9_kernel (K7bb: fused Chebyshev pass on stored 9x9 blocks [K][81][n])" if rep9 else
@@ -683,13 +693,17 @@ def main():
                    help="pin the fused-pass kernel (gtb_kpm_options.kernel); auto: picked from the matrix shape")
     p.add_argument("--rep", default="bonds", choices=["scalar", "blocks", "bonds"],
                    help="--orbitals spd: scalar ELL expansion (K7b9), stored 9x9 blocks (K7bb) or bonds = matrix-free (K7m)")
+    p.add_argument("--stages", type=int, default=0, help="gtb_kpm_options.tile_stages (K7t, K7w); 0 = default")
+    p.add_argument("--no-window", action="store_true", help="keep wide matrices on the plain ELL path (K7t)")
     p.add_argument("--no-pack", action="store_true", help="keep narrow matrices on the plain ELL path (K7x2)")
     p.add_argument("--cutoff", type=float, default=0.0, help="override the neighbour cutoff in Angstrom "
                    "(3.0 on the pristine lattice = third-nearest neighbours, K = 12: Fig. 4a)")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS, HOPPING, KERNEL, REP, PACK
+    global ORBITALS, HOPPING, KERNEL, REP, PACK, WINDOW, STAGES
+    STAGES = args.stages
+    WINDOW = not args.no_window
     PACK = not args.no_pack
     KERNEL = args.kernel
     REP = args.rep

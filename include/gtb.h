@@ -63,6 +63,7 @@ enum {
 #define GTB_MODE_ORB9 32 /* ... from gtb_spd_hamiltonian (9 orbitals per atom)                           */
 #define GTB_MODE_BLOCK9 64  /* ... H holds the 9x9 blocks written by gtb_spd_blocks (H->n = atoms)          */
 #define GTB_MODE_PACKED 256 /* ... H holds the packed rows and value dictionary written by gtb_pack_ell     */
+#define GTB_MODE_WINDOW 512 /* ... H holds the windowed tiles written by gtb_window_ell (wide rows, K7w)          */
 #define GTB_MODE_BOND9 128  /* ... H holds the bond description written by gtb_spd_bonds (matrix-free)      */
 #define GTB_MAX_SPECIES 8
 #define GTB_MAX_WIDTH 64 /* largest ELL width build_hamiltonian can assemble */
@@ -385,6 +386,22 @@ size_t gtb_pack_workspace_bytes(void);
 size_t gtb_packed_rows_bytes(int64_t n);
 size_t gtb_packed_dict_bytes(void);
 int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_bytes, void* stream, int32_t* n_values);
+
+/* ---- windowed tiles for wide rows (K7w; sliced ELL + 16-bit relative columns) ----
+ * A re-arrangement of an ELL matrix for R_batch = R vectors, tile by tile (256 / (R/2) rows): the distinct
+ * 1 KB blocks of phi rows the tile's columns touch (its window, at most 40), every column as a 16-bit index
+ * into that window, the tile's own slot count (longest row of the tile), and its hoppings / diagonal /
+ * columns contiguous.  The pass (gtb_kpm_moments / gtb_kpm_step with mode | GTB_MODE_WINDOW, R_batch = R,
+ * R_total a multiple of R) copies window and tile into shared memory with bulk copies and gathers from there.
+ *   Wd->n = H->n, Wd->width = H->width, Wd->vals = caller-allocated DEVICE block of
+ *   gtb_window_bytes(n, width, R, H->diag != NULL) bytes (128-byte aligned); on return Wd->cols = H->cols
+ *   (unused), Wd->diag = H->diag (only its presence matters: the values are in the tiles) and Wd->width =
+ *   K + 65536 x (blocks of the largest window), which sizes the shared-memory stage of the pass.
+ * SYNC.  scratch: DEVICE int32.  GTB_ERR_NOT_PACKABLE when some tile's neighbours need more than 40 blocks
+ * (*blocks_needed, HOST, may be NULL, receives the largest count): the numbering has no locality to use. */
+size_t gtb_window_bytes(int64_t n, int32_t width, int32_t R, int32_t with_diag);
+int gtb_window_ell(const gtb_ell* H, int32_t R, gtb_ell* Wd, int32_t* scratch, void* stream,
+                   int32_t* blocks_needed);
 
 /* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
  *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):

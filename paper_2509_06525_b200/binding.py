@@ -36,6 +36,7 @@ EXPORTS = (
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_spd_bonds_bytes", "gtb_spd_bonds",
     "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
     "gtb_pack_workspace_bytes", "gtb_packed_rows_bytes", "gtb_packed_dict_bytes", "gtb_pack_ell",
+    "gtb_window_bytes", "gtb_window_ell",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
@@ -44,6 +45,7 @@ OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT, OPT_SEPARATE_AXPY = 1,
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_BLOCK9 = 64            # ... the block form written by spd_blocks (H.n = atoms)
 MODE_BOND9 = 128            # ... the bond form written by spd_bonds (matrix-free)
+MODE_WINDOW = 512           # ... the windowed tiles written by window_ell (wide rows, for one R)
 MODE_PACKED = 256           # ... the packed rows + value dictionary written by pack_ell (K <= 4)
 MODE_ORB4 = 16              # kpm_moments mode flag: H is gtb_sk_hamiltonian's orbital-blocked matrix
 HBAR_EV_FS = 0.6582119569   # hbar in eV*fs: a time of t fs is t / HBAR_EV_FS in the library's hbar/eV
@@ -661,6 +663,31 @@ def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:
         P.diag = H.diag
     P.n_values = int(nv.value)
     return P
+
+
+def window_ell(H: Ell, R: int) -> Optional[Ell]:
+    """The windowed-tile form of a wide matrix for mode=MODE_WINDOW with R_batch = R (2, 4 or 8).  None when a
+    tile's neighbours are too scattered (GTB_ERR_NOT_PACKABLE): stay on the plain path."""
+    L = lib()
+    L.gtb_window_bytes.restype = C.c_size_t
+    dev = H.vals.device
+    nbytes = int(L.gtb_window_bytes(C.c_int64(H.n), C.c_int32(H.width), C.c_int32(R),
+                                    C.c_int32(int(H.diag is not None))))
+    if nbytes == 0:
+        raise GtbError(ERR_INVALID_ARG, "window_ell", "R must be 2, 4 or 8 and the width at least 1")
+    blob = torch.empty(nbytes // 8, dtype=torch.float64, device=dev)
+    scratch = torch.zeros(1, dtype=torch.int32, device=dev)
+    Wd = Ell(H.n, H.width, H.cols, blob, H.diag)
+    hc, wc = H._c(), Wd._c()
+    need = C.c_int32(0)
+    st = L.gtb_window_ell(C.byref(hc), C.c_int32(R), C.byref(wc), _ptr(scratch), _stream(), C.byref(need))
+    if st == ERR_NOT_PACKABLE:
+        return None
+    _check(st, "window_ell")
+    Wd.width = int(wc.width)         # K + 65536 x blocks of the largest window
+    Wd.R = R
+    Wd.blocks = int(need.value)
+    return Wd
 
 
 # ---------------------------------------------------------------- Fig. 4b post-processing

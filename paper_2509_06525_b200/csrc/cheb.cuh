@@ -25,6 +25,7 @@ struct StepArgs {
   const double* dot_with; // dot_with = L:  (sum Re conj(L) phi_n, sum Re conj(L) phi_{n+1})
   double* axpy_acc;       // propagation passes (plan mode 2): axpy_acc += (axpy_cr + i axpy_ci) * phi_{n+1},
   double axpy_cr, axpy_ci;  // fused into the pass; no dot products are taken
+  int32_t aux;              // K7w: blocks of the largest window (sizes the shared-memory stage)
 };
 
 using StepFn = void (*)(const StepArgs);
@@ -55,6 +56,9 @@ bool make_plan_rep9(const gtb_ell* H, int R, int rep, StepPlan* p);
 
 // packed narrow rows (gtb_pack_ell); mode as make_plan's dot; false when (P, R) does not fit
 bool make_plan_packed(const gtb_ell* P, int R, int mode, StepPlan* p);
+
+// windowed wide rows (gtb_window_ell, built for this R); mode as make_plan's dot
+bool make_plan_window(const gtb_ell* Wd, int R, int mode, int stages, StepPlan* p);
 
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);

@@ -19,6 +19,7 @@
 #include <cmath>
 #include <cstdlib>
 
+#include "tma.cuh"
 #include "vecload.cuh"
 
 namespace gtb {
@@ -285,37 +286,6 @@ StepFn pick_x2(bool diag, int width, int mode) {
 // next tiles' ELL slots (cols, vals, diag) into a ring of shared-memory stages with
 // cp.async.bulk (TMA, completion on an mbarrier) and bulk-prefetches the tiles' phi_{n-1}/phi_n
 // lines into L2, so the consumers' dependent chain is  LDS column -> gather  only.
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        " selp.u32 %0, 1, 0, p;\n}"
-        : "=r"(ok)
-        : "r"(bar), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-      "l"(src), "r"(bytes), "r"(bar)
-      : "memory");
-}
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
-
 constexpr int kBarBytes = 128;  // mbarrier ring at the start of dynamic shared memory
 
 // stage layout (TR rows): vals [width][TR] f64 | diag [TR] f64 | cols [width][TR] i32
@@ -828,13 +798,15 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
   if (rc != GTB_OK) return rc;
   rc = check_options(opt);
   if (rc != GTB_OK) return rc;
-  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED)) ||
+  if ((mode_flags & ~(1 | GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED |
+                     GTB_MODE_WINDOW)) ||
       ((mode_flags & GTB_MODE_ORB4) != 0) + ((mode_flags & GTB_MODE_ORB9) != 0) +
               ((mode_flags & GTB_MODE_BLOCK9) != 0) + ((mode_flags & GTB_MODE_BOND9) != 0) +
-              ((mode_flags & GTB_MODE_PACKED) != 0) > 1)
+              ((mode_flags & GTB_MODE_PACKED) != 0) + ((mode_flags & GTB_MODE_WINDOW) != 0) > 1)
     return GTB_ERR_INVALID_ARG;
   const int32_t mode = mode_flags & 1;
   const bool packed = (mode_flags & GTB_MODE_PACKED) != 0;
+  const bool windowed = (mode_flags & GTB_MODE_WINDOW) != 0;
   const int opt_flags = opt ? opt->flags : 0;
   const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   const int rep = (mode_flags & GTB_MODE_BLOCK9) ? 1 : (mode_flags & GTB_MODE_BOND9) ? 2 : 0;
@@ -861,6 +833,9 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     bool blocked = false;
     if (packed) {  // packed rows: no plain reading exists
       if (!make_plan_packed(H, R, 0, &plan)) return GTB_ERR_INVALID_ARG;
+      blocked = true;
+    } else if (windowed) {  // windowed tiles, built for R_batch vectors: every batch must be full
+      if (R != R_batch || !make_plan_window(H, R, 0, opt ? opt->tile_stages : 0, &plan)) return GTB_ERR_INVALID_ARG;
       blocked = true;
     } else if (rep) {  // block / bond representation: no scalar reading exists
       if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
@@ -893,7 +868,9 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     double* io = w.phi_b;    // phi_{k-1} -> phi_{k+1}
     launch_fill(mode, seed, r0, R, n, cur, st);
     GTB_LAUNCHED();
-    StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, cur, io, 1.0 / a, b, w.partial};
+    StepArgs sa{H->cols, H->vals, H->diag, n, windowed ? (H->width & 0xffff) : H->width, plan.T, cur, io, 1.0 / a, b,
+                w.partial};
+    sa.aux = windowed ? (H->width >> 16) : 0;
     if (small_grid > 0) {  // K7p: K6 and all K7 passes in one launch
       if (last_batch && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
       int S_arg = S;
@@ -954,8 +931,10 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   const int orb = (mode_flags & GTB_MODE_ORB4) ? 4 : (mode_flags & GTB_MODE_ORB9) ? 9 : 0;
   const int rep = (mode_flags & GTB_MODE_BLOCK9) ? 1 : (mode_flags & GTB_MODE_BOND9) ? 2 : 0;
   const bool packed = (mode_flags & GTB_MODE_PACKED) != 0;
-  if ((mode_flags & ~(GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED)) ||
-      (orb != 0) + (rep != 0) + (packed ? 1 : 0) > 1 || ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)) ||
+  const bool windowed = (mode_flags & GTB_MODE_WINDOW) != 0;
+  if ((mode_flags & ~(GTB_MODE_ORB4 | GTB_MODE_ORB9 | GTB_MODE_BLOCK9 | GTB_MODE_BOND9 | GTB_MODE_PACKED |
+                      GTB_MODE_WINDOW)) ||
+      (orb != 0) + (rep != 0) + (packed ? 1 : 0) + (windowed ? 1 : 0) > 1 || ((mode_flags & GTB_MODE_ORB4) && (mode_flags & GTB_MODE_ORB9)) ||
       ((mode_flags & GTB_MODE_BLOCK9) && (mode_flags & GTB_MODE_BOND9)))
     return GTB_ERR_INVALID_ARG;
   if (!phi_cur || !phi_io || !sums || !(a > 0.0) || R <= 0 || R > 64 ||
@@ -973,6 +952,9 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   if (packed) {
     if (!make_plan_packed(H, R, 0, &plan)) return GTB_ERR_INVALID_ARG;
     blocked = true;
+  } else if (windowed) {
+    if (!make_plan_window(H, R, 0, opt ? opt->tile_stages : 0, &plan)) return GTB_ERR_INVALID_ARG;
+    blocked = true;
   } else if (rep) {
     if (!make_plan_rep9(H, R, rep, &plan)) return GTB_ERR_INVALID_ARG;
     blocked = true;
@@ -984,8 +966,9 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
     if (rc != GTB_OK) return rc;
   }
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
-  StepArgs sa{H->cols, H->vals, H->diag, n, H->width, plan.T, phi_cur, phi_io,
+  StepArgs sa{H->cols, H->vals, H->diag, n, windowed ? (H->width & 0xffff) : H->width, plan.T, phi_cur, phi_io,
               (first ? 1.0 : 2.0) / a, b, w.partial};
+  sa.aux = windowed ? (H->width >> 16) : 0;
   launch_step(plan, first != 0, sa, st);
   GTB_LAUNCHED();
   reduce_partials_kernel<<<1, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);

@@ -72,9 +72,10 @@ def _record(key, **kv):
 _HAVE = [k for k in KEYS if all(os.path.exists(p) for p in _paths(k))]
 
 
-@pytest.mark.parametrize("key,packed", [(k, False) for k in _HAVE] + [(k, True) for k in _HAVE if k in ("c4", "c5")])
+@pytest.mark.parametrize("key,packed", [(k, False) for k in _HAVE] + [(k, True) for k in _HAVE if k in ("c4", "c5", "c2", "c3")])
 def test_full_size_full_depth_moments_and_dos_match_the_oracle(key, packed):
-    """packed: the same run through the packed-row format (gtb_pack_ell, K7x2p) -- what bench.py times at c5."""
+    """packed: the same run through the compressed form bench.py times -- packed rows (gtb_pack_ell, K7x2p) at
+    c4 / c5, windowed tiles (gtb_window_ell, K7w) at c2 / c3."""
     w = W.CONFIGS[key]
     g = read_fulldepth_golden(key)
     assert g["mu"].shape == (w.M,) and g["E"].shape == (w.n_energies,)
@@ -92,8 +93,11 @@ def test_full_size_full_depth_moments_and_dos_match_the_oracle(key, packed):
     assert np.array_equal(W.energy_grid(w, a, b), g["E"])
     ws = gtb.workspace(gtb.kpm_workspace_bytes(H.n, w.M, w.R))
     Hk, kmode = H, 0
-    if packed:
+    if packed and H.width <= 4:
         Hk, kmode = gtb.pack_ell(H), gtb.MODE_PACKED
+        assert Hk is not None
+    elif packed:
+        Hk, kmode = gtb.window_ell(H, w.R), gtb.MODE_WINDOW
         assert Hk is not None
     mu = gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, w.seed, mode=kmode, ws=ws, check=True)
     dmu = float(np.abs(mu.cpu().numpy() - g["mu"]).max())
