@@ -298,12 +298,19 @@ __host__ __device__ inline uint32_t tile_stage_bytes(int width, int TR, bool dia
 #endif
 constexpr int kTileBlock = GTB_TILE_BLOCK;  // threads per CTA of K7t
 
+// Warp-specialised: warps 0 .. kTileBlock/32 - 1 consume, one more warp produces; a stage goes round on two
+// mbarriers, full[s] (the copies' bytes) and empty[s] (one arrival per consumer warp), so consumer warps never
+// wait for one another (with a __syncthreads per tile and warp 0 doubling as producer ncu showed 3-4 stall
+// cycles per issue on `barrier`).
+constexpr int kTileCta = kTileBlock + 32;
+constexpr int kTileConsumers = kTileBlock / 32;
+
 template <int LOG2T, bool kFirst, bool kDiag, int CH, int kMode>
-__global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a, const int nstages) {
+__global__ void __launch_bounds__(kTileCta, 3) cheb_tile_kernel(const StepArgs a, const int nstages) {
   constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
-  constexpr int TR = kTileBlock / T;  // rows per tile: one thread per 256-bit element
+  constexpr int TR = kTileBlock / T;  // rows per tile: one consumer thread per 256-bit element
   extern __shared__ __align__(128) unsigned char smem[];
   const int64_t n = a.n;
   const int width = a.width;
@@ -312,48 +319,54 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
   const uint32_t vals_off = 0, diag_off = (uint32_t)width * TR * 8;
   const uint32_t cols_off = diag_off + (kDiag ? TR * 8 : 0);
   const uint32_t bar0 = smem_u32(smem);
+  const uint32_t empty0 = bar0 + 64;   // full[s] at bar0 + 8 s, empty[s] at bar0 + 64 + 8 s (s < 8)
   unsigned char* const stage0 = smem + kBarBytes;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int64_t n_tiles = (n + TR - 1) / TR;
   const int64_t my_tiles = blockIdx.x < n_tiles ? (n_tiles - 1 - blockIdx.x) / gridDim.x + 1 : 0;
 
   if (tid == 0) {
-    for (int s = 0; s < nstages; ++s) mbar_init(bar0 + 8 * s, 1);
+    for (int s = 0; s < nstages; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, kTileConsumers);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
-  // producer: executed by all lanes of warp 0
-  auto issue = [&](int64_t i) {
-    const int s = (int)(i % nstages);
-    const int64_t row0 = (blockIdx.x + i * gridDim.x) * TR;
-    const uint32_t rows = (uint32_t)min((int64_t)TR, n - row0);
-    const uint32_t bar = bar0 + 8 * s;
-    const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
-    if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
-    __syncwarp();
-    for (int j = lane; j < 2 * width + (kDotL || kAxpy ? 4 : 3); j += 32) {
-      if (j < width) {
-        bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
-      } else if (j < 2 * width) {
-        const int k = j - width;
-        bulk_g2s(base + vals_off + (uint32_t)k * TR * 8, a.vals + (size_t)k * n + row0, rows * 8, bar);
-      } else if (j == 2 * width) {
-        if (kDiag) bulk_g2s(base + diag_off, a.diag + row0, rows * 8, bar);
-      } else if (j == 2 * width + 1) {
-        bulk_prefetch_l2(a.phi_cur + row0 * (T * VW), rows * (T * VW * 8));
-      } else if (j == 2 * width + 2) {
-        if (!kFirst) bulk_prefetch_l2(a.phi_io + row0 * (T * VW), rows * (T * VW * 8));
-      } else {
-        if (kDotL) bulk_prefetch_l2(a.dot_with + row0 * (T * VW), rows * (T * VW * 8));
-        if (kAxpy) bulk_prefetch_l2(a.axpy_acc + row0 * (T * VW), rows * (T * VW * 8));
+  double s1 = 0.0, s2 = 0.0;
+  if (wid == kTileConsumers) {   // ---- producer warp, lane-parallel
+    for (int64_t i = 0; i < my_tiles; ++i) {
+      const int s = (int)(i % nstages);
+      if (i >= nstages) mbar_wait(empty0 + 8 * s, (uint32_t)(((i / nstages) - 1) & 1));
+      const int64_t row0 = (blockIdx.x + i * gridDim.x) * TR;
+      const uint32_t rows = (uint32_t)min((int64_t)TR, n - row0);
+      const uint32_t bar = bar0 + 8 * s;
+      const uint32_t base = smem_u32(stage0 + (size_t)s * stage_bytes);
+      if (lane == 0) mbar_expect_tx(bar, rows * (uint32_t)(width * 12 + (kDiag ? 8 : 0)));
+      __syncwarp();
+      for (int j = lane; j < 2 * width + (kDotL || kAxpy ? 4 : 3); j += 32) {
+        if (j < width) {
+          bulk_g2s(base + cols_off + (uint32_t)j * TR * 4, a.cols + (size_t)j * n + row0, rows * 4, bar);
+        } else if (j < 2 * width) {
+          const int k = j - width;
+          bulk_g2s(base + vals_off + (uint32_t)k * TR * 8, a.vals + (size_t)k * n + row0, rows * 8, bar);
+        } else if (j == 2 * width) {
+          if (kDiag) bulk_g2s(base + diag_off, a.diag + row0, rows * 8, bar);
+        } else if (j == 2 * width + 1) {
+          bulk_prefetch_l2(a.phi_cur + row0 * (T * VW), rows * (T * VW * 8));
+        } else if (j == 2 * width + 2) {
+          if (!kFirst) bulk_prefetch_l2(a.phi_io + row0 * (T * VW), rows * (T * VW * 8));
+        } else {
+          if (kDotL) bulk_prefetch_l2(a.dot_with + row0 * (T * VW), rows * (T * VW * 8));
+          if (kAxpy) bulk_prefetch_l2(a.axpy_acc + row0 * (T * VW), rows * (T * VW * 8));
+        }
       }
     }
-  };
-  if (wid == 0)
-    for (int64_t i = 0; i < min((int64_t)nstages, my_tiles); ++i) issue(i);
+    block_store_sums<kTileCta>(s1, s2, a.partial + blockIdx.x);
+    return;
+  }
 
-  double s1 = 0.0, s2 = 0.0;
   const int rl = tid >> LOG2T;             // row within the tile
   const int t = tid & (T - 1);             // 256-bit element within the row
   const double* xt = a.phi_cur + t * VW;
@@ -397,8 +410,8 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
         for (int q = 0; q < VW; ++q) acc.v[q] = fma(d, own.v[q], acc.v[q]);
       }
     }
-    __syncthreads();  // every thread has read stage s: hand it back to the producer
-    if (wid == 0 && i + nstages < my_tiles) issue(i + nstages);
+    __syncwarp();     // this warp has read stage s: one arrival hands its share back to the producer
+    if (lane == 0) mbar_arrive(empty0 + 8 * s);
     if (live) {
       if (kDotL) with = load_stream<VW>(a.dot_with + e * VW);  // prefetched into L2 by the producer
       if (kAxpy) with = load_stream<VW>(a.axpy_acc + e * VW);
@@ -419,22 +432,7 @@ __global__ void __launch_bounds__(kTileBlock) cheb_tile_kernel(const StepArgs a,
       }
     }
   }
-  __shared__ double red[kTileBlock / 32][2];
-  s1 = warp_sum(s1);
-  s2 = warp_sum(s2);
-  if (lane == 0) {
-    red[wid][0] = s1;
-    red[wid][1] = s2;
-  }
-  __syncthreads();
-  if (tid == 0) {
-#pragma unroll
-    for (int w = 1; w < kTileBlock / 32; ++w) {
-      s1 += red[w][0];
-      s2 += red[w][1];
-    }
-    a.partial[blockIdx.x] = make_double2(s1, s2);
-  }
+  block_store_sums<kTileCta>(s1, s2, a.partial + blockIdx.x);
 }
 
 // ---- K7p: all passes of a small system in ONE cooperative launch ----------------------------------
@@ -663,7 +661,9 @@ int make_plan(const gtb_ell* H, int R, int dot, const gtb_kpm_options* opt, Step
                        !(reinterpret_cast<uintptr_t>(H->diag) & 15u);
   if (want == GTB_KERNEL_TILE && !tile_ok) return GTB_ERR_INVALID_ARG;
   int stages = 0;
-  if (tile_ok && (want == GTB_KERNEL_TILE || (want == GTB_KERNEL_AUTO && width > 4)))
+  // wide rows, and narrow rows with a full 128-byte line per gathered neighbour (R = 8: c4 0.93 against K7x2's
+  // 0.88 of the measured peak); at R = 2, 4 narrow rows stay on K7x2 (c5: 2.00 against 2.07 ms)
+  if (tile_ok && (want == GTB_KERNEL_TILE || (want == GTB_KERNEL_AUTO && (width > 4 || R == 8))))
     stages = opt && opt->tile_stages ? opt->tile_stages : 2;
   p->stages = 0;
   if (stages > 0) {
@@ -680,7 +680,7 @@ int make_plan(const gtb_ell* H, int R, int dot, const gtb_kpm_options* opt, Step
     if (smem <= (size_t)max_smem) {
       GTB_CUDA_TRY(cudaFuncSetAttribute(p->tfirst, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       GTB_CUDA_TRY(cudaFuncSetAttribute(p->tnext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kTileBlock, smem));
+      GTB_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kTileCta, smem));
       per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm * kBlock / kTileBlock));
       const int64_t n_tiles = (n + TR - 1) / TR;
       p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, (int64_t)sms * per_sm));
@@ -701,7 +701,7 @@ int make_plan(const gtb_ell* H, int R, int dot, const gtb_kpm_options* opt, Step
 
 void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t st) {
   if (p.stages > 0)
-    (first ? p.tfirst : p.tnext)<<<p.grid, p.block ? p.block : kTileBlock, p.smem, st>>>(sa, p.stages);
+    (first ? p.tfirst : p.tnext)<<<p.grid, p.block ? p.block : kTileCta, p.smem, st>>>(sa, p.stages);
   else
     (first ? p.first : p.next)<<<p.grid, p.block ? p.block : kBlock, p.smem, st>>>(sa);
 }
