@@ -430,6 +430,7 @@ def run_ours(args):
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                 "traffic": _ncu_traffic("dos-packed", w.name) if packed is not None else
+                _ncu_traffic("dos-window", w.name) if windowed is not None else
                 _ncu_traffic("dos" if ORBITALS == "pz" else "dos-" + ORBITALS +
                                         ("" if REP == "scalar" else "-" + REP), w.name)
                 if KERNEL == "auto" else None,
