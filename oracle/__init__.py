@@ -397,6 +397,30 @@ def mlp_sk_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, wei
     return H
 
 
+def spd_block_from_integrals(u, V, Vt=None) -> np.ndarray:
+    """E [9][9] of a pair from its bond direction and ten (scaled) integrals; Vt: those of the reversed pair."""
+    u, V = _f64(u), _f64(V)
+    Vt = V if Vt is None else _f64(Vt)
+    E = np.zeros((9, 9))
+    _check(lib().gtbo_spd_block_from_integrals(_p(u), _p(V), _p(Vt), _p(E)), "spd_block_from_integrals")
+    return E
+
+
+def mlp_spd_hamiltonian(nbr: Ell, pos, species, box, pbc, dims, r_cut: float, weights,
+                        with_diag: bool = True) -> Ell:
+    """Eq. 2 feeding the s,p,d Slater-Koster blocks: scalar ELL over 9n orbitals (blob with 10 / 3 outputs)."""
+    ns, F, Nb, Hd = dims
+    pos, species, box, pbc, w = _f64(pos), _i32(species), _f64(box), _i32(pbc), _f64(weights)
+    n, K = nbr.n, nbr.width
+    H = Ell(9 * n, 9 * K, np.zeros((9 * K, 9 * n), dtype=np.int32), np.zeros((9 * K, 9 * n)),
+            np.zeros(9 * n) if with_diag else None)
+    m = _MlpModel(ns, F, Nb, Hd, r_cut, w.ctypes.data)
+    nc, hc = nbr._c(), H._c()
+    _check(lib().gtbo_mlp_spd_hamiltonian(C.byref(m), C.byref(nc), _p(pos), _p(species), _p(box), _p(pbc),
+                                          C.byref(hc)), "mlp_spd_hamiltonian")
+    return H
+
+
 def carrier_density(rho, energies, e_ref: float) -> np.ndarray:
     """n(E_j) = int_{e_ref}^{E_j} rho dE by the trapezoid rule (reading V7)."""
     rho, energies = _f64(rho), _f64(energies)

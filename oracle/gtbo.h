@@ -194,6 +194,12 @@ int gtbo_spd_step_atoms(const gtbo_ell* nbr, const double* pos, const int32_t* s
                         double a, double b, int32_t first, int32_t R, const int64_t* atoms,
                         int64_t n_rows, const double* x_own, const double* x_nbr, const double* prev,
                         double* out);
+/* bond direction + ten integrals (V for l_a <= l_b, Vt for l_a > l_b) -> E [9][9] row-major */
+int gtbo_spd_block_from_integrals(const double u[3], const double* V, const double* Vt, double* E);
+/* Eq. 2 feeding the s,p,d blocks: MLP_lambda with ten outputs, onsite MLPs with three (gtbo_mlp.cpp). */
+int gtbo_mlp_spd_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* nbr, const double* pos,
+                             const int32_t* species, const double box[3], const int32_t pbc[3],
+                             gtbo_ell* H);
 int gtbo_spd_hamiltonian(const gtbo_ell* nbr, const double* pos, const int32_t* species,
                          const double box[3], const int32_t pbc[3],
                          const gtbo_spd_model* model, gtbo_ell* H);

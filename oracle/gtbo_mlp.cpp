@@ -200,3 +200,69 @@ extern "C" int gtbo_mlp_sk_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* 
   }
   return GTBO_OK;
 }
+
+// Eq. 2 feeding the s,p,d Slater-Koster blocks (reading E7 of DESIGN.md sec. 14): the
+// paper's model.  MLP_lambda has TEN outputs, the two-centre integrals ss_sigma, sp_sigma, pp_sigma, pp_pi,
+// sd_sigma, pd_sigma, pd_pi, dd_sigma, dd_pi, dd_delta of the pair, which enter the block construction of
+// gtbo_spd.cpp; the onsite MLPs have three (eps_s, eps_p, eps_d).  e_ij = e_ji (c is symmetric in the species
+// pair), so the same integrals serve both orderings of the pair.  Weight blob as gtbo_mlp_sk_hamiltonian's
+// with 10 / 3 in place of 4 / 2.  Output: scalar ELL over the 9n orbitals as gtbo_spd_hamiltonian's.
+extern "C" int gtbo_mlp_spd_hamiltonian(const gtbo_mlp_model* m, const gtbo_ell* nbr, const double* pos,
+                                        const int32_t* species, const double box[3],
+                                        const int32_t pbc[3], gtbo_ell* H) {
+  if (!m || !nbr || !pos || !species || !box || !pbc || !H || !H->cols || !H->vals || !m->weights ||
+      H->n != 9 * nbr->n || H->width != 9 * nbr->width || !(m->r_cut > 0.0))
+    return GTBO_ERR_INVALID_ARG;
+  const int ns = m->n_species, F = m->n_features, Nb = m->n_basis, Hd = m->n_hidden;
+  const double* w = m->weights;
+  const double* w_env = w + (size_t)ns * ns * F * Nb;
+  const double* w_hop = w_env + (size_t)Hd * F + Hd + (size_t)F * Hd + F;
+  const size_t hop_size = (size_t)Hd * F + Hd + 10 * (size_t)Hd + 10;
+  const size_t ons_size = (size_t)Hd * F + Hd + 3 * (size_t)Hd + 3;
+  const int64_t n = nbr->n, N = 9 * n;
+  std::vector<double> v((size_t)n * F, 0.0), C(F), u(F), env(F), e(F);
+  for (int64_t i = 0; i < n; ++i)
+    for (int32_t k = 0; k < nbr->width; ++k) {
+      const int64_t j = nbr->cols[(size_t)k * n + i];
+      if (j == i) continue;
+      descriptor(w + ((size_t)species[i] * ns + species[j]) * F * Nb, F, Nb, distance(pos, i, j, box, pbc),
+                 m->r_cut, C.data());
+      for (int q = 0; q < F; ++q) v[(size_t)i * F + q] += C[q];
+    }
+  for (int64_t i = 0; i < n; ++i) {
+    for (int32_t k = 0; k < nbr->width; ++k) {
+      const int64_t j = nbr->cols[(size_t)k * n + i];
+      double E[81] = {0.0};
+      if (j != i) {
+        double d[3];
+        for (int a = 0; a < 3; ++a) {
+          d[a] = pos[3 * j + a] - pos[3 * i + a];
+          if (pbc[a]) d[a] = d[a] - box[a] * std::rint(d[a] / box[a]);
+        }
+        const double r = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
+        const double dir[3] = {d[0] / r, d[1] / r, d[2] / r};
+        descriptor(w + ((size_t)species[i] * ns + species[j]) * F * Nb, F, Nb, r, m->r_cut, C.data());
+        for (int q = 0; q < F; ++q) u[q] = v[(size_t)i * F + q] + v[(size_t)j * F + q];
+        mlp(w_env, F, Hd, F, u.data(), env.data());
+        for (int q = 0; q < F; ++q) e[q] = C[q] * env[q];
+        double V[10];
+        mlp(w_hop, F, Hd, 10, e.data(), V);
+        gtbo_spd_block_from_integrals(dir, V, V, E);
+      }
+      for (int mu = 0; mu < 9; ++mu)
+        for (int nu = 0; nu < 9; ++nu) {
+          const size_t at = (size_t)(9 * k + nu) * N + (9 * i + mu);
+          H->cols[at] = (int32_t)(j != i ? 9 * j + nu : 9 * i + mu);
+          H->vals[at] = j != i ? E[9 * mu + nu] : 0.0;
+        }
+    }
+    if (H->diag) {
+      double eps[3];
+      mlp(w_hop + hop_size + (size_t)species[i] * ons_size, F, Hd, 3, &v[(size_t)i * F], eps);
+      H->diag[9 * i] = eps[0];
+      for (int a = 1; a < 4; ++a) H->diag[9 * i + a] = eps[1];
+      for (int a = 4; a < 9; ++a) H->diag[9 * i + a] = eps[2];
+    }
+  }
+  return GTBO_OK;
+}

@@ -80,6 +80,20 @@ double integral(const double* V, int l, int lp, int m) {
   return am == 0 ? V[7] : (am == 1 ? V[8] : V[9]);   // d-d
 }
 
+// E[a][b] from the bond direction u and the (already scaled) integrals V of (s_i, s_j), Vt of (s_j, s_i)
+void block_from_integrals(const double u[3], const double* V, const double* Vt, double E[kOrb][kOrb]) {
+  double c[kOrb][5];
+  frame_coefficients(u, c);
+  for (int a = 0; a < kOrb; ++a)
+    for (int b = 0; b < kOrb; ++b) {
+      const int la = kL[a], lb = kL[b];
+      const int lo = la < lb ? la : lb, hi = la < lb ? lb : la;
+      double s = 0.0;
+      for (int m = 0; m < 5; ++m) s += c[a][m] * integral(la > lb ? Vt : V, lo, hi, m) * c[b][m];
+      E[a][b] = (la > lb && ((la + lb) & 1)) ? -s : s;
+    }
+}
+
 // the 9x9 hopping block E[a][b] of the pair (i, j), j != i: the construction of the file header
 void pair_block(const double* pos, const double box[3], const int32_t pbc[3], const gtbo_spd_model* model,
                 int64_t i, int64_t j, int si, int sj, double E[kOrb][kOrb]) {
@@ -100,16 +114,7 @@ void pair_block(const double* pos, const double box[3], const int32_t pbc[3], co
     V[q] = model->sk[((size_t)si * ns + sj) * 10 + q] * f;
     Vt[q] = model->sk[((size_t)sj * ns + si) * 10 + q] * f;
   }
-  double c[kOrb][5];
-  frame_coefficients(u, c);
-  for (int a = 0; a < kOrb; ++a)
-    for (int b = 0; b < kOrb; ++b) {
-      const int la = kL[a], lb = kL[b];
-      const int lo = la < lb ? la : lb, hi = la < lb ? lb : la;
-      double s = 0.0;
-      for (int m = 0; m < 5; ++m) s += c[a][m] * integral(la > lb ? Vt : V, lo, hi, m) * c[b][m];
-      E[a][b] = (la > lb && ((la + lb) & 1)) ? -s : s;
-    }
+  block_from_integrals(u, V, Vt, E);
 }
 
 }  // namespace
@@ -197,5 +202,17 @@ extern "C" int gtbo_spd_step_atoms(const gtbo_ell* nbr, const double* pos, const
           out[(((size_t)q * kOrb + mu) * R + r) * 2 + c] = v;
         }
   }
+  return GTBO_OK;
+}
+
+// The step of the construction that turns a bond direction and ten two-centre integrals into the 9x9 block
+// (exported for gtbo_mlp.cpp, where the integrals come from MLP_lambda instead of a species table, and for the
+// tests): E [9][9] row-major; V for l_a <= l_b, Vt for l_a > l_b.
+extern "C" int gtbo_spd_block_from_integrals(const double u[3], const double* V, const double* Vt, double* E) {
+  if (!u || !V || !Vt || !E) return GTBO_ERR_INVALID_ARG;
+  double B[kOrb][kOrb];
+  block_from_integrals(u, V, Vt, B);
+  for (int a = 0; a < kOrb; ++a)
+    for (int b = 0; b < kOrb; ++b) E[a * kOrb + b] = B[a][b];
   return GTBO_OK;
 }

@@ -224,3 +224,70 @@ def test_mlp_sk_parameters_are_the_mlp_outputs_and_the_matrix_is_symmetric():
             assert abs(B[i, 0, j, 0] - Vp[0]) <= 1e-12
             assert np.abs(B[i, 0, j, 1:] - u * Vp[1]).max() <= 1e-12
             assert abs(np.trace(B[i, 1:, j, 1:]) - (Vp[2] + 2 * Vp[3])) <= 1e-12   # tr of the p-p block
+
+
+# ---------------------------------------------------------------------------------- P41
+def test_mlp_spd_with_constant_networks_is_the_spd_oracle():
+    """Eq. 2 feeding the s,p,d blocks (reading E7): MLP_lambda with zero weights and the ten integrals as output
+    bias, onsite MLPs with (eps_s, eps_p, eps_d) as bias, must give gtbo_spd_hamiltonian's matrix (beta = 0)."""
+    w = W.CONFIGS["c4"].scaled(8, 3, stripe=2)
+    inp = W.make_inputs(w)
+    ns = 3
+    nbr = _nbr(w, inp, 2.65)
+    V = np.array([-6.769, 5.580, 5.037, -3.033, -2.1, -1.7, 0.9, -1.3, 0.8, -0.15])
+    es, ep, ed = [-8.9, -6.0, -11.0], [0.0, 2.3, -2.3], [6.5, 7.0, 5.5]
+    c = np.random.default_rng(0).normal(size=(NS, NS, F, NB))
+    c = 0.5 * (c + c.transpose(1, 0, 2, 3))
+    env = (np.zeros((HD, F)), np.zeros(HD), np.zeros((F, HD)), np.ones(F))
+    hop = (np.zeros((HD, F)), np.zeros(HD), np.zeros((10, HD)), V)
+    ons = [(np.zeros((HD, F)), np.zeros(HD), np.zeros((3, HD)), np.array([es[s], ep[s], ed[s]])) for s in range(NS)]
+    H = oracle.mlp_spd_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, DIMS, 3.0,
+                                   W.mlp_pack(c, env, hop, ons))
+    Hs = oracle.spd_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, es, ep, ed,
+                                np.broadcast_to(V, (ns, ns, 10)), beta=0.0)
+    assert (H.cols == Hs.cols).all()
+    assert np.abs(H.vals - Hs.vals).max() <= 1e-15 and np.abs(H.diag - Hs.diag).max() == 0.0
+
+
+def test_mlp_spd_blocks_are_built_from_the_mlp_outputs_and_the_matrix_is_symmetric():
+    """A numpy forward pass gives the ten integrals of sampled pairs; the block must be the spd construction
+    (pinned by P31-P35) of those integrals and the bond direction; H = H^T."""
+    w = W.CONFIGS["c2b"].scaled(5, 4)
+    inp = W.make_inputs(w)
+    blob = W.mlp_weights(DIMS, 11, hop_out=10, onsite_out=3)
+    nbr = _nbr(w, inp, 1.95)
+    H = oracle.mlp_spd_hamiltonian(nbr, inp.pos, inp.species, inp.box, inp.pbc, DIMS, RC, blob)
+    D = H.to_dense()
+    assert np.abs(D - D.T).max() <= 1e-14
+    off = NS * NS * F * NB
+    def take(shape):
+        nonlocal off
+        size = int(np.prod(shape))
+        out = blob[off:off + size].reshape(shape)
+        off += size
+        return out
+    envp = (take((HD, F)), take((HD,)), take((F, HD)), take((F,)))
+    hopp = (take((HD, F)), take((HD,)), take((10, HD)), take((10,)))
+    onsp = [(take((HD, F)), take((HD,)), take((3, HD)), take((3,))) for _ in range(NS)]
+    assert off == blob.size
+    def Cn(i, j):
+        d = inp.pos[j] - inp.pos[i]
+        d -= inp.box * np.rint(d / inp.box) * inp.pbc
+        return oracle.mlp_descriptor(DIMS, RC, blob, 0, 0, float(np.linalg.norm(d))), d / np.linalg.norm(d)
+    v = np.zeros((nbr.n, F))
+    for i in range(nbr.n):
+        for k in range(nbr.width):
+            j = nbr.cols[k, i]
+            if j != i:
+                v[i] += Cn(i, j)[0]
+    B = D.reshape(nbr.n, 9, nbr.n, 9)
+    for i in range(0, nbr.n, 9):
+        eps = _np_mlp(onsp[0], v[i])
+        assert np.abs(np.diag(B[i, :, i, :]) - np.repeat(eps, [1, 3, 5])).max() <= 1e-12
+        for k in range(nbr.width):
+            j = nbr.cols[k, i]
+            if j == i:
+                continue
+            Cij, u = Cn(i, j)
+            Vp = _np_mlp(hopp, Cij * _np_mlp(envp, v[i] + v[j]))
+            assert np.abs(B[i, :, j, :] - oracle.spd_block_from_integrals(u, Vp)).max() <= 1e-12
