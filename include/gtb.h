@@ -416,6 +416,18 @@ int gtb_mlp_sk_hamiltonian(const gtb_mlp_model* m, const gtb_ell* nbr, const dou
                            const int32_t* species, const double box[3], const int32_t pbc[3],
                            gtb_ell* H, double* v, int32_t* status, void* stream);
 
+/* ---- Eq. 2 feeding the s,p,d blocks: the paper's model (reading E7) ----
+ * MLP_lambda has TEN outputs, the two-centre integrals ss_sigma .. dd_delta of the pair, which enter the block
+ * construction of gtb_spd_blocks; the onsite MLPs have three (eps_s, eps_p, eps_d).  e_ij = e_ji, so the same
+ * integrals serve both orderings of a pair.  Weight blob as gtb_mlp_sk_hamiltonian's with 10 / 3 in place of
+ * 4 / 2: gtb_mlp_spd_weight_count() doubles.  (F, Nb, Hd) = (8, 8, 16) only.
+ * ASYNC.  Output in the BLOCK form (GTB_MODE_BLOCK9): Hb->n = atoms, Hb->width = K, Hb->cols = nbr->cols (shared),
+ * Hb->vals = double [K][81][n], Hb->diag = double [9][n] or NULL; v: DEVICE [n][F]. */
+size_t gtb_mlp_spd_weight_count(int32_t n_species, int32_t n_features, int32_t n_basis, int32_t n_hidden);
+int gtb_mlp_spd_blocks(const gtb_mlp_model* m, const gtb_ell* nbr, const double* pos, const int32_t* species,
+                       const double box[3], const int32_t pbc[3], gtb_ell* Hb, double* v, int32_t* status,
+                       void* stream);
+
 /* ---- Fig. 4b post-processing: carrier density and mobility (readings V7, V8) ----
  * ASYNC.  n_out[j] = int_{e_ref}^{E_j} rho(E) dE by the trapezoid rule on the grid (rho interpolated
  * linearly at e_ref; negative below it).  energies strictly ascending, e_ref inside the grid, G >= 2;

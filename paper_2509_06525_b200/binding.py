@@ -36,7 +36,7 @@ EXPORTS = (
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_spd_bonds_bytes", "gtb_spd_bonds",
     "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
     "gtb_pack_workspace_bytes", "gtb_packed_rows_bytes", "gtb_packed_dict_bytes", "gtb_pack_ell",
-    "gtb_window_bytes", "gtb_window_ell",
+    "gtb_window_bytes", "gtb_window_ell", "gtb_mlp_spd_weight_count", "gtb_mlp_spd_blocks",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
@@ -636,6 +636,35 @@ def spd_bounds(H: Ell, mode: int) -> torch.Tensor:
     _check(lib().gtb_spd_bounds(C.byref(hc), C.c_int32(mode), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()),
                                 _stream()), "spd_bounds")
     return out
+
+
+def mlp_spd_blocks(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc, dims, r_cut: float,
+                   weights: torch.Tensor, with_diag: bool = True) -> Ell:
+    """Eq. 2 feeding the s,p,d blocks (ten-output MLP_lambda): the block form for mode=MODE_BLOCK9."""
+    ns, F, Nb, Hd = dims
+    pos = _dev(pos, torch.float64, "pos")
+    species = _dev(species, torch.int32, "species")
+    weights = _dev(weights, torch.float64, "weights")
+    lib().gtb_mlp_spd_weight_count.restype = C.c_size_t
+    need = int(lib().gtb_mlp_spd_weight_count(C.c_int32(ns), C.c_int32(F), C.c_int32(Nb), C.c_int32(Hd)))
+    if weights.numel() != need:
+        raise GtbError(ERR_INVALID_ARG, "mlp_spd_blocks", f"weight blob has {weights.numel()} doubles, {need} expected")
+    box_h = _host_f64(box, 3)
+    pbc_h = np.ascontiguousarray(pbc, dtype=np.int32)
+    n, K, dev = nbr.n, nbr.width, pos.device
+    Hb = Ell(n, K, nbr.cols, torch.empty((max(K, 1), 81, n), dtype=torch.float64, device=dev),
+             torch.empty((9, n), dtype=torch.float64, device=dev) if with_diag else None)
+    v = torch.empty((n, F), dtype=torch.float64, device=dev)
+    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    model = _MlpModel(ns, F, Nb, Hd, r_cut, weights.data_ptr())
+    nc, hc = nbr._c(), Hb._c()
+    st = lib().gtb_mlp_spd_blocks(C.byref(model), C.byref(nc), _ptr(pos), _ptr(species),
+                                  C.c_void_p(box_h.ctypes.data), C.c_void_p(pbc_h.ctypes.data),
+                                  C.byref(hc), _ptr(v), _ptr(status), _stream())
+    _check(st, "mlp_spd_blocks")
+    if int(status.item()) != 0:
+        raise GtbError(ERR_INVALID_ARG, "mlp_spd_blocks", "species index out of range")
+    return Hb
 
 
 def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:

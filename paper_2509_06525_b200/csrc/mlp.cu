@@ -11,6 +11,7 @@
 #include <cmath>
 
 #include "cheb.cuh"
+#include "spd_pair.cuh"
 
 namespace gtb {
 namespace {
@@ -255,6 +256,73 @@ __global__ void __launch_bounds__(kBlock) mlp_sk_onsite_kernel(int64_t n, const 
   }
 }
 
+// ---- Eq. 2 feeding the s,p,d blocks (reading E7): MLP_lambda with ten outputs, onsite MLPs with three --------
+// one thread per (atom, neighbour slot): the pair's ten integrals from the networks, then the closed form of
+// spd_pair.cuh into the block layout of gtb_spd_blocks, blocks[k][9 nu + mu][i]
+template <int F, int NB, int HD>
+__global__ void __launch_bounds__(128) mlp_spd_block_kernel(const int32_t* __restrict__ nbr_cols, int64_t n,
+                                                            int32_t K, const double* __restrict__ pos,
+                                                            const int32_t* __restrict__ species,
+                                                            const MlpGeom g, const double* __restrict__ w,
+                                                            const double* __restrict__ v,
+                                                            double* __restrict__ blocks) {
+  using B10 = Blob<F, NB, HD, 10, 3>;
+  const double* sw = stage_weights<F, NB, HD, 10, 3>(w, g.ns);
+  const int64_t total = n * K;
+  for (int64_t e = (int64_t)blockIdx.x * 128 + threadIdx.x; e < total; e += (int64_t)gridDim.x * 128) {
+    const int64_t k = e / n;
+    const int64_t i = e - k * n;
+    const int64_t j = nbr_cols[e];
+    double E[9][9];
+    if (j == i) {
+      for (int mu = 0; mu < 9; ++mu)
+        for (int nu = 0; nu < 9; ++nu) E[mu][nu] = 0.0;
+    } else {
+      double d[3];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        d[a] = __dsub_rn(pos[j * 3 + a], pos[i * 3 + a]);
+        if (g.pbc[a]) d[a] = __dsub_rn(d[a], __dmul_rn(g.box[a], rint(__ddiv_rn(d[a], g.box[a]))));
+      }
+      const double r = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])),
+                                      __dmul_rn(d[2], d[2])));
+      double C[F], u[F], env[F], V[10], c[kNc];
+      descriptor<F, NB>(B10::c(sw, g.ns, sp(species, i, g.ns), sp(species, j, g.ns)), r, g.r_cut, C);
+#pragma unroll
+      for (int q = 0; q < F; ++q) u[q] = v[i * F + q] + v[j * F + q];
+      mlp<F, HD, F>(B10::env(sw, g.ns), u, env);
+#pragma unroll
+      for (int q = 0; q < F; ++q) u[q] = C[q] * env[q];
+      mlp<F, HD, 10>(B10::hop(sw, g.ns), u, V);
+      pair_coefficients(V, V, c);   // e_ij = e_ji: the same integrals serve both orderings of the pair
+      Geometry geo;
+      geo.l = d[0] / r;
+      geo.m = d[1] / r;
+      geo.n = d[2] / r;
+      geo.f = 1.0;
+      pair_block(geo, c, E);
+    }
+    double* out = blocks + (size_t)k * 81 * n + i;
+    for (int nu = 0; nu < 9; ++nu)
+      for (int mu = 0; mu < 9; ++mu) out[(size_t)(9 * nu + mu) * n] = E[mu][nu];
+  }
+}
+
+template <int F, int NB, int HD>
+__global__ void __launch_bounds__(kBlock) mlp_spd_onsite_kernel(int64_t n, const int32_t* __restrict__ species,
+                                                                const MlpGeom g, const double* __restrict__ w,
+                                                                const double* __restrict__ v,
+                                                                double* __restrict__ onsite) {
+  const double* sw = stage_weights<F, NB, HD, 10, 3>(w, g.ns);
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += (int64_t)gridDim.x * kBlock) {
+    double x[F], y[3];
+#pragma unroll
+    for (int q = 0; q < F; ++q) x[q] = v[i * F + q];
+    mlp<F, HD, 3>(Blob<F, NB, HD, 10, 3>::ons(sw, g.ns, sp(species, i, g.ns)), x, y);
+    for (int mu = 0; mu < 9; ++mu) onsite[(size_t)mu * n + i] = y[mu == 0 ? 0 : (mu < 4 ? 1 : 2)];
+  }
+}
+
 __global__ void species_check_kernel(const int32_t* __restrict__ species, int64_t n, int32_t ns,
                                      int32_t* status) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
@@ -311,6 +379,33 @@ int run_sk(const gtb_mlp_model* m, const gtb_ell* nbr, const double* pos, const 
   }
   if (H->diag) {
     mlp_sk_onsite_kernel<F, NB, HD><<<grid(n), kBlock, smem, st>>>(n, species, g, m->weights, v, H->diag);
+    GTB_LAUNCHED();
+  }
+  return GTB_OK;
+}
+
+template <int F, int NB, int HD>
+int run_spd(const gtb_mlp_model* m, const gtb_ell* nbr, const double* pos, const int32_t* species,
+            const MlpGeom& g, gtb_ell* Hb, double* v, cudaStream_t st) {
+  const size_t smem = sizeof(double) * Blob<F, NB, HD, 10, 3>::size(g.ns);
+  if (smem > 200 * 1024) return GTB_ERR_INVALID_ARG;
+  GTB_CUDA_TRY(cudaFuncSetAttribute(node_feature_kernel<F, NB, HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  GTB_CUDA_TRY(cudaFuncSetAttribute(mlp_spd_block_kernel<F, NB, HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  GTB_CUDA_TRY(cudaFuncSetAttribute(mlp_spd_onsite_kernel<F, NB, HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int64_t n = nbr->n;
+  auto grid = [](int64_t total, int threads) {
+    return (int)std::max<int64_t>(1, std::min<int64_t>((total + threads - 1) / threads, kSmCount * 4));
+  };
+  node_feature_kernel<F, NB, HD><<<grid(n, kBlock), kBlock, smem, st>>>(nbr->cols, n, nbr->width, pos, species, g,
+                                                                        m->weights, v);
+  GTB_LAUNCHED();
+  if (nbr->width > 0) {
+    mlp_spd_block_kernel<F, NB, HD><<<grid(n * nbr->width, 128), 128, smem, st>>>(
+        nbr->cols, n, nbr->width, pos, species, g, m->weights, v, Hb->vals);
+    GTB_LAUNCHED();
+  }
+  if (Hb->diag) {
+    mlp_spd_onsite_kernel<F, NB, HD><<<grid(n, kBlock), kBlock, smem, st>>>(n, species, g, m->weights, v, Hb->diag);
     GTB_LAUNCHED();
   }
   return GTB_OK;
@@ -384,5 +479,39 @@ extern "C" int gtb_mlp_sk_hamiltonian(const gtb_mlp_model* m, const gtb_ell* nbr
   GTB_LAUNCHED();
   if (m->n_features == 8 && m->n_basis == 8 && m->n_hidden == 16)
     return run_sk<8, 8, 16>(m, nbr, pos, species, g, H, v, st);
+  return GTB_ERR_INVALID_ARG;  // (F, Nb, Hd) = (8, 8, 16) is the instantiated size
+}
+
+extern "C" size_t gtb_mlp_spd_weight_count(int32_t ns, int32_t F, int32_t Nb, int32_t Hd) {
+  if (ns <= 0 || F <= 0 || Nb <= 0 || Hd <= 0) return 0;
+  return (size_t)ns * ns * F * Nb + ((size_t)Hd * F + Hd + (size_t)F * Hd + F) +
+         ((size_t)Hd * F + Hd + 10 * (size_t)Hd + 10) + (size_t)ns * ((size_t)Hd * F + Hd + 3 * (size_t)Hd + 3);
+}
+
+extern "C" int gtb_mlp_spd_blocks(const gtb_mlp_model* m, const gtb_ell* nbr, const double* pos,
+                                  const int32_t* species, const double box[3], const int32_t pbc[3],
+                                  gtb_ell* Hb, double* v, int32_t* status, void* stream) {
+  int rc = check_ell(nbr);
+  if (rc != GTB_OK) return rc;
+  if (!m || !pos || !species || !box || !pbc || !Hb || !v || !status || !m->weights || Hb->n != nbr->n ||
+      Hb->width != nbr->width || Hb->cols != nbr->cols || (Hb->width > 0 && !Hb->vals) ||
+      (reinterpret_cast<uintptr_t>(Hb->vals) & 31u) || m->n_species < 1 || m->n_species > GTB_MAX_SPECIES ||
+      !(m->r_cut > 0.0))
+    return GTB_ERR_INVALID_ARG;
+  if (9 * nbr->n > (int64_t)INT32_MAX - 64) return GTB_ERR_INDEX_RANGE;
+  MlpGeom g{};
+  for (int a = 0; a < 3; ++a) {
+    if (pbc[a] && !(box[a] > 0.0)) return GTB_ERR_INVALID_ARG;
+    g.box[a] = box[a];
+    g.pbc[a] = pbc[a];
+  }
+  g.r_cut = m->r_cut;
+  g.ns = m->n_species;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  GTB_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int32_t), st));
+  species_check_kernel<<<kSmCount, 256, 0, st>>>(species, nbr->n, g.ns, status);
+  GTB_LAUNCHED();
+  if (m->n_features == 8 && m->n_basis == 8 && m->n_hidden == 16)
+    return run_spd<8, 8, 16>(m, nbr, pos, species, g, Hb, v, st);
   return GTB_ERR_INVALID_ARG;  // (F, Nb, Hd) = (8, 8, 16) is the instantiated size
 }

@@ -110,3 +110,39 @@ def test_mlp_feeding_the_slater_koster_blocks(key, nx, ny, cutoff, kw):
     ref = oracle.kpm_moments(Ho, a, b, 48, 4, 3, mode=0, algo=0)
     got = gtb.kpm_moments(Hg, a, b, 48, 4, 4, 3, mode=gtb.MODE_ORB4, check=True).cpu().numpy()
     assert np.abs(got - ref).max() <= 1e-9 and np.abs(got - ref).max() <= 1e-11
+
+
+# ---- Eq. 2 feeding the s,p,d blocks (ten-output MLP_lambda, reading E7): blocks and blocked moments ----------
+@pytest.mark.parametrize("key,nx,ny,kw,cutoff", [("c2b", 9, 7, {}, 2.65), ("c4", 12, 5, {"stripe": 3}, 1.95),
+                                                 ("c5", 11, 9, {}, 3.0)])
+def test_mlp_spd_blocks_and_moments_match_the_oracle(key, nx, ny, kw, cutoff):
+    import numpy as np, torch
+    w = W.CONFIGS[key].scaled(nx, ny, **kw)
+    inp = W.make_inputs(w)
+    ns = len(w.onsite)
+    dims = (3, 8, 8, 16)
+    blob = W.mlp_weights(dims, 23, hop_out=10, onsite_out=3)
+    r_cut = max(2.0, 1.05 * cutoff)
+    ones = np.ones((ns, ns))
+    nbr_o = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, cutoff, [0.0] * ns, ones,
+                                     with_diag=False)
+    Ho = oracle.mlp_spd_hamiltonian(nbr_o, inp.pos, inp.species, inp.box, inp.pbc, dims, r_cut, blob)
+    dev = lambda x: torch.as_tensor(np.ascontiguousarray(x)).cuda()
+    nbr_g = gtb.build_hamiltonian(dev(inp.pos), dev(inp.species), inp.box, inp.pbc, cutoff, [0.0] * ns, ones,
+                                  with_diag=False)
+    Hb = gtb.mlp_spd_blocks(nbr_g, dev(inp.pos), dev(inp.species), inp.box, inp.pbc, dims, r_cut, dev(blob))
+    n, K = nbr_o.n, nbr_o.width
+    got = Hb.vals.cpu().numpy().reshape(K, 9, 9, n)                      # [k][nu][mu][i]
+    want = Ho.vals.reshape(K, 9, n, 9).transpose(0, 1, 3, 2)
+    scale = max(np.abs(want).max(), 1.0)
+    assert np.abs(got - want).max() <= 1e-12 * scale
+    assert np.abs(Hb.diag.cpu().numpy() - Ho.diag.reshape(n, 9).T).max() <= 1e-12 * scale
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    bounds = gtb.spd_bounds(Hb, gtb.MODE_BLOCK9).cpu().numpy()
+    assert bounds[0] == pytest.approx(lo, rel=1e-11) and bounds[1] == pytest.approx(hi, rel=1e-11)
+    for R in (2, 8):
+        ref = oracle.kpm_moments(Ho, a, b, 33, R, 5, mode=0, algo=0)
+        mu = gtb.kpm_moments(Hb, a, b, 33, R, R, 5, mode=gtb.MODE_BLOCK9, check=True).cpu().numpy()
+        assert np.abs(mu - ref).max() <= 1e-9
+        assert np.abs(mu - ref).max() <= 1e-11
