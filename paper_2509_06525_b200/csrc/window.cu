@@ -259,29 +259,20 @@ __global__ void __launch_bounds__(kWinCtaThreads, 2) cheb_window_kernel(const St
   const int t = tid & (T - 1);
   const bool odd = (rl & 1) != 0;
   const uint32_t first_half = odd ? 16u : 0u, second_half = odd ? 0u : 16u;
-  // the thread's own elements of phi_{n-1} and phi_n are loaded one tile AHEAD (before the gather loop of the
-  // current tile), so their L2 latency is covered by that loop instead of stalling in front of the barrier
-  Vec<VW> prev_next, own_next;
-  auto load_own = [&](int64_t i) {
-#pragma unroll
-    for (int q = 0; q < VW; ++q) prev_next.v[q] = own_next.v[q] = 0.0;
-    const int64_t row = (blockIdx.x + i * gridDim.x) * TR + rl;
-    if (i < my_tiles && row < n) {
-      const int64_t e = row * T + t;
-      if (!kFirst) prev_next = load_stream<VW>(a.phi_io + e * VW);
-      own_next = load_gather<VW>(a.phi_cur + e * VW);
-    }
-  };
-  load_own(0);
+  // (loading the thread's own phi_{n-1} / phi_n elements one tile ahead was measured: no gain for K7w, and K7t
+  // loses a third at its 72-register cap)
   for (int64_t i = 0; i < my_tiles; ++i) {
     const int s = (int)(i % nstages);
     const int64_t row = (blockIdx.x + i * gridDim.x) * TR + rl;
     const bool live = row < n;
     const int64_t e = row * T + t;
-    Vec<VW> prev = prev_next, own = own_next, acc, with;
+    Vec<VW> prev, own, acc, with;
 #pragma unroll
-    for (int q = 0; q < VW; ++q) acc.v[q] = with.v[q] = 0.0;
-    load_own(i + 1);
+    for (int q = 0; q < VW; ++q) acc.v[q] = prev.v[q] = own.v[q] = with.v[q] = 0.0;
+    if (live) {
+      if (!kFirst) prev = load_stream<VW>(a.phi_io + e * VW);
+      own = load_gather<VW>(a.phi_cur + e * VW);
+    }
     mbar_wait(bar0 + 8 * s, (uint32_t)((i / nstages) & 1));
     const unsigned char* st = stage0 + (size_t)s * stage_bytes;
     const int kt = reinterpret_cast<const int32_t*>(st)[1];
