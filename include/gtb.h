@@ -428,6 +428,26 @@ int gtb_mlp_spd_blocks(const gtb_mlp_model* m, const gtb_ell* nbr, const double*
                        const double box[3], const int32_t pbc[3], gtb_ell* Hb, double* v, int32_t* status,
                        void* stream);
 
+/* ---- 1-D strip decomposition with one halo exchange per pass, on one device ----
+ * The rows are cut into n_strips contiguous strips (multiples of 4 rows, the last takes the rest); a strip owns
+ * its rows of the vectors plus a lo and a hi halo of `halo` rows each -- the rows of its ring neighbours that its
+ * columns reach -- and runs the fused pass on its own column-localised copy of H.  Per pass: one contiguous
+ * copy per strip and side from the neighbour's owned rows (the exchange step; a peer copy on several GPUs),
+ * then the pass on every strip; block sums are reduced strip after strip in a fixed order.  Same vectors bit
+ * for bit as gtb_kpm_moments, moments equal up to the order of the block sums.  Unmeasured on more than one GPU.
+ * gtb_strip_plan: HOST only; out = { row0, rows, lo_first, hi_first, lo_owner, hi_owner } of strip p (lo_first /
+ * hi_first: global index of the first halo row on the ring); GTB_ERR_INVALID_ARG when a strip is narrower than
+ * the halo.  gtb_ring_halo: SYNC, *halo = largest ring distance min(|col - row|, n - |col - row|) in H.
+ * gtb_kpm_moments_strips: ASYNC; mode 0 / 1 as gtb_kpm_moments; phi_out (DEVICE [n][R_batch][2] or NULL)
+ * receives the last Chebyshev vector of the last batch gathered from the strips. */
+int gtb_strip_plan(int64_t n, int32_t n_strips, int64_t halo, int32_t p, int64_t out[6]);
+int gtb_ring_halo(const gtb_ell* H, int32_t* scratch, void* stream, int64_t* halo);
+size_t gtb_strips_workspace_bytes(int64_t n, int32_t width, int32_t with_diag, int32_t n_strips, int64_t halo,
+                                  int32_t M, int32_t R_batch);
+int gtb_kpm_moments_strips(const gtb_ell* H, int32_t n_strips, int64_t halo, double a, double b, int32_t M,
+                           int32_t R_total, int32_t R_batch, uint64_t seed, int32_t mode, double* mu,
+                           double* phi_out, void* ws, size_t ws_bytes, void* stream, const gtb_kpm_options* opt);
+
 /* ---- Fig. 4b post-processing: carrier density and mobility (readings V7, V8) ----
  * ASYNC.  n_out[j] = int_{e_ref}^{E_j} rho(E) dE by the trapezoid rule on the grid (rho interpolated
  * linearly at e_ref; negative below it).  energies strictly ascending, e_ref inside the grid, G >= 2;

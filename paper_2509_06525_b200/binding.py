@@ -37,6 +37,7 @@ EXPORTS = (
     "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
     "gtb_pack_workspace_bytes", "gtb_packed_rows_bytes", "gtb_packed_dict_bytes", "gtb_pack_ell",
     "gtb_window_bytes", "gtb_window_ell", "gtb_mlp_spd_weight_count", "gtb_mlp_spd_blocks",
+    "gtb_strip_plan", "gtb_ring_halo", "gtb_strips_workspace_bytes", "gtb_kpm_moments_strips",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
 
@@ -665,6 +666,50 @@ def mlp_spd_blocks(nbr: Ell, pos: torch.Tensor, species: torch.Tensor, box, pbc,
     if int(status.item()) != 0:
         raise GtbError(ERR_INVALID_ARG, "mlp_spd_blocks", "species index out of range")
     return Hb
+
+
+def strip_plan(n: int, n_strips: int, halo: int, p: int) -> dict:
+    """Host-only: the rows strip p owns and where its two halos come from (include/gtb.h)."""
+    out = (C.c_int64 * 6)()
+    _check(lib().gtb_strip_plan(C.c_int64(n), C.c_int32(n_strips), C.c_int64(halo), C.c_int32(p), out), "strip_plan")
+    return dict(zip(("row0", "rows", "lo_first", "hi_first", "lo_owner", "hi_owner"), (int(x) for x in out)))
+
+
+def ring_halo(H: Ell) -> int:
+    scratch = torch.zeros(1, dtype=torch.int32, device=H.vals.device)
+    h = C.c_int64(0)
+    hc = H._c()
+    _check(lib().gtb_ring_halo(C.byref(hc), _ptr(scratch), _stream(), C.byref(h)), "ring_halo")
+    return int(h.value)
+
+
+def kpm_moments_strips(H: Ell, n_strips: int, a: float, b: float, M: int, R_total: int = 1,
+                       R_batch: Optional[int] = None, seed: int = 0, mode: int = 0, halo: Optional[int] = None,
+                       want_phi: bool = False, check: bool = False, opt: Optional[_Options] = None):
+    """gtb_kpm_moments on n_strips row strips with one halo exchange per pass; (mu, phi_last or None)."""
+    dev = H.vals.device
+    if R_batch is None:
+        R_batch = R_total if mode == 0 else 8
+    if halo is None:
+        halo = ring_halo(H)
+    L = lib()
+    L.gtb_strips_workspace_bytes.restype = C.c_size_t
+    need = int(L.gtb_strips_workspace_bytes(C.c_int64(H.n), C.c_int32(H.width), C.c_int32(int(H.diag is not None)),
+                                            C.c_int32(n_strips), C.c_int64(halo), C.c_int32(M), C.c_int32(R_batch)))
+    if need == 0:
+        raise GtbError(ERR_INVALID_ARG, "kpm_moments_strips", "a strip is narrower than the halo")
+    ws = workspace(need, dev)
+    mu = torch.empty(M, dtype=torch.float64, device=dev)
+    phi = torch.empty((H.n, R_batch, 2), dtype=torch.float64, device=dev) if want_phi else None
+    hc = H._c()
+    st = L.gtb_kpm_moments_strips(C.byref(hc), C.c_int32(n_strips), C.c_int64(halo), C.c_double(a), C.c_double(b),
+                                  C.c_int32(M), C.c_int32(R_total), C.c_int32(R_batch),
+                                  C.c_uint64(seed & (2**64 - 1)), C.c_int32(mode), _ptr(mu), _ptr(phi), _ptr(ws),
+                                  C.c_size_t(ws.numel()), _stream(), _opt(opt))
+    _check(st, "kpm_moments_strips")
+    if check:
+        kpm_status(ws)
+    return mu, phi
 
 
 def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:

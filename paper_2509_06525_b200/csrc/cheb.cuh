@@ -63,7 +63,11 @@ bool make_plan_window(const gtb_ell* Wd, int R, int mode, int stages, StepPlan* 
 int check_ell(const gtb_ell* H);
 int check_ws(const void* ws, size_t ws_bytes, size_t need);
 // mode 0: random phases of (seed, r0..r0+R-1); mode 1: basis vectors e_{r0}..e_{r0+R-1}
-void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st);
+// row_offset: global index of the first row written (a strip of the vectors)
+void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st,
+                 int64_t row_offset = 0);
+// mu[n] from the pass sums by the doubling identities (K8b); status: the non-finite flag
+void launch_finish_moments(const double2* sums, int M, double norm, double* mu, int32_t* status, cudaStream_t st);
 // sums[s] += sum_{k<grid} partial[s*stride + k]   for s = 0..nslots-1, fixed order
 void launch_reduce_partials(const double2* partial, int stride, int grid, double2* sums, int nslots,
                             cudaStream_t st);

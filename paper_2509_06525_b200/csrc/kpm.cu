@@ -36,14 +36,15 @@ __host__ __device__ __forceinline__ uint64_t mix64(uint64_t z) {
 
 // K5: phi[i][k] = exp(i theta), theta = fl(2 pi u(seed, r0 + k, i))
 __global__ void __launch_bounds__(kBlock) random_phase_kernel(uint64_t seed, int32_t r0, int32_t R,
-                                                              int64_t n, double2* __restrict__ phi) {
+                                                              int64_t n, double2* __restrict__ phi,
+                                                              int64_t row_offset = 0) {
   const int64_t total = n * R;
   for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
        e += (int64_t)gridDim.x * kBlock) {
     const int64_t i = e / R;
     const int32_t k = (int32_t)(e - i * R);
     const uint64_t key = mix64(seed + ((uint64_t)(uint32_t)(r0 + k) + 1ull) * kGamma);
-    const uint64_t h = mix64(key + ((uint64_t)i + 1ull) * kGamma);
+    const uint64_t h = mix64(key + ((uint64_t)(i + row_offset) + 1ull) * kGamma);   // row_offset: a strip's first row
     const double u = (double)(h >> 11) * 0x1.0p-53;
     const double theta = 6.283185307179586 * u;
     double s, c;
@@ -54,13 +55,13 @@ __global__ void __launch_bounds__(kBlock) random_phase_kernel(uint64_t seed, int
 
 // exact-trace mode: phi[i][k] = delta(i, r0 + k)   (basis vectors e_{r0} .. e_{r0+R-1})
 __global__ void __launch_bounds__(kBlock) basis_fill_kernel(int64_t r0, int32_t R, int64_t n,
-                                                            double2* __restrict__ phi) {
+                                                            double2* __restrict__ phi, int64_t row_offset = 0) {
   const int64_t total = n * R;
   for (int64_t e = (int64_t)blockIdx.x * kBlock + threadIdx.x; e < total;
        e += (int64_t)gridDim.x * kBlock) {
     const int64_t i = e / R;
     const int64_t k = e - i * R;
-    phi[e] = make_double2(i == r0 + k ? 1.0 : 0.0, 0.0);
+    phi[e] = make_double2(i + row_offset == r0 + k ? 1.0 : 0.0, 0.0);
   }
 }
 
@@ -708,12 +709,17 @@ void launch_step(const StepPlan& p, bool first, const StepArgs& sa, cudaStream_t
     (first ? p.first : p.next)<<<p.grid, p.block ? p.block : kBlock, p.smem, st>>>(sa);
 }
 
-void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st) {
+void launch_fill(int mode, uint64_t seed, int64_t r0, int R, int64_t n, double* phi, cudaStream_t st,
+                 int64_t row_offset) {
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n * R + kBlock - 1) / kBlock, kMaxGrid));
   if (mode == 0)
-    random_phase_kernel<<<grid, kBlock, 0, st>>>(seed, (int32_t)r0, R, n, reinterpret_cast<double2*>(phi));
+    random_phase_kernel<<<grid, kBlock, 0, st>>>(seed, (int32_t)r0, R, n, reinterpret_cast<double2*>(phi), row_offset);
   else
-    basis_fill_kernel<<<grid, kBlock, 0, st>>>(r0, R, n, reinterpret_cast<double2*>(phi));
+    basis_fill_kernel<<<grid, kBlock, 0, st>>>(r0, R, n, reinterpret_cast<double2*>(phi), row_offset);
+}
+
+void launch_finish_moments(const double2* sums, int M, double norm, double* mu, int32_t* status, cudaStream_t st) {
+  finish_moments_kernel<<<(M + kBlock - 1) / kBlock, kBlock, 0, st>>>(sums, M, norm, mu, status);
 }
 
 void launch_reduce_partials(const double2* partial, int stride, int grid, double2* sums, int nslots,
