@@ -549,7 +549,17 @@ def run_vac(args):
         else:
             a, b = w.a, w.b
         vv = gtb.velocity_ell(H, vpos, inp.box, inp.pbc, 0)
-        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, mode=vmode, ws=ws_vac, out=Cm, opt=opt)
+        vopt, state["alt"] = opt, None
+        if ORBITALS == "pz" and w.R in (2, 4, 8):   # the fused passes on the compressed form, as the DOS path
+            alt = None
+            if PACK and H.width <= 4 and w.R in (2, 4):
+                alt, amode, aname = gtb.pack_ell(H), gtb.MODE_PACKED, "packed rows (K7x2p)"
+            elif WINDOW and H.width >= 16:
+                alt, amode, aname = gtb.window_ell(H, w.R), gtb.MODE_WINDOW, "windowed tiles (K7w)"
+            if alt is not None:
+                vopt = gtb.options(timer=timer, alt=alt, alt_mode=amode)
+                state["alt"] = aname
+        gtb.vac_moments(H, vv, a, b, w.M, T, VAC_DT, w.R, w.R, seed, mode=vmode, ws=ws_vac, out=Cm, opt=vopt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
         _, sigma = gtb.vac_conductivity(Cm, a, b, state["E"], VAC_DT)
@@ -643,6 +653,7 @@ def run_vac(args):
             "vs_baseline": None, "dtype": "f64 (complex128 vectors)", "data": "synthetic",
             "config": {"workload": w.name, "quantity": "vac (Eq. 3)", "atoms": n, "orbitals_per_atom": B,
                        "ell_width": H.width,
+                       "fused_passes_on": state.get("alt") or "plain ELL",
                        "moments": w.M, "vectors": w.R, "time_steps": T, "dt_fs": 0.1,
                        "energies": w.n_energies, "passes_per_step": T * (w.M - 1),
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (

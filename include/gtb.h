@@ -115,6 +115,12 @@ typedef struct gtb_kpm_options {
   void* loop_begin;
   void* loop_end;
   int32_t* loop_passes;
+  /* gtb_vac_moments only: a compressed form of the SAME matrix (from gtb_pack_ell or gtb_window_ell built for
+   * R_batch) on which the moment passes (packed rows: and the propagation passes) run; the velocity operator
+   * keeps reading H.  NULL: none.
+   * alt_mode = GTB_MODE_PACKED or GTB_MODE_WINDOW. */
+  const struct gtb_ell* alt;
+  int32_t alt_mode;
 } gtb_kpm_options;
 
 /* ---- status -------------------------------------------------------------- */
@@ -396,7 +402,8 @@ int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_bytes, void* 
  *   Wd->n = H->n, Wd->width = H->width, Wd->vals = caller-allocated DEVICE block of
  *   gtb_window_bytes(n, width, R, H->diag != NULL) bytes (128-byte aligned); on return Wd->cols = H->cols
  *   (unused), Wd->diag = H->diag (only its presence matters: the values are in the tiles) and Wd->width =
- *   K + 65536 x (blocks of the largest window), which sizes the shared-memory stage of the pass.
+ *   K | (blocks of the largest window) << 16 | R << 24: the window sizes the shared-memory stage of the pass,
+ *   and a pass asked for another R_batch than the tiles were built for is GTB_ERR_INVALID_ARG.
  * SYNC.  scratch: DEVICE int32.  GTB_ERR_NOT_PACKABLE when some tile's neighbours need more than 40 blocks
  * (*blocks_needed, HOST, may be NULL, receives the largest count): the numbering has no locality to use. */
 size_t gtb_window_bytes(int64_t n, int32_t width, int32_t R, int32_t with_diag);

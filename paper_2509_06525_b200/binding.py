@@ -74,7 +74,7 @@ class _Ell(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("tile_stages", C.c_int32), ("flags", C.c_int32),
                 ("loop_begin", C.c_void_p), ("loop_end", C.c_void_p),
-                ("loop_passes", C.POINTER(C.c_int32))]
+                ("loop_passes", C.POINTER(C.c_int32)), ("alt", C.c_void_p), ("alt_mode", C.c_int32)]
 
 
 class LoopTimer:
@@ -95,9 +95,15 @@ class LoopTimer:
 
 
 def options(kernel: int = KERNEL_AUTO, tile_stages: int = 0, flags: int = 0,
-            timer: Optional[LoopTimer] = None) -> _Options:
-    """A gtb_kpm_options value (argument marshalling only)."""
-    o = _Options(kernel, tile_stages, flags, None, None, None)
+            timer: Optional[LoopTimer] = None, alt=None, alt_mode: int = 0) -> _Options:
+    """A gtb_kpm_options value (argument marshalling only).  alt: an Ell from pack_ell / window_ell of the same
+    matrix for vac_moments' fused passes (alt_mode MODE_PACKED / MODE_WINDOW)."""
+    o = _Options(kernel, tile_stages, flags, None, None, None, None, 0)
+    if alt is not None:
+        o._alt_c = alt._c()              # keep the struct (and through `alt` the tensors) alive
+        o._alt = alt
+        o.alt = C.addressof(o._alt_c)
+        o.alt_mode = alt_mode
     if timer is not None:
         o.loop_begin = timer.begin.cuda_event
         o.loop_end = timer.end.cuda_event

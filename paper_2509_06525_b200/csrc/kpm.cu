@@ -745,7 +745,8 @@ int check_options(const gtb_kpm_options* opt) {
       opt->tile_stages > 8 ||
       (opt->flags & ~(GTB_OPT_PER_PASS_LAUNCH | GTB_OPT_SCALAR_BLOCKS | GTB_OPT_BLOCK_DIRECT |
                       GTB_OPT_SEPARATE_AXPY)) ||
-      ((opt->loop_begin == nullptr) != (opt->loop_end == nullptr)))
+      ((opt->loop_begin == nullptr) != (opt->loop_end == nullptr)) ||
+      (opt->alt && opt->alt_mode != GTB_MODE_PACKED && opt->alt_mode != GTB_MODE_WINDOW))
     return GTB_ERR_INVALID_ARG;
   return GTB_OK;
 }
@@ -878,7 +879,7 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     GTB_LAUNCHED();
     StepArgs sa{H->cols, H->vals, H->diag, n, windowed ? (H->width & 0xffff) : H->width, plan.T, cur, io, 1.0 / a, b,
                 w.partial};
-    sa.aux = windowed ? (H->width >> 16) : 0;
+    sa.aux = windowed ? ((H->width >> 16) & 0xff) : 0;
     if (small_grid > 0) {  // K7p: K6 and all K7 passes in one launch
       if (last_batch && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
       int S_arg = S;
@@ -976,7 +977,7 @@ extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first,
   GTB_CUDA_TRY(cudaMemsetAsync(w.sums, 0, sizeof(double2), st));
   StepArgs sa{H->cols, H->vals, H->diag, n, windowed ? (H->width & 0xffff) : H->width, plan.T, phi_cur, phi_io,
               (first ? 1.0 : 2.0) / a, b, w.partial};
-  sa.aux = windowed ? (H->width >> 16) : 0;
+  sa.aux = windowed ? ((H->width >> 16) & 0xff) : 0;
   launch_step(plan, first != 0, sa, st);
   GTB_LAUNCHED();
   reduce_partials_kernel<<<1, 128, 0, st>>>(w.partial, kMaxGrid, plan.grid, w.sums);

@@ -145,7 +145,7 @@ std::vector<double2> bessel_coefficients(double a, double b, double dt) {
 // state <- U(dt) state.  Buffers: *state (in), *s1, *s2 scratch; on return *state points at the
 // result and *s1, *s2 at the two free buffers.  fused: `plan` is a mode-2 plan (make_plan(..., 2, ...)):
 // the accumulation acc += c_m t_m runs inside the pass that produces t_m; else one caxpy launch per term.
-int evolve_in_place(const gtb_ell* H, const StepPlan& plan, bool fused, double a, double b,
+int evolve_in_place(const gtb_ell* H, int32_t aux, const StepPlan& plan, bool fused, double a, double b,
                     const std::vector<double2>& c, int R, double** state, double** s1, double** s2,
                     double2* scratch_partial, cudaStream_t st) {
   const int64_t total = H->n * R;
@@ -156,8 +156,10 @@ int evolve_in_place(const gtb_ell* H, const StepPlan& plan, bool fused, double a
   caxpy_kernel<<<g, kBlock, 0, st>>>(total, c[0].x, c[0].y, reinterpret_cast<const double2*>(x),
                                      reinterpret_cast<double2*>(acc), 1);
   GTB_LAUNCHED();
-  StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width, plan.T, x, t, 1.0 / a, b, scratch_partial,
+  // H: the matrix of the passes (plain, or the packed / windowed form of it: aux = blocks of the largest window)
+  StepArgs sa{H->cols, H->vals, H->diag, H->n, H->width & 0xffff, plan.T, x, t, 1.0 / a, b, scratch_partial,
               nullptr};
+  sa.aux = aux;
   double* cur = x;
   double* io = t;
   for (size_t m = 1; m < c.size(); ++m) {
@@ -255,7 +257,7 @@ extern "C" int gtb_evolve(const gtb_ell* H, double a, double b, double dt, int32
   const size_t bytes = sizeof(double) * (size_t)H->n * R * 2;
   double *state = w.buf[0], *s1 = w.buf[1], *s2 = w.buf[2];
   GTB_CUDA_TRY(cudaMemcpyAsync(state, phi, bytes, cudaMemcpyDeviceToDevice, st));
-  rc = evolve_in_place(H, plan, true, a, b, c, R, &state, &s1, &s2, w.partial, st);
+  rc = evolve_in_place(H, 0, plan, true, a, b, c, R, &state, &s1, &s2, w.partial, st);
   if (rc != GTB_OK) return rc;
   GTB_CUDA_TRY(cudaMemcpyAsync(phi, state, bytes, cudaMemcpyDeviceToDevice, st));
   return GTB_OK;
@@ -301,6 +303,28 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     StepPlan plan, dplan;  // evolution passes (no bra) and moment passes (dot with psiL)
     const bool direct = (opt_flags & GTB_OPT_BLOCK_DIRECT) != 0;
     bool fused = false;   // the blocked passes (K7b, K7b9) keep the separate accumulation kernel
+    // the fused passes may run on a compressed form of the same matrix (gtb_kpm_options.alt): packed rows or
+    // windowed tiles; the velocity operator always reads the plain ELL
+    const gtb_ell *Hprop = H, *Hmom = H;   // matrices of the propagation / moment passes
+    int32_t aux = 0;
+    if (opt && opt->alt) {
+      const gtb_ell* A = opt->alt;
+      bool ok = A->n == n && !orb && R == R_batch;
+      if (ok && opt->alt_mode == GTB_MODE_PACKED) {
+        ok = make_plan_packed(A, R, 2, &plan) && make_plan_packed(A, R, 1, &dplan);
+        Hprop = Hmom = A;
+      } else if (ok && opt->alt_mode == GTB_MODE_WINDOW) {
+        // windowed tiles serve the moment passes; the propagation passes (a fourth streamed vector beside a
+        // 50 KB stage) measured slower on them than on K7t and stay on the plain matrix
+        ok = make_plan_window(A, R, 1, opt->tile_stages, &dplan) && make_plan(H, R, 2, nullptr, &plan) == GTB_OK;
+        Hmom = A;
+        aux = (A->width >> 16) & 0xff;
+      } else {
+        ok = false;
+      }
+      if (!ok) return GTB_ERR_INVALID_ARG;
+      fused = true;
+    } else
     if (!(orb && !(opt_flags & GTB_OPT_SCALAR_BLOCKS) && make_plan_orb(H, R, orb, false, direct, &plan) &&
           make_plan_orb(H, R, orb, true, direct, &dplan))) {
       fused = !(opt_flags & GTB_OPT_SEPARATE_AXPY);
@@ -318,9 +342,9 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
     GTB_LAUNCHED();
     for (int j = 0; j < n_steps; ++j) {
       if (j > 0) {
-        rc = evolve_in_place(H, plan, fused, a, b, coef, R, &psiL, &sa_, &sb_, w.partial, st);
+        rc = evolve_in_place(Hprop, 0, plan, fused, a, b, coef, R, &psiL, &sa_, &sb_, w.partial, st);
         if (rc != GTB_OK) return rc;
-        rc = evolve_in_place(H, plan, fused, a, b, coef, R, &psiR, &sa_, &sb_, w.partial, st);
+        rc = evolve_in_place(Hprop, 0, plan, fused, a, b, coef, R, &psiR, &sa_, &sb_, w.partial, st);
         if (rc != GTB_OK) return rc;
       }
       double* cur = sa_;  // chi_0 = V psiR, partial slot 0 = Re<psiL|chi_0>
@@ -331,8 +355,9 @@ extern "C" int gtb_vac_moments(const gtb_ell* H, const double* vvals, double a, 
       GTB_LAUNCHED();
       const bool timed = last_batch && j == n_steps - 1;
       if (timed && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
-      StepArgs sa{H->cols, H->vals, H->diag, n, H->width, dplan.T, cur, io, 1.0 / a, b,
+      StepArgs sa{Hmom->cols, Hmom->vals, Hmom->diag, n, Hmom->width & 0xffff, dplan.T, cur, io, 1.0 / a, b,
                   w.partial + kMaxGrid, psiL};
+      sa.aux = aux;
       for (int k = 1; k < M; ++k) {  // io <- chi_k, slot k = (Re<psiL|chi_{k-1}>, Re<psiL|chi_k>)
         sa.phi_cur = cur;
         sa.phi_io = io;

@@ -344,11 +344,11 @@ void pick_window(bool diag, int mode, StepPlan* p) {
 
 }  // namespace
 
-// plan of the windowed pass: Wd->n rows, Wd->width = K + 65536 x (blocks of the largest window), Wd->vals = the
-// blob of gtb_window_ell built for THIS R, Wd->diag != NULL iff the tiles carry a diagonal.  stages: 0 = default
+// plan of the windowed pass: Wd->n rows, Wd->width = K | blocks of the largest window << 16 | R << 24, Wd->vals =
+// the blob of gtb_window_ell built for THIS R (checked), Wd->diag != NULL iff the tiles carry a diagonal.  stages: 0 = default
 bool make_plan_window(const gtb_ell* Wd, int R, int mode, int want_stages, StepPlan* p) {
-  const int K = Wd->width & 0xffff, blocks = Wd->width >> 16;
-  if ((R != 2 && R != 4 && R != 8) || K < 1 || blocks < 0 || blocks > kMaxBlocks || !Wd->vals || mode < 0 ||
+  const int K = Wd->width & 0xffff, blocks = (Wd->width >> 16) & 0xff, built_for = Wd->width >> 24;
+  if ((R != 2 && R != 4 && R != 8) || built_for != R || K < 1 || blocks < 0 || blocks > kMaxBlocks || !Wd->vals || mode < 0 ||
       mode > 2 || (reinterpret_cast<uintptr_t>(Wd->vals) & 127u))
     return false;
   const bool diag = Wd->diag != nullptr;
@@ -409,7 +409,7 @@ extern "C" int gtb_window_ell(const gtb_ell* H, int32_t R, gtb_ell* Wd, int32_t*
   GTB_CUDA_TRY(cudaStreamSynchronize(st));
   if (blocks_needed) *blocks_needed = worst;
   if (worst > kMaxBlocks) return GTB_ERR_NOT_PACKABLE;
-  Wd->width = H->width + 65536 * worst;
+  Wd->width = H->width | (worst << 16) | (R << 24);
   Wd->cols = H->cols;   // unused by the pass; kept non-NULL for the argument checks
   Wd->diag = H->diag;
   return GTB_OK;

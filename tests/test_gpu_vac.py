@@ -177,3 +177,28 @@ def test_carrier_density_and_mobility_match_oracle():
             assert np.abs(mu - mu_ref).max() <= 1e-12 * np.abs(mu_ref).max()
     with pytest.raises(gtb.GtbError):
         gtb.carrier_density(_dev(rho), _dev(E), 99.0)
+
+
+# ---- the fused passes of the VAC path on a compressed form of the same matrix (gtb_kpm_options.alt) ----------
+@pytest.mark.parametrize("key,nx,ny,kw,R,form", [("c5", 57, 43, {}, 2, "packed"), ("c4", 48, 21, {"stripe": 6}, 4, "packed"),
+                                                 ("c2", 61, 47, {}, 8, "window"), ("c3", 53, 41, {}, 4, "window")])  # noqa: E501
+def test_vac_moments_on_packed_rows_and_windowed_tiles(key, nx, ny, kw, R, form):
+    w, inp, Ho, Hg, a, b = _setup(key, nx, ny, **kw)
+    vo = oracle.velocity_ell(Ho, inp.pos, inp.box, inp.pbc, 0)
+    vg = gtb.velocity_ell(Hg, _dev(inp.pos), inp.box, inp.pbc, 0)
+    M, T = 20, 4
+    ref = oracle.vac_moments(Ho, vo, a, b, M, T, DT, R=R, seed=7, mode=0)
+    plain = gtb.vac_moments(Hg, vg, a, b, M, T, DT, R, R, 7, check=True).cpu().numpy()
+    if form == "packed":
+        alt, mode = gtb.pack_ell(Hg), gtb.MODE_PACKED
+    else:
+        alt, mode = gtb.window_ell(Hg, R), gtb.MODE_WINDOW
+    assert alt is not None
+    got = gtb.vac_moments(Hg, vg, a, b, M, T, DT, R, R, 7, check=True,
+                          opt=gtb.options(alt=alt, alt_mode=mode)).cpu().numpy()
+    c00 = abs(ref[0, 0])
+    assert np.abs(got - plain).max() <= 1e-13 * c00          # same vectors bit for bit, other block sums
+    assert np.abs(got - ref).max() <= 1e-11 * c00
+    if form == "window":
+        with pytest.raises(gtb.GtbError):                     # built for R vectors per pass
+            gtb.vac_moments(Hg, vg, a, b, M, T, DT, 2, 2, 7, opt=gtb.options(alt=alt, alt_mode=mode))

@@ -40,7 +40,7 @@ def test_windowed_pass_matches_the_oracle_and_the_tile_pass(key, nx, ny, R, diag
     inp = W.make_inputs(w)
     Ho, Hg = _both(w, inp, with_diag=diag)
     Wd = gtb.window_ell(Hg, R)
-    assert Wd is not None and 1 <= Wd.blocks <= 40 and Wd.width == Ho.width + 65536 * Wd.blocks
+    assert Wd is not None and 1 <= Wd.blocks <= 40 and Wd.width == Ho.width + 65536 * Wd.blocks + (R << 24)
     n = Ho.n
     if w.a is not None:
         a, b = w.a, w.b
