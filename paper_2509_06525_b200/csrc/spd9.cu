@@ -294,48 +294,18 @@ constexpr int kBond9Threads = 128;
 // (Also measured and removed: one complex number per thread, 160 registers and 12 instead of 8 warps per
 // SM for a second copy of the geometry -- the same 6.24 ms at K = 12; an L2 prefetch of the rows two grid
 // strides ahead -- 5 % slower.  ncu at 10^8 atoms, K = 12: fp64 pipe 35 %, L1 data pipe 57 %, DRAM 24 % with
-// traffic = 1.006 x the algorithmic bytes, 5.3 stall cycles per issue on long_scoreboard.)
-template <int VW, int LOG2T, bool kFirst, bool kDotL>
-__global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const StepArgs a) {
-  constexpr int T = 1 << LOG2T;
-  __shared__ double s_coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES * kNc];
-  __shared__ double s_onsite[3][GTB_MAX_SPECIES];
-  const BondHeader& h = *reinterpret_cast<const BondHeader*>(a.vals);
-  const int ns = h.n_species;
-  for (int q = threadIdx.x; q < ns * ns * kNc; q += kBond9Threads) s_coef[q] = (&h.coef[0][0])[q];
-  for (int q = threadIdx.x; q < 3 * GTB_MAX_SPECIES; q += kBond9Threads) (&s_onsite[0][0])[q] = (&h.onsite[0][0])[q];
-  // periodic axes: d -= L rint(d / L), as a multiplication by 1/L (a neighbour's d / L is within
-  // cutoff / L < 1/2 of an integer, far from the ties where the two roundings could differ)
-  const double Lx = h.box[0], Ly = h.box[1], Lz = h.box[2];
-  const double iLx = h.pbc[0] ? 1.0 / Lx : 0.0, iLy = h.pbc[1] ? 1.0 / Ly : 0.0, iLz = h.pbc[2] ? 1.0 / Lz : 0.0;
-  const double r0 = h.r0, beta = h.beta;
-  __syncthreads();
-  const int64_t n = a.n / 9;   // atoms
-  const int K = a.width;
-  const int64_t total = n * T;
-  const double* posw = a.vals + kBondHeaderBytes / 8;
-  const double* shift = posw + 4 * n;
-  double s1 = 0.0, s2 = 0.0;
-  for (int64_t e = (int64_t)blockIdx.x * kBond9Threads + threadIdx.x; e < total;
-       e += (int64_t)gridDim.x * kBond9Threads) {
-    const int64_t i = e >> LOG2T;
-    const int64_t t = e - i * T;
-    const double* xt = a.phi_cur + t * VW;
-    const Vec<4> pi = ld_rec(posw + 4 * i);
-    const int si = (int)pi.v[3];
-    Vec<VW> acc[9];
-#pragma unroll
-    for (int mu = 0; mu < 9; ++mu)
-#pragma unroll
-      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
-    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : i;
-    for (int k = 0; k < K; ++k) {
-      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : i;
-      if (j != i) {   // padding slots carry the atom's own index
-        const Vec<4> pj = ld_rec(posw + 4 * j);
-        Vec<VW> x[9];
-#pragma unroll
-        for (int nu = 0; nu < 9; ++nu) x[nu] = load_gather<VW>(xt + vec_off<LOG2T>(j, nu) * VW);
+// traffic = 1.006 x the algorithmic bytes, 5.3 stall cycles per issue on long_scoreboard.  And at R = 2, where a
+// neighbour's nine elements are 288 contiguous bytes: one cp.async.bulk per lane and neighbour into a per-lane
+// shared-memory slot, one neighbour ahead, per-warp mbarriers -- bit-identical, 8.52 ms against 6.25 at K = 12:
+// 1.2e8 small bulk copies per pass are one per ~20 cycles and SM, slower than the gathers they replace.)
+// geometry + closed-form action of one pair on the neighbour's nine orbital elements x into acc
+struct BondCtx {
+  double Lx, Ly, Lz, iLx, iLy, iLz, r0, beta;
+  const double* s_coef;
+  int ns;
+  template <int VW>
+  __device__ __forceinline__ void apply(const Vec<4>& pi, int si, const Vec<4>& pj, const Vec<VW> (&x)[9],
+                                        Vec<VW> (&acc)[9]) const {
         double dx = __dsub_rn(pj.v[0], pi.v[0]), dy = __dsub_rn(pj.v[1], pi.v[1]), dz = __dsub_rn(pj.v[2], pi.v[2]);
         dx = fma(-Lx, rint(dx * iLx), dx);
         dy = fma(-Ly, rint(dy * iLy), dy);
@@ -378,6 +348,55 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
           acc[7].v[q] = fma(c[11], d3, fma(D[3], Q, fma(hl, vx, fma(-hm, vy, acc[7].v[q]))));
           acc[8].v[q] = fma(c[11], d4, fma(D[4], Q, fma(-l2, vx, fma(-m2, vy, fma(g.n, vz, acc[8].v[q])))));
         }
+  }
+};
+
+template <int VW, int LOG2T, bool kFirst, bool kDotL>
+__global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const StepArgs a) {
+  constexpr int T = 1 << LOG2T;
+  __shared__ double s_coef[GTB_MAX_SPECIES * GTB_MAX_SPECIES * kNc];
+  __shared__ double s_onsite[3][GTB_MAX_SPECIES];
+  const BondHeader& h = *reinterpret_cast<const BondHeader*>(a.vals);
+  const int ns = h.n_species;
+  for (int q = threadIdx.x; q < ns * ns * kNc; q += kBond9Threads) s_coef[q] = (&h.coef[0][0])[q];
+  for (int q = threadIdx.x; q < 3 * GTB_MAX_SPECIES; q += kBond9Threads) (&s_onsite[0][0])[q] = (&h.onsite[0][0])[q];
+  // periodic axes: d -= L rint(d / L), as a multiplication by 1/L (a neighbour's d / L is within
+  // cutoff / L < 1/2 of an integer, far from the ties where the two roundings could differ)
+  BondCtx bond;
+  bond.Lx = h.box[0]; bond.Ly = h.box[1]; bond.Lz = h.box[2];
+  bond.iLx = h.pbc[0] ? 1.0 / bond.Lx : 0.0;
+  bond.iLy = h.pbc[1] ? 1.0 / bond.Ly : 0.0;
+  bond.iLz = h.pbc[2] ? 1.0 / bond.Lz : 0.0;
+  bond.r0 = h.r0; bond.beta = h.beta;
+  bond.s_coef = s_coef; bond.ns = ns;
+  __syncthreads();
+  const int64_t n = a.n / 9;   // atoms
+  const int K = a.width;
+  const int64_t total = n * T;
+  const double* posw = a.vals + kBondHeaderBytes / 8;
+  const double* shift = posw + 4 * n;
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * kBond9Threads + threadIdx.x; e < total;
+       e += (int64_t)gridDim.x * kBond9Threads) {
+    const int64_t i = e >> LOG2T;
+    const int64_t t = e - i * T;
+    const double* xt = a.phi_cur + t * VW;
+    const Vec<4> pi = ld_rec(posw + 4 * i);
+    const int si = (int)pi.v[3];
+    Vec<VW> acc[9];
+#pragma unroll
+    for (int mu = 0; mu < 9; ++mu)
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
+    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : i;
+    for (int k = 0; k < K; ++k) {
+      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : i;
+      if (j != i) {   // padding slots carry the atom's own index
+        const Vec<4> pj = ld_rec(posw + 4 * j);
+        Vec<VW> x[9];
+#pragma unroll
+        for (int nu = 0; nu < 9; ++nu) x[nu] = load_gather<VW>(xt + vec_off<LOG2T>(j, nu) * VW);
+        bond.apply(pi, si, pj, x, acc);
       }
       j = jn;
     }
@@ -401,12 +420,13 @@ void pick_rep9(int rep, StepPlan* p) {
     p->first = cheb_block9_kernel<LOG2T, true, false>;
     p->next = cheb_block9_kernel<LOG2T, false, false>;
     p->block = kBlock9Threads;
+    p->smem = 0;
   } else {
     p->first = cheb_bond9_kernel<4, LOG2T, true, false>;
     p->next = cheb_bond9_kernel<4, LOG2T, false, false>;
     p->block = kBond9Threads;
+    p->smem = 0;
   }
-  p->smem = 0;
 }
 
 int grid_of(int64_t total, int threads) {
