@@ -421,6 +421,8 @@ def run_ours(args):
                "cheb_bond9_kernel (K7m: fused Chebyshev pass, 9x9 pair action rebuilt from the bond vector)"
                if rep9 and REP == "bonds" else
                "cheb_block9_kernel (K7bb: fused Chebyshev pass on stored 9x9 blocks [K][81][n])" if rep9 else
+               "cheb_cluster_kernel (K7c: all passes in one 8-CTA cluster, phi in distributed shared memory; "
+               "ms_per_launch is per PASS)" if small and H.width <= 4 and n_orb * (w.R // 2) <= 8192 else
                "cheb_small_kernel (K7p: all passes in one cooperative launch; ms_per_launch is per PASS)" if small else
                ("cheb_orb%d_kernel (K7b: fused Chebyshev pass on %dx%d orbital blocks)" % (B, B, B)) if orb4 else
                "cheb_tile_kernel (K7t: fused Chebyshev pass, ELL slots staged by TMA)" if tile else

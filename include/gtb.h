@@ -99,9 +99,10 @@ enum {
   GTB_KERNEL_ROW_X2 = 2, /* K7x2: two elements in flight per thread; width <= 4, R in {2,4,8}          */
   GTB_KERNEL_TILE = 3    /* K7t: ELL slots staged by TMA; R in {2,4,8}, n % 4 == 0, 16-byte aligned H  */
 };
-#define GTB_OPT_PER_PASS_LAUNCH 1 /* never fold a small system's passes into one cooperative launch (K7p) */
+#define GTB_OPT_PER_PASS_LAUNCH 1 /* never fold a small system's passes into one launch (K7p, K7c)        */
 #define GTB_OPT_SCALAR_BLOCKS 2   /* ignore GTB_MODE_ORB4 / ORB9: run the scalar kernels on the expanded H */
 #define GTB_OPT_BLOCK_DIRECT 4    /* K7b9: strided block loads instead of the shared-memory hand-off      */
+#define GTB_OPT_GRID_SYNC 16      /* tiny systems: K7p (cooperative launch, grid barrier) instead of K7c (one cluster)   */
 #define GTB_OPT_SEPARATE_AXPY 8   /* gtb_vac_moments: one accumulation launch per Chebyshev-Bessel term
                                      instead of the accumulation fused into the propagation pass (same bits) */
 typedef struct gtb_kpm_options {

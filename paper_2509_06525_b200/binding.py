@@ -43,6 +43,7 @@ EXPORTS = (
 
 KERNEL_AUTO, KERNEL_ROW, KERNEL_ROW_X2, KERNEL_TILE = 0, 1, 2, 3      # gtb_kpm_options.kernel
 OPT_PER_PASS_LAUNCH, OPT_SCALAR_BLOCKS, OPT_BLOCK_DIRECT, OPT_SEPARATE_AXPY = 1, 2, 4, 8   # gtb_kpm_options.flags
+OPT_GRID_SYNC = 16
 MODE_ORB9 = 32              # ... gtb_spd_hamiltonian's (9 orbitals per atom)
 MODE_BLOCK9 = 64            # ... the block form written by spd_blocks (H.n = atoms)
 MODE_BOND9 = 128            # ... the bond form written by spd_bonds (matrix-free)

@@ -528,6 +528,122 @@ __global__ void __launch_bounds__(kBlock) cheb_small_kernel(const StepArgs a, co
 }
 
 
+// ---- K7c: all passes of a TINY system inside one thread-block cluster, phi in distributed shared memory -----
+// Config 1 (2 304 atoms, R = 4: 4 608 elements of 32 bytes) fits the shared memory of one cluster of 8 CTAs with
+// one thread per element.  Each CTA keeps its slice of both vector sets in its own shared memory for the whole
+// run, a thread keeps its row's <= 4 columns and hoppings in registers, gathers go to the owning CTA's shared
+// memory (mapa + ld.shared::cluster), and the passes are separated by a cluster barrier (arrive.release /
+// wait.acquire) instead of K7p's grid-wide barrier: no global-memory traffic per pass but the block sums.
+// Same arithmetic order per element and the same per-(pass, block) sums layout as K7p.
+constexpr int kClusterSize = 8;
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ Vec<4> ld_cluster(uint32_t addr) {
+  Vec<4> r;
+  asm volatile("ld.shared::cluster.v2.f64 {%0,%1}, [%2];" : "=d"(r.v[0]), "=d"(r.v[1]) : "r"(addr) : "memory");
+  asm volatile("ld.shared::cluster.v2.f64 {%0,%1}, [%2];" : "=d"(r.v[2]), "=d"(r.v[3]) : "r"(addr + 16) : "memory");
+  return r;
+}
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+template <int LOG2T, bool kDiag>
+__global__ void __cluster_dims__(kClusterSize, 1, 1) __launch_bounds__(1024)
+    cheb_cluster_kernel(const StepArgs a, const int S, const double inv_a, const int per_cta) {
+  constexpr int VW = 4;
+  constexpr int T = 1 << LOG2T;
+  constexpr int W = 4;   // width bound: columns and hoppings live in registers
+  extern __shared__ __align__(16) unsigned char s_phi[];   // [2][per_cta] elements of 32 bytes
+  const int64_t n = a.n;
+  const int64_t total = n * T;
+  const uint32_t rank = cluster_ctarank();
+  const int tid = threadIdx.x;
+  const int64_t e = (int64_t)rank * per_cta + tid;
+  const bool live = tid < per_cta && e < total;
+  const int64_t row = live ? (e >> LOG2T) : 0;
+  const int t = (int)(e & (T - 1));
+  const uint32_t base = smem_u32(s_phi);
+  const uint32_t buf_bytes = (uint32_t)per_cta * 32;
+  double* mine = reinterpret_cast<double*>(s_phi) + (size_t)tid * VW;   // + buffer * per_cta * VW
+  // phi_0 (written by the fill kernel) -> buffer 0
+  if (live) {
+    const Vec<VW> x0 = load_gather<VW>(a.phi_cur + e * VW);
+#pragma unroll
+    for (int q = 0; q < VW; ++q) mine[q] = x0.v[q];
+  }
+  // the row's slots: remote addresses of the gathered elements in buffer 0 (buffer 1: + buf_bytes)
+  uint32_t gaddr[W];
+  double v[W];
+#pragma unroll
+  for (int k = 0; k < W; ++k) {
+    const bool ok = live && k < a.width;
+    const int64_t c = ok ? (int64_t)__ldg(a.cols + (size_t)k * n + row) : row;
+    v[k] = ok ? __ldg(a.vals + (size_t)k * n + row) : 0.0;
+    const int64_t ce = c * T + t;
+    gaddr[k] = map_to_cta(base + (uint32_t)(ce % per_cta) * 32, (uint32_t)(ce / per_cta));
+  }
+  const double dg = kDiag && live ? __ldg(a.diag + row) : 0.0;
+  const double b = a.b;
+  const int nwarps = (int)(blockDim.x >> 5);
+  double2* s_sums = reinterpret_cast<double2*>(s_phi + 2 * (size_t)buf_bytes);   // [S][nwarps]
+  cluster_sync();   // every CTA's slice of phi_0 is in place
+  int cur = 0;
+  for (int k = 0; k < S; ++k) {
+    const double scale = k == 0 ? inv_a : 2.0 * inv_a;
+    double s1 = 0.0, s2 = 0.0;
+    if (live) {
+      const uint32_t off = cur ? buf_bytes : 0u;
+      Vec<VW> acc;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) acc.v[q] = 0.0;
+#pragma unroll
+      for (int s = 0; s < W; ++s) {
+        const Vec<VW> x = ld_cluster(gaddr[s] + off);
+#pragma unroll
+        for (int q = 0; q < VW; ++q) acc.v[q] = fma(v[s], x.v[q], acc.v[q]);
+      }
+      const double* own_p = mine + (size_t)cur * per_cta * VW;
+      double* io_p = mine + (size_t)(cur ^ 1) * per_cta * VW;
+#pragma unroll
+      for (int q = 0; q < VW; ++q) {
+        const double own = own_p[q];
+        double hx = acc.v[q];
+        if (kDiag) hx = fma(dg, own, hx);
+        double y = (hx - b * own) * scale;
+        if (k > 0) y -= io_p[q];
+        s1 = fma(own, own, s1);
+        s2 = fma(y, own, s2);
+        io_p[q] = y;
+      }
+    }
+    // warp sums parked in shared memory, [pass][warp]: no block barrier and no serial block sum inside a pass
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if ((tid & 31) == 0) s_sums[(size_t)k * nwarps + (tid >> 5)] = make_double2(s1, s2);
+    cluster_sync();   // phi_{k+1} complete in every CTA before anyone gathers it
+    cur ^= 1;
+  }
+  for (int k = tid; k < S; k += (int)blockDim.x) {   // block sums in warp order, as K7p's
+    double2 acc = s_sums[(size_t)k * nwarps];
+    for (int w = 1; w < nwarps; ++w) {
+      acc.x += s_sums[(size_t)k * nwarps + w].x;
+      acc.y += s_sums[(size_t)k * nwarps + w].y;
+    }
+    a.partial[(size_t)k * kMaxGrid + blockIdx.x] = acc;
+  }
+}
+
 // K8a: sums[step] += sum over blocks of partial[step][block], in a fixed order
 __global__ void __launch_bounds__(128) reduce_partials_kernel(const double2* __restrict__ partial,
                                                               int stride, int grid, double2* sums) {
@@ -744,7 +860,7 @@ int check_options(const gtb_kpm_options* opt) {
   if (opt->kernel < GTB_KERNEL_AUTO || opt->kernel > GTB_KERNEL_TILE || opt->tile_stages < 0 ||
       opt->tile_stages > 8 ||
       (opt->flags & ~(GTB_OPT_PER_PASS_LAUNCH | GTB_OPT_SCALAR_BLOCKS | GTB_OPT_BLOCK_DIRECT |
-                      GTB_OPT_SEPARATE_AXPY)) ||
+                      GTB_OPT_SEPARATE_AXPY | GTB_OPT_GRID_SYNC)) ||
       ((opt->loop_begin == nullptr) != (opt->loop_end == nullptr)) ||
       (opt->alt && opt->alt_mode != GTB_MODE_PACKED && opt->alt_mode != GTB_MODE_WINDOW))
     return GTB_ERR_INVALID_ARG;
@@ -856,6 +972,13 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
       rc = make_plan(H, R, false, opt, &plan);
       if (rc != GTB_OK) return rc;
     }
+    // K7c: a tiny system inside one cluster of 8 CTAs, phi in distributed shared memory
+    int cluster_threads = 0;
+    if (!blocked && plan.vw == 4 && S >= 2 && H->width <= 4 && n * plan.T <= kClusterSize * 1024 &&
+        !(opt_flags & (GTB_OPT_PER_PASS_LAUNCH | GTB_OPT_GRID_SYNC)) && (!opt || opt->kernel == GTB_KERNEL_AUTO))
+      cluster_threads = (int)(((n * plan.T + kClusterSize - 1) / kClusterSize + 31) / 32 * 32);
+    if (cluster_threads > 0 && (size_t)2 * cluster_threads * 32 + (size_t)S * (cluster_threads / 32) * 16 > 200 * 1024)
+      cluster_threads = 0;   // the per-pass warp sums must fit beside the vectors
     // K7p: every element of phi on its own resident thread -> all passes in one cooperative launch
     int small_grid = 0;
     void* small_fn = nullptr;
@@ -880,6 +1003,25 @@ extern "C" int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, 
     StepArgs sa{H->cols, H->vals, H->diag, n, windowed ? (H->width & 0xffff) : H->width, plan.T, cur, io, 1.0 / a, b,
                 w.partial};
     sa.aux = windowed ? ((H->width >> 16) & 0xff) : 0;
+    if (cluster_threads > 0) {  // K7c: K6 and all K7 passes in one cluster launch
+      const bool dg = H->diag != nullptr;
+      using ClusterFn = void (*)(const StepArgs, const int, const double, const int);
+      ClusterFn fn = plan.T == 1 ? (dg ? cheb_cluster_kernel<0, true> : cheb_cluster_kernel<0, false>)
+                   : plan.T == 2 ? (dg ? cheb_cluster_kernel<1, true> : cheb_cluster_kernel<1, false>)
+                                 : (dg ? cheb_cluster_kernel<2, true> : cheb_cluster_kernel<2, false>);
+      const size_t smem = (size_t)2 * cluster_threads * 32 + (size_t)S * (cluster_threads / 32) * 16;
+      GTB_CUDA_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      if (last_batch && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
+      fn<<<kClusterSize, cluster_threads, smem, st>>>(sa, S, 1.0 / a, cluster_threads);
+      GTB_LAUNCHED();
+      if (last_batch && ev_end) {
+        GTB_CUDA_TRY(cudaEventRecord(ev_end, st));
+        if (opt->loop_passes) *opt->loop_passes = S;
+      }
+      reduce_partials_kernel<<<S, 128, 0, st>>>(w.partial, kMaxGrid, kClusterSize, w.sums);
+      GTB_LAUNCHED();
+      continue;
+    }
     if (small_grid > 0) {  // K7p: K6 and all K7 passes in one launch
       if (last_batch && ev_beg) GTB_CUDA_TRY(cudaEventRecord(ev_beg, st));
       int S_arg = S;

@@ -273,6 +273,35 @@ def test_single_launch_path_matches_oracle_and_per_pass_path(key, nx, ny, kw, R,
     assert np.abs(got - per_pass).max() <= 1e-13
     if M >= 64:
         assert used < (gtb.launch_count() - l0) // 4      # the single-launch path really was taken
+    grid = gtb.kpm_moments(Hg, a, b, M, R, R, 9, check=True, opt=gtb.options(flags=gtb.OPT_GRID_SYNC)).cpu().numpy()
+    assert np.abs(got - grid).max() <= 1e-13              # K7c (one cluster) vs K7p (grid barrier), where both apply
+
+
+# K7c: tiny systems (n T <= 8192 elements, K <= 4) run inside one thread-block cluster with phi in distributed
+# shared memory; sizes around the limits: one element per CTA slot, ragged last CTA, exactly full, one too many
+@pytest.mark.parametrize("nx,ny,R,width", [(24, 24, 4, None), (24, 24, 4, 4), (32, 32, 4, None), (45, 45, 2, None),
+                                           (16, 16, 8, None), (3, 3, 2, None), (32, 33, 4, None), (23, 19, 2, None)])
+def test_cluster_path_matches_oracle(nx, ny, R, width):
+    w, inp = _small("c1", nx, ny, {})
+    Ho = _oracle_H(w, inp, width=width, with_diag=False)
+    Hg = _gpu_H(w, inp, width=width, with_diag=False)
+    M = 96
+    ref = oracle.kpm_moments(Ho, w.a, w.b, M, R, 9, mode=0, algo=0)
+    l0 = gtb.launch_count()
+    got = gtb.kpm_moments(Hg, w.a, w.b, M, R, R, 9, check=True).cpu().numpy()
+    used = gtb.launch_count() - l0
+    assert np.abs(got - ref).max() <= 1e-12
+    if Ho.n * (R // 2) <= 8192:
+        assert used <= 6                                   # fill, one cluster launch, reduce, finish
+    exact = gtb.kpm_moments(Hg, w.a, w.b, 32, mode=1, R_batch=8).cpu().numpy()
+    want = oracle.kpm_moments(Ho, w.a, w.b, 32, mode=1, algo=0) if Ho.n <= 2400 else None
+    if want is not None:
+        assert np.abs(exact - want).max() <= 1e-12
+    w4, inp4 = _small("c4", 12, 8, {"stripe": 3})          # with a diagonal and three species
+    Ho4, Hg4 = _oracle_H(w4, inp4, with_diag=True), _gpu_H(w4, inp4, with_diag=True)
+    ref4 = oracle.kpm_moments(Ho4, w4.a, w4.b, 40, R, 3, mode=0, algo=0)
+    got4 = gtb.kpm_moments(Hg4, w4.a, w4.b, 40, R, R, 3, check=True).cpu().numpy()
+    assert np.abs(got4 - ref4).max() <= 1e-12
 
 
 # K7x2 (narrow rows: two elements in flight per thread) against the oracle's rows and against K7, on sizes
