@@ -40,9 +40,12 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
     for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
       for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
-    int64_t j = K > 0 ? (int64_t)(__ldg(cp) >> 2) : 0;
+    // the next column is carried as loaded: any arithmetic on it here would wait for the load at once
+    // (ncu on K7m: a quarter of the stall samples sat on the sign extension of the "prefetched" column)
+    int32_t craw = K > 0 ? __ldg(cp) : 0;
     for (int k = 0; k < K; ++k) {
-      const int64_t jn = k + 1 < K ? (int64_t)(__ldg(cp + (size_t)(4 * (k + 1)) * N) >> 2) : 0;
+      const int64_t j = (int64_t)(craw >> 2);
+      const int32_t cnext = k + 1 < K ? __ldg(cp + (size_t)(4 * (k + 1)) * N) : 0;
       Vec<VW> B[4], x[4];
 #pragma unroll
       for (int nu = 0; nu < 4; ++nu) B[nu] = load_stream<VW>(vp + (size_t)(4 * k + nu) * N);
@@ -54,7 +57,7 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb4_kernel(const StepArgs a) 
         for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
           for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(B[nu].v[mu], x[nu].v[q], acc[mu].v[q]);
-      j = jn;
+      craw = cnext;
     }
     Vec<VW> dg;
     if (kDiag) dg = load_stream<VW>(a.diag + 4 * i);
@@ -143,9 +146,10 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb9_kernel(const StepArgs a) 
 #pragma unroll
       for (int q = 0; q < NL; ++q) pre[q] = (K > 0 && lane + 32 * q < run) ? __ldg(vrun + lane + 32 * q) : 0.0;
     }
-    int64_t j = K > 0 ? (int64_t)(__ldg(cp) / B) : 0;
+    int32_t craw = K > 0 ? __ldg(cp) : 0;   // carried as loaded (see K7b)
     for (int k = 0; k < K; ++k) {
-      const int64_t jn = k + 1 < K ? (int64_t)(__ldg(cp + (size_t)(B * (k + 1)) * N) / B) : 0;
+      const int64_t j = (int64_t)(craw / B);
+      const int32_t cnext = k + 1 < K ? __ldg(cp + (size_t)(B * (k + 1)) * N) : 0;
 #pragma unroll 3
       for (int nu = 0; nu < B; ++nu) {
         if (kStage) {
@@ -172,7 +176,7 @@ __global__ void __launch_bounds__(kBlock, 2) cheb_orb9_kernel(const StepArgs a) 
           }
         }
       }
-      j = jn;
+      craw = cnext;
     }
     if (live) {
 #pragma unroll

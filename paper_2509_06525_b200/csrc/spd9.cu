@@ -258,9 +258,10 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
     for (int mu = 0; mu < 9; ++mu)
 #pragma unroll
       for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
-    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : 0;
+    int32_t craw = K > 0 ? ld_stream_i32(a.cols + i) : 0;   // carried as loaded (see K7m below)
     for (int k = 0; k < K; ++k) {
-      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : 0;
+      const int64_t j = craw;
+      const int32_t cnext = k + 1 < K ? ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : 0;
       const double* blk = a.vals + (size_t)k * 81 * n + i;
 #pragma unroll 3
       for (int nu = 0; nu < 9; ++nu) {
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(kBlock9Threads, 2) cheb_block9_kernel(const St
 #pragma unroll
           for (int q = 0; q < VW; ++q) acc[mu].v[q] = fma(hcol[mu], x.v[q], acc[mu].v[q]);
       }
-      j = jn;
+      craw = cnext;
     }
     double eps[9];
 #pragma unroll
@@ -388,17 +389,26 @@ __global__ void __launch_bounds__(kBond9Threads, 2) cheb_bond9_kernel(const Step
     for (int mu = 0; mu < 9; ++mu)
 #pragma unroll
       for (int q = 0; q < VW; ++q) acc[mu].v[q] = 0.0;
-    int64_t j = K > 0 ? (int64_t)ld_stream_i32(a.cols + i) : i;
+    // Columns run two neighbours ahead and the neighbour's record one ahead, all carried as loaded (32-bit
+    // index, raw record): ncu's source page showed 26 % of the pass's stall samples on the sign extension of
+    // the "prefetched" column, which the compiler had placed right behind its load, and 10 % on the record.
+    const int32_t self = (int32_t)i;
+    int32_t j0 = K > 0 ? ld_stream_i32(a.cols + i) : self;
+    int32_t j1 = K > 1 ? ld_stream_i32(a.cols + (size_t)n + i) : self;
+    Vec<4> p0 = ld_rec(posw + 4 * (int64_t)j0);
     for (int k = 0; k < K; ++k) {
-      const int64_t jn = k + 1 < K ? (int64_t)ld_stream_i32(a.cols + (size_t)(k + 1) * n + i) : i;
-      if (j != i) {   // padding slots carry the atom's own index
-        const Vec<4> pj = ld_rec(posw + 4 * j);
+      const int32_t j2 = k + 2 < K ? ld_stream_i32(a.cols + (size_t)(k + 2) * n + i) : self;
+      const Vec<4> p1 = ld_rec(posw + 4 * (int64_t)j1);
+      if (j0 != self) {   // padding slots carry the atom's own index
+        const int64_t j = j0;
         Vec<VW> x[9];
 #pragma unroll
         for (int nu = 0; nu < 9; ++nu) x[nu] = load_gather<VW>(xt + vec_off<LOG2T>(j, nu) * VW);
-        bond.apply(pi, si, pj, x, acc);
+        bond.apply(pi, si, p0, x, acc);
       }
-      j = jn;
+      j0 = j1;
+      j1 = j2;
+      p0 = p1;
     }
     const double sh = ld_stream_f64(shift + i);
     double eps[9];
