@@ -299,6 +299,20 @@ constexpr int kBond9Threads = 128;
 // neighbour's nine elements are 288 contiguous bytes: one cp.async.bulk per lane and neighbour into a per-lane
 // shared-memory slot, one neighbour ahead, per-warp mbarriers -- bit-identical, 8.52 ms against 6.25 at K = 12:
 // 1.2e8 small bulk copies per pass are one per ~20 cycles and SM, slower than the gathers they replace.)
+// Round 2, after the column / record carry below (6.25 -> 5.48 ms): the first use of the gathered rows holds 37 %
+// of the stall samples, fixed-latency dependencies 24 %, fp64 pipe 44 %.  Two more decompositions measured at
+// K = 12, 1.02e7 atoms and removed: one complex number per thread again (168 registers, 12 warps per SM) 5.71 ms;
+// one lane per REAL number (K7q: 2 R lanes per atom, nine accumulators each, 128 registers, 16 warps per SM; the
+// pair's geometry worked out once by one lane of the atom per chunk of 2 R neighbours and handed to the others
+// through shared memory, so the fp64 work per pair stays 75 + 4 x 64) 6.96 ms: bit-compatible with the tests, but
+// l1tex__data_pipe_lsu_wavefronts goes to 91 % -- the gathers cost the same ~9 wavefronts per pair in any
+// decomposition (a neighbour's 288 bytes lie in lines that no other lane of the instruction shares) and the
+// records add 6 per pair.  So the L1 data pipe, ~3.6 ms of the 5.48, is this pass's floor short of staging the
+// gathered rows in shared memory (the windowed tiles of window.cu applied to 288-byte rows); prefetch.global.L1
+// of the next neighbour's rows: 5.66 ms.  At 10^8 atoms the pass reads 1.4 x its algorithmic bytes from DRAM: a
+// neighbour's rows are used again one lattice row (20 000 atoms, two grid strides) later, at the edge of what L2
+// keeps; an L2 evict-first policy on the streamed prev / y rows changes neither bytes nor time, a tile-major
+// numbering of the INPUT atoms (16 x 16 cells) brings 1.07 x and 54.4 instead of 56.6 ms.
 // geometry + closed-form action of one pair on the neighbour's nine orbital elements x into acc
 struct BondCtx {
   double Lx, Ly, Lz, iLx, iLy, iLz, r0, beta;
