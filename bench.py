@@ -37,6 +37,7 @@ UNIT = "atom*moment*vector updates/s"
 KERNEL = "auto"                 # set by --kernel: pins the fused-pass kernel through gtb_kpm_options
 STAGES = 0                      # set by --stages: ring depth of the staged passes (0 = the library's default)
 WINDOW = True                   # cleared by --no-window: windowed tiles (gtb_window_ell, K7w) for wide rows
+TILE_NUMBERING = None           # --tile-numbering TXxTY: the same lattice with its atoms numbered tile-major (input order study)
 PACK = True                     # cleared by --no-pack: packed narrow rows (gtb_pack_ell, K7x2p) when the matrix fits
 REP = "scalar"                  # set by --rep (spd only): scalar ELL expansion, stored 9x9 blocks, or bonds (matrix-free)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x clocks.max.sm
@@ -247,7 +248,7 @@ def run_ours(args):
     gtb.lib()
 
     w = _workload(args)
-    inp = W.make_inputs(w)
+    inp = W.make_inputs(w, tile=TILE_NUMBERING)
     n = w.n_atoms
     seed = replicas.replica_seed(w.seed, rank)      # independent replica per rank
     # host inputs in pinned memory (e2e arm) and resident copies (device arm)
@@ -461,7 +462,8 @@ def run_ours(args):
             "config": {"workload": w.name, "atoms": n, "orbitals_per_atom": n_orb // n,
                        "ell_width": H.width,
                        "representation": REP if ORBITALS == "spd" else "packed rows" if packed is not None else "ell",
-                       "cutoff_A": w.cutoff, "moments": w.M,
+                       "cutoff_A": w.cutoff, "numbering": ("tile-major %dx%d cells" % TILE_NUMBERING) if TILE_NUMBERING else "row-major",
+                       "moments": w.M,
                        "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
                        "l2": "inputs larger than L2 (working set %.1f GB)" % (
                            (2 * n_orb * w.R * 16 + (H.nbytes() if not rep9 else H.cols.numel() * 4 + H.vals.numel() * 8)) / 1e9),
@@ -712,13 +714,18 @@ def main():
     p.add_argument("--stages", type=int, default=0, help="gtb_kpm_options.tile_stages (K7t, K7w); 0 = default")
     p.add_argument("--no-window", action="store_true", help="keep wide matrices on the plain ELL path (K7t)")
     p.add_argument("--no-pack", action="store_true", help="keep narrow matrices on the plain ELL path (K7x2)")
+    p.add_argument("--tile-numbering", default="", help="TXxTY: number the input atoms tile-major in blocks of TX x TY "
+                   "cells instead of row-major (same lattice; shows what the input order costs the gathers)")
     p.add_argument("--cutoff", type=float, default=0.0, help="override the neighbour cutoff in Angstrom "
                    "(3.0 on the pristine lattice = third-nearest neighbours, K = 12: Fig. 4a)")
     p.add_argument("--orbitals", default="pz", choices=["pz", "sp", "spd"],
                    help="pz: one orbital per atom (the headline); sp: Slater-Koster s,px,py,pz blocks (NEXT-2, dos only)")
     args = p.parse_args()
-    global ORBITALS, HOPPING, KERNEL, REP, PACK, WINDOW, STAGES
+    global ORBITALS, HOPPING, KERNEL, REP, PACK, WINDOW, STAGES, TILE_NUMBERING
     STAGES = args.stages
+    if args.tile_numbering:
+        tx, _, ty = args.tile_numbering.lower().partition("x")
+        TILE_NUMBERING = (int(tx), int(ty))
     WINDOW = not args.no_window
     PACK = not args.no_pack
     KERNEL = args.kernel

@@ -111,7 +111,11 @@ class Inputs:
     workload: Workload = field(repr=False, default=None)
 
 
-def make_inputs(w: Workload, seed: int = SEED_LATTICE) -> Inputs:
+def make_inputs(w: Workload, seed: int = SEED_LATTICE, tile: Optional[tuple] = None) -> Inputs:
+    """The lattice of workload `w`.  Atoms are numbered row-major (cell row, cell, basis atom).  tile = (tx, ty)
+    renumbers the SAME atoms tile-major: blocks of tx x ty cells one after the other (row-major inside a block
+    and over the blocks) -- the same structure, another order of its rows, for measuring what the numbering of
+    the input costs the gathers (bench.py --tile-numbering)."""
     nx, ny = w.nx, w.ny
     n = 4 * nx * ny
     basis = np.array([[0.0, 0.0], [0.0, A_CC], [LX / 2, 1.5 * A_CC], [LX / 2, 2.5 * A_CC]])
@@ -140,6 +144,17 @@ def make_inputs(w: Workload, seed: int = SEED_LATTICE) -> Inputs:
     species = species.reshape(n)
     box = np.array([nx * LX, ny * LY, LZ])
     pbc = np.array([1, 1, 0], dtype=np.int32)
+    if tile is not None:
+        tx, ty = int(tile[0]), int(tile[1])
+        if tx < 1 or ty < 1:
+            raise ValueError("tile = (tx, ty) cells, both >= 1")
+        cy, cx, bs = np.meshgrid(np.arange(ny), np.arange(nx), np.arange(4), indexing="ij")
+        cy, cx, bs = cy.ravel(), cx.ravel(), bs.ravel()
+        order = np.lexsort((bs, cx % tx, cy % ty, cx // tx, cy // ty))   # last key is the primary one
+        pos = np.ascontiguousarray(pos[order])
+        species = np.ascontiguousarray(species[order])
+        if shift is not None:
+            shift = np.ascontiguousarray(shift[order])
     return Inputs(pos, species, box, pbc, shift, w)
 
 

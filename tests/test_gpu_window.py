@@ -76,6 +76,26 @@ def test_windowed_pass_matches_the_oracle_and_the_tile_pass(key, nx, ny, R, diag
         gtb.kpm_moments(Wd, a, b, 8, 3 * R // 2, R, 5, mode=gtb.MODE_WINDOW)
 
 
+def test_tile_major_numbering_shrinks_the_window_and_keeps_parity():
+    """The same lattice with its atoms numbered tile-major (workloads.make_inputs(tile=...), bench.py
+    --tile-numbering): smaller windows, and moments equal to the oracle's on the same renumbered input."""
+    w = W.CONFIGS["c2"].scaled(128, 96)
+    R, M = 8, 33
+    blocks = []
+    for tile in (None, (4, 4)):
+        inp = W.make_inputs(w, tile=tile)
+        Ho, Hg = _both(w, inp)
+        Wd = gtb.window_ell(Hg, R)
+        assert Wd is not None
+        blocks.append(Wd.blocks)
+        lo, hi = oracle.spectral_bounds(Ho)
+        a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+        got = gtb.kpm_moments(Wd, a, b, M, R, R, 5, mode=gtb.MODE_WINDOW, check=True).cpu().numpy()
+        ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
+        assert np.abs(got - ref).max() <= 1e-12
+    assert blocks[1] < blocks[0]
+
+
 def test_a_numbering_without_locality_stays_on_the_plain_path():
     w = W.CONFIGS["c2"].scaled(61, 47)
     inp = W.make_inputs(w)

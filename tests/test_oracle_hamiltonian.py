@@ -168,3 +168,23 @@ def test_gershgorin_bounds_contain_spectrum():
     off = np.abs(dense).sum(1) - np.abs(np.diag(dense))
     assert lo == pytest.approx((np.diag(dense) - off).min(), rel=1e-14)
     assert hi == pytest.approx((np.diag(dense) + off).max(), rel=1e-14)
+
+
+def test_tile_major_numbering_is_the_same_structure():
+    """workloads.make_inputs(tile=...) renumbers the atoms and nothing else: the same set of atoms (positions,
+    species, onsite shifts), every block of tx x ty cells contiguous, and the exact-trace moments -- which do not
+    depend on the order of the rows -- unchanged."""
+    w = W.CONFIGS["c4"].scaled(16, 12, stripe=4, M=24)
+    a, t = W.make_inputs(w), W.make_inputs(w, tile=(4, 3))
+    ka, kt = np.lexsort(a.pos.T), np.lexsort(t.pos.T)
+    assert np.array_equal(a.pos[ka], t.pos[kt]) and np.array_equal(a.species[ka], t.species[kt])
+    assert not np.array_equal(a.pos, t.pos)
+    # the first 4 x 3 x 4 atoms are the first block of cells (disorder << cell size)
+    first = t.pos[: 4 * 3 * 4]
+    assert first[:, 0].max() < 4 * W.LX and first[:, 1].max() < 3 * W.LY
+    mus = []
+    for inp in (a, t):
+        H = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
+                                     w.beta, inp.onsite_shift)
+        mus.append(oracle.kpm_moments(H, w.a, w.b, w.M, mode=1))
+    np.testing.assert_allclose(mus[0], mus[1], rtol=0, atol=1e-13)
