@@ -55,8 +55,10 @@ enum {
   GTB_ERR_DIVERGED = -5,      /* non-finite moments: spectrum outside [b-a, b+a]   */
   GTB_ERR_CUDA = -6,          /* CUDA runtime error; see gtb_last_cuda_error()     */
   GTB_ERR_INDEX_RANGE = -7,   /* n too large for int32 indices                     */
-  GTB_ERR_NOT_PACKABLE = -8   /* gtb_pack_ell: width > 4, a column offset beyond +-32767 rows or more than
+  GTB_ERR_NOT_PACKABLE = -8,  /* gtb_pack_ell: width > 4, a column offset beyond +-32767 rows or more than
                                  65535 distinct values: stay on the plain ELL path       */
+  GTB_ERR_STATIC_LIMIT = -9   /* gtb_kpm_moments_static: the run needs more than GTB_STATIC_WS_BYTES of
+                                 scratch; use gtb_kpm_moments with a caller-owned workspace           */
 };
 
 #define GTB_MODE_ORB4 16 /* flag for gtb_kpm_moments' mode: H comes from gtb_sk_hamiltonian  (4 orbitals) */
@@ -190,6 +192,26 @@ int gtb_kpm_moments(const gtb_ell* H, double a, double b, int32_t M, int32_t R_t
 /* SYNC.  GTB_ERR_DIVERGED if the last gtb_kpm_moments run on this workspace
  * produced a non-finite moment, else GTB_OK. */
 int gtb_kpm_status(const void* ws, void* stream);
+
+/* ---- the same moments with NO allocation and no caller workspace ------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it).  gtb_kpm_moments_static is gtb_kpm_moments (north_star (3); same arguments,
+ * same kernels, same results bit for bit) with the workspace taken from a static device array inside the
+ * library instead of from the caller: GTB_STATIC_WS_BYTES (4 MiB) on every GPU that loads the library, held
+ * until the process exits.  The caller still owns and passes H and mu (DEVICE [M]).
+ * Limit: gtb_kpm_workspace_bytes(rows, M, R_batch) <= GTB_STATIC_WS_BYTES, rows = H->n (9 H->n in the
+ * BLOCK9 / BOND9 modes); e.g. config 1 (2304 atoms, M = 256, R = 4) needs 2.7 MiB.  Anything larger returns
+ * GTB_ERR_STATIC_LIMIT before a kernel is launched.
+ * The call uses no cudaMalloc / cudaFree or other allocating routine (once per device it asks the runtime for
+ * the array's device address).  ASYNC on the caller's stream.
+ * Sharing: every call on a device uses the SAME array, which keeps the previous call's contents.  What must
+ * start at zero is cleared on the stream at the start of each call; calls that may overlap on the GPU (two
+ * streams, two host threads) race on it -- order them.  There is no status word to read afterwards: a
+ * diverged run (spectrum outside [b - a, b + a]) shows as non-finite mu. */
+#define GTB_STATIC_WS_BYTES (4 << 20)
+int gtb_kpm_moments_static(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
+                           int32_t R_batch, uint64_t seed, int32_t mode, double* mu, void* stream,
+                           const gtb_kpm_options* opt);
 
 /* ASYNC.  One fused recursion pass, exported for the full-size sampled parity test:
  *   first != 0:  out = (H phi_cur - b phi_cur) / a                 (phi_io is written only)

@@ -20,7 +20,7 @@ from . import build as _build
 
 OK = 0
 ERR_INVALID_ARG, ERR_BOX_TOO_SMALL, ERR_ELL_OVERFLOW, ERR_WORKSPACE = -1, -2, -3, -4
-ERR_DIVERGED, ERR_CUDA, ERR_INDEX_RANGE, ERR_NOT_PACKABLE = -5, -6, -7, -8
+ERR_DIVERGED, ERR_CUDA, ERR_INDEX_RANGE, ERR_NOT_PACKABLE, ERR_STATIC_LIMIT = -5, -6, -7, -8, -9
 MAX_WIDTH = 64
 
 # every symbol include/gtb.h declares (tests check that the library exports each of them)
@@ -28,7 +28,7 @@ EXPORTS = (
     "gtb_status_string", "gtb_last_cuda_error", "gtb_version", "gtb_launch_count",
     "gtb_build_workspace_bytes", "gtb_neighbor_width", "gtb_build_hamiltonian",
     "gtb_bounds_workspace_bytes", "gtb_spectral_bounds", "gtb_random_phase_fill",
-    "gtb_kpm_workspace_bytes", "gtb_kpm_moments", "gtb_kpm_status", "gtb_kpm_step",
+    "gtb_kpm_workspace_bytes", "gtb_kpm_moments", "gtb_kpm_status", "gtb_kpm_step", "gtb_kpm_moments_static",
     "gtb_dos", "gtb_jackson",
     "gtb_velocity_ell", "gtb_velocity_apply", "gtb_evolve_workspace_bytes", "gtb_evolve",
     "gtb_vac_workspace_bytes", "gtb_vac_moments", "gtb_vac_conductivity",
@@ -324,6 +324,28 @@ def kpm_moments(H: Ell, a: float, b: float, M: int, R_total: int = 1,
     _check(st, "kpm_moments")
     if check:
         kpm_status(ws)
+    return mu
+
+
+STATIC_WS_BYTES = 4 << 20          # GTB_STATIC_WS_BYTES
+
+
+def kpm_moments_static(H: Ell, a: float, b: float, M: int, R_total: int = 1, R_batch: Optional[int] = None,
+                       seed: int = 0, mode: int = 0, mu: Optional[torch.Tensor] = None,
+                       opt: Optional[_Options] = None) -> torch.Tensor:
+    """gtb_kpm_moments_static: the moments with the scratch in the library's static device array (no
+    allocation inside the call; pass `mu` to allocate nothing here either).  GtbError(ERR_STATIC_LIMIT)
+    when the run needs more than STATIC_WS_BYTES."""
+    dev = H.vals.device if H.width else H.diag.device
+    if R_batch is None:
+        R_batch = R_total if (mode & 1) == 0 else 8
+    if mu is None:
+        mu = torch.empty(M, dtype=torch.float64, device=dev)
+    hc = H._c()
+    st = lib().gtb_kpm_moments_static(C.byref(hc), C.c_double(a), C.c_double(b), C.c_int32(M),
+                                      C.c_int32(R_total), C.c_int32(R_batch), C.c_uint64(seed & (2**64 - 1)),
+                                      C.c_int32(mode), _ptr(mu), _stream(), _opt(opt))
+    _check(st, "kpm_moments_static")
     return mu
 
 

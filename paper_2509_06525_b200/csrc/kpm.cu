@@ -18,6 +18,7 @@
 
 #include <cmath>
 #include <cstdlib>
+#include <mutex>
 
 #include "tma.cuh"
 #include "vecload.cuh"
@@ -1070,6 +1071,51 @@ extern "C" int gtb_kpm_status(const void* ws, void* stream) {
   GTB_CUDA_TRY(cudaMemcpyAsync(&flag, ws, sizeof(flag), cudaMemcpyDeviceToHost, st));
   GTB_CUDA_TRY(cudaStreamSynchronize(st));
   return flag ? GTB_ERR_DIVERGED : GTB_OK;
+}
+
+// ---- gtb_kpm_moments_static: the same run with its scratch in a static device array -------------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the
+// workspace of gtb_kpm_moments lives in g_static_ws below, GTB_STATIC_WS_BYTES per GPU that loads the library,
+// held until the process exits.  In host code the NAME g_static_ws is a host-side stand-in, not a device
+// address -- a kernel handed &g_static_ws[0] from the host faults (or, where the GPU reaches host memory,
+// silently uses the wrong memory) -- so the device address is asked for once per device, with that device
+// current, by cudaGetSymbolAddress, and that pointer is what goes down as the workspace.
+static __device__ __align__(256) unsigned char g_static_ws[GTB_STATIC_WS_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_addr[kMaxDevices] = {};   // device address of g_static_ws on device d, once asked for
+}  // namespace
+
+extern "C" int gtb_kpm_moments_static(const gtb_ell* H, double a, double b, int32_t M, int32_t R_total,
+                                      int32_t R_batch, uint64_t seed, int32_t mode_flags, double* mu,
+                                      void* stream, const gtb_kpm_options* opt) {
+  int rc = check_ell(H);
+  if (rc != GTB_OK) return rc;
+  if (M <= 0 || R_batch <= 0 || R_batch > 64) return GTB_ERR_INVALID_ARG;
+  const bool rep = (mode_flags & (GTB_MODE_BLOCK9 | GTB_MODE_BOND9)) != 0;
+  const int64_t rows = rep ? 9 * H->n : H->n;
+  // the size is checked before anything is launched: nothing beyond the array is ever carved
+  if (rows > (int64_t)GTB_STATIC_WS_BYTES || gtb_kpm_workspace_bytes(rows, M, R_batch) > (size_t)GTB_STATIC_WS_BYTES)
+    return GTB_ERR_STATIC_LIMIT;
+  int dev = 0;
+  GTB_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return GTB_ERR_INVALID_ARG;
+  void* ws = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+      void* p = nullptr;
+      GTB_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_ws));
+      g_static_addr[dev] = p;
+    }
+    ws = g_static_addr[dev];
+  }
+  // gtb_kpm_moments clears what must start at zero (the per-pass sums and the status word) on the stream and
+  // overwrites every other word it later reads; it calls no allocating routine
+  return gtb_kpm_moments(H, a, b, M, R_total, R_batch, seed, mode_flags, mu, ws, (size_t)GTB_STATIC_WS_BYTES, stream,
+                         opt);
 }
 
 extern "C" int gtb_kpm_step(const gtb_ell* H, double a, double b, int32_t first, int32_t R,

@@ -30,6 +30,9 @@ extern "C" const char* gtb_status_string(int status) {
     case GTB_ERR_CUDA: return "CUDA runtime error";
     case GTB_ERR_INDEX_RANGE: return "too many atoms for int32 indices";
     case GTB_ERR_NOT_PACKABLE: return "matrix does not fit the packed-row format (width, offsets or distinct values)";
+    case GTB_ERR_STATIC_LIMIT:
+      return "the run needs more scratch than the static array holds (GTB_STATIC_WS_BYTES); use gtb_kpm_moments "
+             "with a caller-owned workspace";
     default: return "unknown status";
   }
 }

@@ -33,7 +33,7 @@ def test_library_builds_for_sm_100a_and_exports_every_declared_symbol():
 
 def test_status_strings_and_version():
     assert gtb.status_string(0) == "ok"
-    for st in range(-8, 0):
+    for st in range(-9, 0):
         assert gtb.status_string(st) not in ("ok", "unknown status")
     assert gtb.status_string(-99) == "unknown status"
     assert gtb.version() >= 100
