@@ -417,7 +417,7 @@ size_t gtb_packed_dict_bytes(void);
 int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_bytes, void* stream, int32_t* n_values);
 
 /* ---- windowed tiles for wide rows (K7w; sliced ELL + 16-bit relative columns) ----
- * A re-arrangement of an ELL matrix for R_batch = R vectors, tile by tile (256 / (R/2) rows): the distinct
+ * A re-arrangement of an ELL matrix for R_batch = R vectors, tile by tile (256 / (R/2) rows; R = 8: 32 rows): the distinct
  * 1 KB blocks of phi rows the tile's columns touch (its window, at most 40), every column as a 16-bit index
  * into that window, the tile's own slot count (longest row of the tile), and its hoppings / diagonal /
  * columns contiguous.  The pass (gtb_kpm_moments / gtb_kpm_step with mode | GTB_MODE_WINDOW, R_batch = R,

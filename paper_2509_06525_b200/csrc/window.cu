@@ -5,7 +5,7 @@
 // data pipe and on the latency of the gathers that miss L1 (profiles/r01_wide_k7_full.md).  Lattices are
 // numbered so that the neighbours of a tile of consecutive rows fall into a few short runs of rows (the tile's
 // own row of cells and the two next to it).  gtb_window_ell therefore re-arranges H once, tile by tile
-// (TR = 256 / T rows, T = R / 2 threads per row):
+// (T = R / 2 threads per row; TR = 256 / T rows, at R = 8 TR = 128 / T = 32 rows -- tile_threads below):
 //   * the distinct row BLOCKS (G rows = 1 KB of phi each) the tile's columns touch, ascending: its window;
 //   * every column as a 16-bit index into that window (position of its block x G + row within the block);
 //   * the tile's own slot count K_t = longest row of the tile (sliced ELL: padding slots beyond it are dropped);
@@ -37,10 +37,18 @@ struct WinLayout {
   int64_t n_tiles;
 };
 
+// Consumer threads per tile and CTAs per SM.  R = 8 takes 32-row tiles (128 consumer threads, four CTAs per SM):
+// ncu had the 64-row pass waiting for its stages to fill (profiles/r02_wide_k7w.md), and eight 27 KB stages in
+// flight per SM fill more evenly than four 50 KB ones although a smaller tile brings more window per row:
+// c2 0.148 -> 0.143 ms.  Measured around it: 128-row tiles (one CTA per SM) 0.186 ms, 16-row tiles (six CTAs)
+// 0.159 ms; R = 4 with 64-row tiles 0.96 instead of 0.92 ms at c3 (that pass sits on the shared-memory pipe).
+__host__ __device__ constexpr int tile_threads(int R) { return R == 8 ? 128 : kWinThreads; }
+__host__ __device__ constexpr int tile_ctas(int R) { return R == 8 ? 4 : 2; }
+
 __host__ __device__ inline WinLayout win_layout(int64_t n, int K, int R, bool diag) {
   WinLayout L;
   L.T = R / 2;
-  L.TR = kWinThreads / L.T;
+  L.TR = tile_threads(R) / L.T;
   L.G = kBlockBytes / (R * 16);
   L.vals_off = kHeadBytes;
   L.diag_off = L.vals_off + (uint32_t)K * L.TR * 8;
@@ -166,19 +174,21 @@ __device__ __forceinline__ Vec<VW> swap_halves(const Vec<VW>& x, bool odd) {
   return r;
 }
 
-// Warp-specialised: warps 0..7 consume (one thread per 256-bit element of the tile), warp 8 produces.  A stage
+// Warp-specialised: the first CT / 32 warps consume (one thread per 256-bit element of the tile), the last warp
+// produces.  A stage
 // goes round on two mbarriers: full[s] (the copies' bytes) and empty[s] (one arrival per consumer warp once it
 // has read the stage), so the consumer warps never wait for one another -- with a __syncthreads per tile and
 // warp 0 doubling as producer, ncu showed 5.9 stall cycles per issue on `barrier` and nothing else.
-constexpr int kWinCtaThreads = kWinThreads + 32;
-constexpr int kConsumerWarps = kWinThreads / 32;
-
 template <int LOG2T, bool kFirst, bool kDiag, int kMode>
-__global__ void __launch_bounds__(kWinCtaThreads, 2) cheb_window_kernel(const StepArgs a, const int nstages) {
+__global__ void __launch_bounds__(tile_threads(2 << LOG2T) + 32, tile_ctas(2 << LOG2T))
+cheb_window_kernel(const StepArgs a, const int nstages) {
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
-  constexpr int TR = kWinThreads / T;
   constexpr int R = 2 * T;
+  constexpr int CT = tile_threads(R);
+  constexpr int kWinCtaThreads = CT + 32;
+  constexpr int kConsumerWarps = CT / 32;
+  constexpr int TR = CT / T;
   constexpr int G = kBlockBytes / (R * 16);
   constexpr uint32_t kRowBytes = R * 16;
   constexpr int CH = 6;
@@ -356,7 +366,7 @@ bool make_plan_window(const gtb_ell* Wd, int R, int mode, int want_stages, StepP
   else if (R == 4) { pick_window<1>(diag, mode, p); p->T = 2; }
   else { pick_window<2>(diag, mode, p); p->T = 4; }
   p->vw = 4;
-  p->block = kWinCtaThreads;
+  p->block = tile_threads(R) + 32;
   const WinLayout L = win_layout(Wd->n, K, R, diag);
   const size_t stage_bytes = (size_t)L.tile_bytes + (size_t)blocks * kBlockBytes;
   int dev = 0, sms = kSmCount, per_sm = 0, max_smem = 0;
@@ -370,7 +380,7 @@ bool make_plan_window(const gtb_ell* Wd, int R, int mode, int want_stages, StepP
   if (smem > (size_t)max_smem) return false;
   if (cudaFuncSetAttribute(p->tfirst, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
       cudaFuncSetAttribute(p->tnext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, kWinCtaThreads, smem) != cudaSuccess)
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, p->tnext, p->block, smem) != cudaSuccess)
     return false;
   per_sm = std::max(1, std::min(per_sm, kMaxBlocksPerSm));
   p->grid = (int)std::max<int64_t>(1, std::min<int64_t>(L.n_tiles, (int64_t)sms * per_sm));
