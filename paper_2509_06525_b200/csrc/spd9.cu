@@ -307,8 +307,8 @@ constexpr int kBond9Threads = 128;
 // through shared memory, so the fp64 work per pair stays 75 + 4 x 64) 6.96 ms: bit-compatible with the tests, but
 // l1tex__data_pipe_lsu_wavefronts goes to 91 % -- the gathers cost the same ~9 wavefronts per pair in any
 // decomposition (a neighbour's 288 bytes lie in lines that no other lane of the instruction shares) and the
-// records add 6 per pair.  So the L1 data pipe, ~3.6 ms of the 5.48, is this pass's floor short of staging the
-// gathered rows in shared memory (the windowed tiles of window.cu applied to 288-byte rows); prefetch.global.L1
+// records add 6 per pair.  So the L1 data pipe, ~3.6 ms of the 5.48, is this pass's floor (staging the gathered
+// rows in shared memory like window.cu does not fit: a 64-atom tile's window at K = 12 is 69 KB); prefetch.global.L1
 // of the next neighbour's rows: 5.66 ms.  At 10^8 atoms the pass reads 1.4 x its algorithmic bytes from DRAM: a
 // neighbour's rows are used again one lattice row (20 000 atoms, two grid strides) later, at the edge of what L2
 // keeps; an L2 evict-first policy on the streamed prev / y rows changes neither bytes nor time, a tile-major
