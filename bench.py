@@ -392,8 +392,8 @@ def run_ours(args):
     flops_per_launch = None
     plain_per_atom = per_atom
     packed = state.get("packed")
-    if packed is not None:   # one 16-byte word per row (+ the diagonal array when K = 4), + the vectors
-        per_atom = 16 + (8 if packed.diag is not None else 0) + 48 * w.R
+    if packed is not None:   # one 16-byte (short rows: 8-byte) word per row (+ the diagonal array when K = 4), + the vectors
+        per_atom = (8 if packed.short_rows else 16) + (8 if packed.diag is not None else 0) + 48 * w.R
     rep9 = ORBITALS == "spd" and REP != "scalar"
     if rep9 and REP == "blocks":   # per ATOM: K x (column + 81 values) + 9 onsite + 9 orbital rows of vectors; / 9 per row
         per_atom = (H.width * (4 + 648) + 72 + 9 * 48 * w.R) / 9.0
@@ -414,8 +414,8 @@ def run_ours(args):
     windowed = state.get("windowed")
     if rep9 or packed is not None or windowed is not None:
         small = False
-    k7_name = ("cheb_packed_kernel (K7x2p: fused Chebyshev pass on packed rows, 16-bit relative columns + value "
-               "dictionary of %d entries, two elements in flight per thread)" % packed.n_values
+    k7_name = ("cheb_packed_kernel (K7x2p: fused Chebyshev pass on packed rows of %d bytes, 16-bit relative columns + value "
+               "dictionary of %d entries, two elements in flight per thread)" % (8 if packed.short_rows else 16, packed.n_values)
                if packed is not None else
                "cheb_window_kernel (K7w: fused Chebyshev pass on windowed tiles, phi_n gathered from shared memory; "
                "largest window %d blocks)" % windowed.blocks if windowed is not None else

@@ -403,6 +403,9 @@ int gtb_spd_bounds(const gtb_ell* H, int32_t mode, double* lo_hi, void* ws, size
  * (ring distance) and a 16-bit index into a dictionary of the distinct fp64 hopping values (lossless);
  * with K <= 3 the fourth slot carries the dictionary index of the onsite energy.  H then costs 16 bytes per
  * atom and pass instead of 12 K + 8 [diag]: config 5 132 -> 112, config 4 428 -> 400 bytes per atom.
+ * SHORT rows: with K <= 3 and at most 16 distinct values (hoppings and onsite energies together) a row is ONE
+ * 8-byte word, three 16-bit offsets and four 4-bit dictionary indices: config 5 132 -> 104 bytes per atom.
+ * gtb_pack_ell picks the format; on return P->width = K | 0x100 for short rows (the pass reads the flag).
  *   P->n = H->n, P->width = H->width, P->cols = caller-allocated DEVICE block of gtb_packed_rows_bytes(n)
  *   bytes (16-byte aligned) receiving the packed rows, P->vals = caller-allocated DEVICE block of
  *   gtb_packed_dict_bytes() bytes receiving a 256-byte header and the dictionary; on return P->diag = NULL,

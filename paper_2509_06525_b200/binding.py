@@ -743,7 +743,7 @@ def kpm_moments_strips(H: Ell, n_strips: int, a: float, b: float, M: int, R_tota
 
 def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:
     """The packed form of a narrow matrix (K <= 4) for mode=MODE_PACKED: `cols` holds the 16-byte packed rows
-    (int32 [n][4]), `vals` the header + value dictionary.  None when the matrix does not fit the format
+    (int32 [n][4]; `short_rows`: 8-byte rows in its first half), `vals` the header + value dictionary.  None when the matrix does not fit the format
     (GTB_ERR_NOT_PACKABLE): stay on the plain path."""
     L = lib()
     for name in ("gtb_pack_workspace_bytes", "gtb_packed_dict_bytes"):
@@ -765,6 +765,8 @@ def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:
     if pc.diag:                      # K = 4 with a diagonal: the array is still read
         P.diag = H.diag
     P.n_values = int(nv.value)
+    P.width = int(pc.width)          # K | 0x100: 8-byte rows (K <= 3 and at most 16 distinct values)
+    P.short_rows = bool(P.width & 0x100)
     return P
 
 

@@ -9,6 +9,10 @@
 //   config 4:  12*3 + 8 + 384 = 428  ->  16 + 384 = 400                      (-6.5 %)
 // A matrix that does not fit (an offset beyond +-32767 rows, more than 65535 distinct values -- any beta != 0
 // model) is reported as GTB_ERR_NOT_PACKABLE and stays on the plain path.
+// SHORT rows: with K <= 3 and at most 16 distinct values (hoppings and onsite energies together) the row is ONE
+// 8-byte word -- three 16-bit offsets and four 4-bit dictionary indices (slot 3: the onsite energy):
+//   config 5:  132  ->  8 + 96 = 104 bytes per atom and pass  (-21 %)
+// gtb_pack_ell picks the format and says so in P->width (bit 8).
 //
 // K7x2p is K7x2 (two elements in flight per thread) reading this word: same values, same slot order, same
 // arithmetic per element, so the vectors are bit-identical to the plain path's.
@@ -26,6 +30,8 @@ constexpr int kMaxValues = 65535;
 constexpr int kHeaderWords = 32;                     // blob: 32 words of header, then the dictionary
 constexpr uint64_t kMagic = 0x4754425041434B31ull;   // "GTBPACK1"
 constexpr int kSmemValues = 1024;
+constexpr int kShortFlag = 0x100;                   // in P->width: 8-byte rows
+constexpr int kShortValues = 16;                    // ... need 4-bit dictionary indices
 
 __device__ __forceinline__ uint32_t hash_slot(uint64_t key) {
   key ^= key >> 33;
@@ -115,7 +121,8 @@ __global__ void __launch_bounds__(kIndexThreads) hash_index_kernel(const unsigne
   }
 }
 
-// one thread per row: four (offset, index) pairs
+// one thread per row: four (offset, index) pairs; kShort: three offsets and four 4-bit indices in 8 bytes
+template <bool kShort>
 __global__ void __launch_bounds__(kBlock) pack_rows_kernel(const int32_t* __restrict__ cols,
                                                            const double* __restrict__ vals,
                                                            const double* __restrict__ diag, int64_t n, int32_t K,
@@ -130,15 +137,20 @@ __global__ void __launch_bounds__(kBlock) pack_rows_kernel(const int32_t* __rest
       if (2 * d <= -n) d += n;
       const int32_t id = hash_find(table, index, (uint64_t)__double_as_longlong(vals[(size_t)k * n + i]));
       if (d < -32768 || d > 32767) atomicOr(flags + 1, 1);
-      if (id < 0 || id > kMaxValues) atomicOr(flags + 1, 2);
+      if (id < 0 || id > kMaxValues || (kShort && id >= kShortValues)) atomicOr(flags + 1, 2);
       w[k] = ((uint32_t)id << 16) | ((uint32_t)d & 0xffffu);
     }
     if (diag && K <= 3) {
       const int32_t id = hash_find(table, index, (uint64_t)__double_as_longlong(diag[i]));
-      if (id < 0 || id > kMaxValues) atomicOr(flags + 1, 2);
+      if (id < 0 || id > kMaxValues || (kShort && id >= kShortValues)) atomicOr(flags + 1, 2);
       w[3] = (uint32_t)id << 16;
     }
-    rows[i] = make_uint4(w[0], w[1], w[2], w[3]);
+    if (kShort) {
+      const uint32_t ids = (w[0] >> 16) | ((w[1] >> 16) << 4) | ((w[2] >> 16) << 8) | ((w[3] >> 16) << 12);
+      reinterpret_cast<uint2*>(rows)[i] = make_uint2((w[0] & 0xffffu) | (w[1] << 16), (w[2] & 0xffffu) | (ids << 16));
+    } else {
+      rows[i] = make_uint4(w[0], w[1], w[2], w[3]);
+    }
   }
 }
 
@@ -149,6 +161,11 @@ __global__ void pack_header_kernel(const int32_t* flags, int32_t diag_in_slot, d
   h[2] = (unsigned long long)diag_in_slot;
 }
 
+__device__ __forceinline__ uint2 ld_stream_u2(const uint2* p) {
+  uint2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
 __device__ __forceinline__ uint4 ld_stream_u4(const uint4* p) {
   uint4 v;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
@@ -160,8 +177,10 @@ __device__ __forceinline__ uint4 ld_stream_u4(const uint4* p) {
 // ---- K7x2p ------------------------------------------------------------------------------------------
 // kDiagArr: the diagonal is a separate fp64 array (K = 4 with a diagonal); otherwise header word 2 says
 // whether slot 3 carries the dictionary index of the onsite energy (K <= 3) or there is no diagonal
-template <int LOG2T, bool kFirst, bool kDiagArr, int W, int kMode>
+// kShort: 8-byte rows (W = 3, no diagonal array)
+template <int LOG2T, bool kFirst, bool kDiagArr, int W, int kMode, bool kShort = false>
 __global__ void __launch_bounds__(kBlock) cheb_packed_kernel(const StepArgs a) {
+  static_assert(!kShort || (W == 3 && !kDiagArr), "short rows: K <= 3, diagonal folded");
   constexpr int VW = 4;
   constexpr int T = 1 << LOG2T;
   constexpr int NE = 2;
@@ -196,7 +215,14 @@ __global__ void __launch_bounds__(kBlock) cheb_packed_kernel(const StepArgs a) {
       own[r] = load_gather<VW>(a.phi_cur + e[r] * VW);
       if (kDotL) with[r] = load_stream<VW>(a.dot_with + e[r] * VW);
       if (kAxpy) with[r] = load_stream<VW>(a.axpy_acc + e[r] * VW);
-      pk[r] = ld_stream_u4(rows + row[r]);
+      if (kShort) {   // expanded to the long form's four words: the decode below is shared
+        const uint2 q = ld_stream_u2(reinterpret_cast<const uint2*>(rows) + row[r]);
+        const uint32_t ids = q.y >> 16;
+        pk[r] = make_uint4((q.x & 0xffffu) | ((ids & 15u) << 16), (q.x >> 16) | (((ids >> 4) & 15u) << 16),
+                           (q.y & 0xffffu) | (((ids >> 8) & 15u) << 16), (ids >> 12) << 16);
+      } else {
+        pk[r] = ld_stream_u4(rows + row[r]);
+      }
     }
     double dg[NE];
 #pragma unroll
@@ -256,23 +282,24 @@ __global__ void __launch_bounds__(kBlock) cheb_packed_kernel(const StepArgs a) {
   block_store_sums<kBlock>(s1, s2, a.partial + blockIdx.x);
 }
 
-template <int LOG2T, bool DIAG, int W>
+template <int LOG2T, bool DIAG, int W, bool SHORT = false>
 void pick_packed_mode(int mode, StepPlan* p) {
   if (mode == 2) {
-    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 2>;
-    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 2>;
+    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 2, SHORT>;
+    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 2, SHORT>;
   } else if (mode == 1) {
-    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 1>;
-    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 1>;
+    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 1, SHORT>;
+    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 1, SHORT>;
   } else {
-    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 0>;
-    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 0>;
+    p->first = cheb_packed_kernel<LOG2T, true, DIAG, W, 0, SHORT>;
+    p->next = cheb_packed_kernel<LOG2T, false, DIAG, W, 0, SHORT>;
   }
 }
 
 template <int LOG2T>
-void pick_packed(bool diag_array, int width, int mode, StepPlan* p) {
-  if (width <= 3) pick_packed_mode<LOG2T, false, 3>(mode, p);
+void pick_packed(bool diag_array, int width, bool short_rows, int mode, StepPlan* p) {
+  if (short_rows) pick_packed_mode<LOG2T, false, 3, true>(mode, p);
+  else if (width <= 3) pick_packed_mode<LOG2T, false, 3>(mode, p);
   else if (diag_array) pick_packed_mode<LOG2T, true, 4>(mode, p);
   else pick_packed_mode<LOG2T, false, 4>(mode, p);
 }
@@ -300,16 +327,19 @@ int grid_for(int64_t total) {
 
 }  // namespace
 
-// plan of the packed pass; P->width = K (1..4), P->diag != NULL only for K = 4 with a diagonal
+// plan of the packed pass; P->width = K (1..4) | kShortFlag for 8-byte rows, P->diag != NULL only for K = 4 with a
+// diagonal
 bool make_plan_packed(const gtb_ell* P, int R, int mode, StepPlan* p) {
-  if (P->width < 1 || P->width > 4 || (R != 2 && R != 4 && R != 8) || !P->cols || !P->vals ||
-      (reinterpret_cast<uintptr_t>(P->cols) & 15u) || mode < 0 || mode > 2)
+  const int K = P->width & 0xff;
+  const bool short_rows = (P->width & kShortFlag) != 0;
+  if ((P->width & ~(0xff | kShortFlag)) || K < 1 || K > 4 || (short_rows && K > 3) || (R != 2 && R != 4 && R != 8) ||
+      !P->cols || !P->vals || (reinterpret_cast<uintptr_t>(P->cols) & 15u) || mode < 0 || mode > 2)
     return false;
-  if (P->diag && P->width <= 3) return false;   // gtb_pack_ell folds the diagonal into slot 3 for K <= 3
+  if (P->diag && K <= 3) return false;   // gtb_pack_ell folds the diagonal into slot 3 for K <= 3
   const bool diag = P->diag != nullptr;
-  if (R == 2) { pick_packed<0>(diag, P->width, mode, p); p->T = 1; }
-  else if (R == 4) { pick_packed<1>(diag, P->width, mode, p); p->T = 2; }
-  else { pick_packed<2>(diag, P->width, mode, p); p->T = 4; }
+  if (R == 2) { pick_packed<0>(diag, K, short_rows, mode, p); p->T = 1; }
+  else if (R == 4) { pick_packed<1>(diag, K, short_rows, mode, p); p->T = 2; }
+  else { pick_packed<2>(diag, K, short_rows, mode, p); p->T = 4; }
   p->vw = 4;
   p->stages = 0;
   p->block = 0;
@@ -360,10 +390,15 @@ extern "C" int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_by
   GTB_CUDA_TRY(cudaMemcpyAsync(flags, w.flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
   GTB_CUDA_TRY(cudaStreamSynchronize(st));
   if (flags[1] || flags[0] > kMaxValues) return GTB_ERR_NOT_PACKABLE;
+  const bool short_rows = H->width <= 3 && flags[0] <= kShortValues;
   hash_index_kernel<<<1, kIndexThreads, 0, st>>>(w.table, w.index, P->vals + kHeaderWords);
   GTB_LAUNCHED();
-  pack_rows_kernel<<<grid_for(n), kBlock, 0, st>>>(H->cols, H->vals, fold_diag ? H->diag : nullptr, n, H->width,
-                                                  w.table, w.index, reinterpret_cast<uint4*>(P->cols), w.flags);
+  if (short_rows)
+    pack_rows_kernel<true><<<grid_for(n), kBlock, 0, st>>>(H->cols, H->vals, fold_diag ? H->diag : nullptr, n, H->width,
+                                                          w.table, w.index, reinterpret_cast<uint4*>(P->cols), w.flags);
+  else
+    pack_rows_kernel<false><<<grid_for(n), kBlock, 0, st>>>(H->cols, H->vals, fold_diag ? H->diag : nullptr, n, H->width,
+                                                           w.table, w.index, reinterpret_cast<uint4*>(P->cols), w.flags);
   GTB_LAUNCHED();
   pack_header_kernel<<<1, 1, 0, st>>>(w.flags, fold_diag ? 1 : 0, P->vals);
   GTB_LAUNCHED();
@@ -371,6 +406,7 @@ extern "C" int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_by
   GTB_CUDA_TRY(cudaStreamSynchronize(st));
   if (flags[1]) return GTB_ERR_NOT_PACKABLE;
   P->diag = fold_diag ? nullptr : H->diag;
+  P->width = H->width | (short_rows ? kShortFlag : 0);
   if (n_values) *n_values = flags[0];
   return GTB_OK;
 }

@@ -39,7 +39,9 @@ def test_packed_pass_is_bit_identical_to_the_plain_pass_and_matches_the_oracle(k
     inp = W.make_inputs(w)
     Ho, Hg = _both(w, inp, width=width, with_diag=diag)
     P = gtb.pack_ell(Hg)
-    assert P is not None and P.width == Ho.width
+    assert P is not None and (P.width & 0xff) == Ho.width
+    # 8-byte rows when K <= 3 and the dictionary has at most 16 entries, else 16-byte rows
+    assert P.short_rows == (Ho.width <= 3 and P.n_values <= 16) and P.short_rows == bool(P.width & 0x100)
     assert (P.diag is None) == (not diag or Ho.width <= 3)
     if kw.get("beta"):
         assert P.n_values > 1024                       # dictionary read from global memory
