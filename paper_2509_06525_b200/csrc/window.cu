@@ -17,6 +17,7 @@
 // no padding slot is involved.
 // A tile whose columns need more than kMaxBlocks blocks makes the matrix GTB_ERR_NOT_PACKABLE: K7t stays.
 #include <algorithm>
+#include <type_traits>
 
 #include "tma.cuh"
 #include "vecload.cuh"
@@ -290,23 +291,31 @@ cheb_window_kernel(const StepArgs a, const int nstages) {
     const double* sv = reinterpret_cast<const double*>(st + L.vals_off) + rl;
     const uint32_t win = smem_u32(st) + L.tile_bytes + (uint32_t)t * 32;
     if (live) {
-      for (int k0 = 0; k0 < kt; k0 += CH) {
-        double v[CH];
-        Vec<VW> x[CH];
+      // kt is the tile's own slot count (uniform over the CTA): whole chunks of CH gathers in flight, then the
+      // remainder in chunks of 4, 2, 1 -- no gather is issued for a slot beyond kt (with every chunk padded to CH,
+      // kt = 20 cost 24 gathers: a sixth of the shared-memory wavefronts of the pass)
+      auto chunk = [&](auto width, int k0) {
+        constexpr int N = decltype(width)::value;
+        double v[N];
+        Vec<VW> x[N];
 #pragma unroll
-        for (int j = 0; j < CH; ++j) {
-          const bool ok = k0 + j < kt;
-          const uint32_t c = ok ? sc[(k0 + j) * TR] : 0u;
-          v[j] = ok ? sv[(k0 + j) * TR] : 0.0;
+        for (int j = 0; j < N; ++j) {
+          const uint32_t c = sc[(k0 + j) * TR];
+          v[j] = sv[(k0 + j) * TR];
           const uint32_t at = win + c * kRowBytes;
           const double2 p = lds_f64x2(at + first_half), q2 = lds_f64x2(at + second_half);
           x[j].v[0] = p.x; x[j].v[1] = p.y; x[j].v[2] = q2.x; x[j].v[3] = q2.y;
         }
 #pragma unroll
-        for (int j = 0; j < CH; ++j)
+        for (int j = 0; j < N; ++j)
 #pragma unroll
           for (int q = 0; q < VW; ++q) acc.v[q] = fma(v[j], x[j].v[q], acc.v[q]);
-      }
+      };
+      int k0 = 0;
+      for (; k0 + CH <= kt; k0 += CH) chunk(std::integral_constant<int, CH>{}, k0);
+      if (kt - k0 >= 4) { chunk(std::integral_constant<int, 4>{}, k0); k0 += 4; }
+      if (kt - k0 >= 2) { chunk(std::integral_constant<int, 2>{}, k0); k0 += 2; }
+      if (kt - k0 >= 1) chunk(std::integral_constant<int, 1>{}, k0);
     }
     double dg = 0.0;
     if (kDiag) dg = reinterpret_cast<const double*>(st + L.diag_off)[rl];
