@@ -192,7 +192,7 @@ cheb_window_kernel(const StepArgs a, const int nstages) {
   constexpr int TR = CT / T;
   constexpr int G = kBlockBytes / (R * 16);
   constexpr uint32_t kRowBytes = R * 16;
-  constexpr int CH = 6;
+  constexpr int CH = R == 8 ? 4 : 5;   // gathers in flight per chunk (A/B on one box: 4 / 5 / 6 / 7 -> c2 0.138 / 0.141 / 0.141 / 0.141 ms, c3 0.950 / 0.943 / 0.957 / 0.955)
   constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   extern __shared__ __align__(128) unsigned char smem[];
   const int64_t n = a.n;
