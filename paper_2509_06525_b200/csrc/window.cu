@@ -61,6 +61,7 @@ __host__ __device__ inline WinLayout win_layout(int64_t n, int K, int R, bool di
 
 // ---- build: one CTA per tile ---------------------------------------------------------------------------
 constexpr int kSetSize = 2048;
+constexpr int kPairSlots = 48;   // widest matrix whose slots are re-ordered for R = 4 (local arrays of the builder)
 
 __global__ void __launch_bounds__(kWinThreads) window_build_kernel(const int32_t* __restrict__ cols,
                                                                    const double* __restrict__ vals,
@@ -148,6 +149,54 @@ __global__ void __launch_bounds__(kWinThreads) window_build_kernel(const int32_t
     if (diag) {
       double* td = reinterpret_cast<double*>(rec + L.diag_off);
       for (int rl = threadIdx.x; rl < L.TR; rl += kWinThreads) td[rl] = rl < rows ? diag[row0 + rl] : 0.0;
+    }
+    __syncthreads();
+    // R = 4: a gathered neighbour is 64 bytes = half of the 32 banks, read by the row's two threads with two
+    // LDS.128, and a quarter-warp holds four rows.  Rows rl and rl + 2 read the same halves of their elements in
+    // the same step (the half-swap of the pass separates rl from rl + 1), so they collide whenever their window
+    // indices have the same parity: 45 % of the shared-memory wavefronts of the pass at c3 were such conflicts
+    // (profiles/r02_wide_k7w.md).  The order of a row's slots is free, so the two rows of such a pair get their
+    // slots re-ordered here until, position by position, one index is even and the other odd; what cannot be
+    // matched meets a padding slot (value 0) of the opposite parity while the tile's slot count allows, and only
+    // the rest stays same-parity.  The sum over a row's slots then runs in another order than the ELL's: the
+    // vectors equal K7t's to rounding, no longer bit for bit.
+    if (R == 4 && K <= kPairSlots && kt > 0) {
+      for (int p = threadIdx.x; p < L.TR / 2; p += kWinThreads) {
+        const int a = 4 * (p >> 1) + (p & 1), b = a + 2;
+        double va[kPairSlots], vb[kPairSlots];
+        uint16_t ia[kPairSlots], ib[kPairSlots];
+        unsigned char ae[kPairSlots], ao[kPairSlots], be[kPairSlots], bo[kPairSlots];
+        int nae = 0, nao = 0, nbe = 0, nbo = 0;
+        for (int k = 0; k < K; ++k) {
+          va[k] = tv[k * L.TR + a]; ia[k] = tc[k * L.TR + a];
+          vb[k] = tv[k * L.TR + b]; ib[k] = tc[k * L.TR + b];
+          if (va[k] != 0.0) { if (ia[k] & 1) ao[nao++] = (unsigned char)k; else ae[nae++] = (unsigned char)k; }
+          if (vb[k] != 0.0) { if (ib[k] & 1) bo[nbo++] = (unsigned char)k; else be[nbe++] = (unsigned char)k; }
+        }
+        int pos = 0;
+        auto put = [&](int ka, int kb, int pad_a, int pad_b) {   // k < 0: a padding slot of the given parity
+          tv[pos * L.TR + a] = ka >= 0 ? va[ka] : 0.0;
+          tc[pos * L.TR + a] = ka >= 0 ? ia[ka] : (uint16_t)pad_a;
+          tv[pos * L.TR + b] = kb >= 0 ? vb[kb] : 0.0;
+          tc[pos * L.TR + b] = kb >= 0 ? ib[kb] : (uint16_t)pad_b;
+          ++pos;
+        };
+        const int n1 = min(nae, nbo), n2 = min(nao, nbe);
+        for (int i = 0; i < n1; ++i) put(ae[i], bo[i], 0, 0);
+        for (int i = 0; i < n2; ++i) put(ao[i], be[i], 0, 0);
+        // leftovers: A's (even ones first), B's (odd ones first); at most one kind on each side meets its like
+        unsigned char la[kPairSlots], lb[kPairSlots];
+        int nla = 0, nlb = 0;
+        for (int i = n1; i < nae; ++i) la[nla++] = ae[i];
+        for (int i = n2; i < nao; ++i) la[nla++] = ao[i];
+        for (int i = n2; i < nbe; ++i) lb[nlb++] = be[i];
+        for (int i = n1; i < nbo; ++i) lb[nlb++] = bo[i];
+        const int merges = max(0, nla + nlb - (kt - pos));   // same-parity meetings that the slot count forces
+        for (int i = 0; i < merges; ++i) put(la[i], lb[i], 0, 0);
+        for (int i = merges; i < nla; ++i) put(la[i], -1, 0, (ia[la[i]] & 1) ^ 1);
+        for (int i = merges; i < nlb; ++i) put(-1, lb[i], (ib[lb[i]] & 1) ^ 1, 0);
+        while (pos < kt) put(-1, -1, 0, 1);
+      }
     }
     __syncthreads();
   }
