@@ -425,6 +425,9 @@ int gtb_pack_ell(const gtb_ell* H, gtb_ell* P, void* ws, size_t ws_bytes, void* 
  * into that window, the tile's own slot count (longest row of the tile), and its hoppings / diagonal /
  * columns contiguous.  The pass (gtb_kpm_moments / gtb_kpm_step with mode | GTB_MODE_WINDOW, R_batch = R,
  * R_total a multiple of R) copies window and tile into shared memory with bulk copies and gathers from there.
+ * At R = 4 the slots of row pairs are stored in another order than the ELL's (so that the two rows' window indices
+ * differ in parity position by position: no shared-memory bank conflicts between them); the sums over a row then run
+ * in that order and the vectors equal the plain pass's to rounding, not bit for bit.  R = 2 and R = 8 keep the order.
  *   Wd->n = H->n, Wd->width = H->width, Wd->vals = caller-allocated DEVICE block of
  *   gtb_window_bytes(n, width, R, H->diag != NULL) bytes (128-byte aligned); on return Wd->cols = H->cols
  *   (unused), Wd->diag = H->diag (only its presence matters: the values are in the tiles) and Wd->width =
