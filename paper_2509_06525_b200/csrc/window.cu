@@ -61,6 +61,7 @@ __host__ __device__ inline WinLayout win_layout(int64_t n, int K, int R, bool di
 
 // ---- build: one CTA per tile ---------------------------------------------------------------------------
 constexpr int kSetSize = 2048;
+constexpr int kSwapWord = 44;     // tile header word of the swap bits (after n_blocks, K_t, 2 spare words, 40 block ids)
 constexpr int kPairSlots = 48;   // widest matrix whose slots are re-ordered for R = 4 (local arrays of the builder)
 
 __global__ void __launch_bounds__(kWinThreads) window_build_kernel(const int32_t* __restrict__ cols,
@@ -73,6 +74,7 @@ __global__ void __launch_bounds__(kWinThreads) window_build_kernel(const int32_t
   __shared__ int32_t s_set[kSetSize];
   __shared__ int32_t s_list[kMaxBlocks], s_sorted[kMaxBlocks];
   __shared__ int32_t s_count, s_kt;
+  __shared__ uint32_t s_swap[8];   // bit per row of the tile: the row reads the halves of its elements in swapped order
   for (int64_t tile = blockIdx.x; tile < L.n_tiles; tile += gridDim.x) {
     const int64_t row0 = tile * L.TR;
     const int rows = (int)min((int64_t)L.TR, n - row0);
@@ -152,52 +154,84 @@ __global__ void __launch_bounds__(kWinThreads) window_build_kernel(const int32_t
     }
     __syncthreads();
     // R = 4: a gathered neighbour is 64 bytes = half of the 32 banks, read by the row's two threads with two
-    // LDS.128, and a quarter-warp holds four rows.  Rows rl and rl + 2 read the same halves of their elements in
-    // the same step (the half-swap of the pass separates rl from rl + 1), so they collide whenever their window
-    // indices have the same parity: 45 % of the shared-memory wavefronts of the pass at c3 were such conflicts
-    // (profiles/r02_wide_k7w.md).  The order of a row's slots is free, so the two rows of such a pair get their
+    // LDS.128, and a quarter-warp holds four rows.  Two rows that read the same halves of their elements in the
+    // same step (the same swap bit) collide whenever their window indices have the same parity: with the fixed
+    // pattern "odd rows swap" 45 % of the shared-memory wavefronts of the pass at c3 were such conflicts
+    // (profiles/r02_wide_k7w.md).  The order of a row's slots is free, so the two rows sharing a swap bit get their
     // slots re-ordered here until, position by position, one index is even and the other odd; what cannot be
     // matched meets a padding slot (value 0) of the opposite parity while the tile's slot count allows, and only
     // the rest stays same-parity.  The sum over a row's slots then runs in another order than the ELL's: the
     // vectors equal K7t's to rounding, no longer bit for bit.
+    // Which two rows of a quarter-warp read the same halves in the same step is the tile's choice (one bit per
+    // row in the header, read by the pass): of the three ways to pair four rows the builder takes the one whose
+    // slot counts leave the fewest same-parity meetings -- on a lattice the even / odd counts of a row follow its
+    // sublattice, and the fixed pairing (rl, rl + 2) met its like in a third of the positions at c3.
+    if (threadIdx.x < 8) s_swap[threadIdx.x] = 0xAAAAAAAAu;   // default: odd rows swap (what R = 2 and R = 8 use)
+    __syncthreads();
     if (R == 4 && K <= kPairSlots && kt > 0) {
-      for (int p = threadIdx.x; p < L.TR / 2; p += kWinThreads) {
-        const int a = 4 * (p >> 1) + (p & 1), b = a + 2;
-        double va[kPairSlots], vb[kPairSlots];
-        uint16_t ia[kPairSlots], ib[kPairSlots];
-        unsigned char ae[kPairSlots], ao[kPairSlots], be[kPairSlots], bo[kPairSlots];
-        int nae = 0, nao = 0, nbe = 0, nbo = 0;
-        for (int k = 0; k < K; ++k) {
-          va[k] = tv[k * L.TR + a]; ia[k] = tc[k * L.TR + a];
-          vb[k] = tv[k * L.TR + b]; ib[k] = tc[k * L.TR + b];
-          if (va[k] != 0.0) { if (ia[k] & 1) ao[nao++] = (unsigned char)k; else ae[nae++] = (unsigned char)k; }
-          if (vb[k] != 0.0) { if (ib[k] & 1) bo[nbo++] = (unsigned char)k; else be[nbe++] = (unsigned char)k; }
-        }
-        int pos = 0;
-        auto put = [&](int ka, int kb, int pad_a, int pad_b) {   // k < 0: a padding slot of the given parity
-          tv[pos * L.TR + a] = ka >= 0 ? va[ka] : 0.0;
-          tc[pos * L.TR + a] = ka >= 0 ? ia[ka] : (uint16_t)pad_a;
-          tv[pos * L.TR + b] = kb >= 0 ? vb[kb] : 0.0;
-          tc[pos * L.TR + b] = kb >= 0 ? ib[kb] : (uint16_t)pad_b;
-          ++pos;
+      for (int quad = threadIdx.x; quad < L.TR / 4; quad += kWinThreads) {
+        double v4[4][kPairSlots];
+        uint16_t i4[4][kPairSlots];
+        int ne[4] = {0, 0, 0, 0}, no[4] = {0, 0, 0, 0};
+        for (int r = 0; r < 4; ++r)
+          for (int k = 0; k < K; ++k) {
+            v4[r][k] = tv[k * L.TR + 4 * quad + r];
+            i4[r][k] = tc[k * L.TR + 4 * quad + r];
+            if (v4[r][k] != 0.0) { if (i4[r][k] & 1) ++no[r]; else ++ne[r]; }
+          }
+        auto meetings = [&](int x, int y) {   // same-parity positions the slot count forces on the pair (x, y)
+          const int n1 = min(ne[x], no[y]), n2 = min(no[x], ne[y]);
+          return max(0, (ne[x] + no[x] - n1 - n2) + (ne[y] + no[y] - n1 - n2) - (kt - n1 - n2));
         };
-        const int n1 = min(nae, nbo), n2 = min(nao, nbe);
-        for (int i = 0; i < n1; ++i) put(ae[i], bo[i], 0, 0);
-        for (int i = 0; i < n2; ++i) put(ao[i], be[i], 0, 0);
-        // leftovers: A's (even ones first), B's (odd ones first); at most one kind on each side meets its like
-        unsigned char la[kPairSlots], lb[kPairSlots];
-        int nla = 0, nlb = 0;
-        for (int i = n1; i < nae; ++i) la[nla++] = ae[i];
-        for (int i = n2; i < nao; ++i) la[nla++] = ao[i];
-        for (int i = n2; i < nbe; ++i) lb[nlb++] = be[i];
-        for (int i = n1; i < nbo; ++i) lb[nlb++] = bo[i];
-        const int merges = max(0, nla + nlb - (kt - pos));   // same-parity meetings that the slot count forces
-        for (int i = 0; i < merges; ++i) put(la[i], lb[i], 0, 0);
-        for (int i = merges; i < nla; ++i) put(la[i], -1, 0, (ia[la[i]] & 1) ^ 1);
-        for (int i = merges; i < nlb; ++i) put(-1, lb[i], (ib[lb[i]] & 1) ^ 1, 0);
-        while (pos < kt) put(-1, -1, 0, 1);
+        const int cost0 = meetings(0, 2) + meetings(1, 3), cost1 = meetings(0, 1) + meetings(2, 3),
+                  cost2 = meetings(0, 3) + meetings(1, 2);
+        int pa[2], pb[2];
+        uint32_t bits;   // bit r: row r of the quad swaps its halves; partners share the bit
+        if (cost0 <= cost1 && cost0 <= cost2) { pa[0] = 0; pb[0] = 2; pa[1] = 1; pb[1] = 3; bits = 0xAu; }
+        else if (cost1 <= cost2) { pa[0] = 0; pb[0] = 1; pa[1] = 2; pb[1] = 3; bits = 0xCu; }
+        else { pa[0] = 0; pb[0] = 3; pa[1] = 1; pb[1] = 2; bits = 0x6u; }
+        const int word = (4 * quad) >> 5, shift = (4 * quad) & 31;
+        atomicAnd(&s_swap[word], ~(0xFu << shift));
+        atomicOr(&s_swap[word], bits << shift);
+        for (int h = 0; h < 2; ++h) {
+          const int ra = pa[h], rb = pb[h];
+          const int a = 4 * quad + ra, b = 4 * quad + rb;
+          const double *va = v4[ra], *vb = v4[rb];
+          const uint16_t *ia = i4[ra], *ib = i4[rb];
+          unsigned char ae[kPairSlots], ao[kPairSlots], be[kPairSlots], bo[kPairSlots];
+          int nae = 0, nao = 0, nbe = 0, nbo = 0;
+          for (int k = 0; k < K; ++k) {
+            if (va[k] != 0.0) { if (ia[k] & 1) ao[nao++] = (unsigned char)k; else ae[nae++] = (unsigned char)k; }
+            if (vb[k] != 0.0) { if (ib[k] & 1) bo[nbo++] = (unsigned char)k; else be[nbe++] = (unsigned char)k; }
+          }
+          int pos = 0;
+          auto put = [&](int ka, int kb, int pad_a, int pad_b) {   // k < 0: a padding slot of the given parity
+            tv[pos * L.TR + a] = ka >= 0 ? va[ka] : 0.0;
+            tc[pos * L.TR + a] = ka >= 0 ? ia[ka] : (uint16_t)pad_a;
+            tv[pos * L.TR + b] = kb >= 0 ? vb[kb] : 0.0;
+            tc[pos * L.TR + b] = kb >= 0 ? ib[kb] : (uint16_t)pad_b;
+            ++pos;
+          };
+          const int n1 = min(nae, nbo), n2 = min(nao, nbe);
+          for (int i2 = 0; i2 < n1; ++i2) put(ae[i2], bo[i2], 0, 0);
+          for (int i2 = 0; i2 < n2; ++i2) put(ao[i2], be[i2], 0, 0);
+          // leftovers: A's (even ones first), B's (even ones first): like meets like only when the count forces it
+          unsigned char la[kPairSlots], lb[kPairSlots];
+          int nla = 0, nlb = 0;
+          for (int i2 = n1; i2 < nae; ++i2) la[nla++] = ae[i2];
+          for (int i2 = n2; i2 < nao; ++i2) la[nla++] = ao[i2];
+          for (int i2 = n2; i2 < nbe; ++i2) lb[nlb++] = be[i2];
+          for (int i2 = n1; i2 < nbo; ++i2) lb[nlb++] = bo[i2];
+          const int merges = max(0, nla + nlb - (kt - pos));
+          for (int i2 = 0; i2 < merges; ++i2) put(la[i2], lb[i2], 0, 0);
+          for (int i2 = merges; i2 < nla; ++i2) put(la[i2], -1, 0, (ia[la[i2]] & 1) ^ 1);
+          for (int i2 = merges; i2 < nlb; ++i2) put(-1, lb[i2], (ib[lb[i2]] & 1) ^ 1, 0);
+          while (pos < kt) put(-1, -1, 0, 1);
+        }
       }
     }
+    __syncthreads();
+    if (threadIdx.x < 8) head[kSwapWord + threadIdx.x] = (int32_t)s_swap[threadIdx.x];
     __syncthreads();
   }
 }
@@ -210,7 +244,8 @@ __device__ __forceinline__ double2 lds_f64x2(uint32_t addr) {
   return v;
 }
 
-// Odd rows of a tile keep the two complex numbers of their 256-bit element in swapped order in registers:
+// Rows whose swap bit is set (tile header; the odd rows unless gtb_window_ell chose otherwise at R = 4) keep the
+// two complex numbers of their 256-bit element in swapped order in registers:
 // the two 16-byte halves of a gathered element are read with two LDS.128, and when the row pair sharing a
 // quarter-warp reads opposite halves first, the eight lanes cover all 32 banks (without it: 2-way conflicts,
 // twice the shared-memory wavefronts).  The sums over the element do not depend on the order.
@@ -317,8 +352,6 @@ cheb_window_kernel(const StepArgs a, const int nstages) {
   }
   const int rl = tid >> LOG2T;
   const int t = tid & (T - 1);
-  const bool odd = (rl & 1) != 0;
-  const uint32_t first_half = odd ? 16u : 0u, second_half = odd ? 0u : 16u;
   // (loading the thread's own phi_{n-1} / phi_n elements one tile ahead was measured: no gain for K7w, and K7t
   // loses a third at its 72-register cap)
   for (int64_t i = 0; i < my_tiles; ++i) {
@@ -336,6 +369,9 @@ cheb_window_kernel(const StepArgs a, const int nstages) {
     mbar_wait(bar0 + 8 * s, (uint32_t)((i / nstages) & 1));
     const unsigned char* st = stage0 + (size_t)s * stage_bytes;
     const int kt = reinterpret_cast<const int32_t*>(st)[1];
+    // the row's swap bit of this tile (gtb_window_ell: rows sharing the bit read the same halves in the same step)
+    const bool odd = ((reinterpret_cast<const uint32_t*>(st)[kSwapWord + (rl >> 5)] >> (rl & 31)) & 1u) != 0;
+    const uint32_t first_half = odd ? 16u : 0u, second_half = odd ? 0u : 16u;
     const uint16_t* sc = reinterpret_cast<const uint16_t*>(st + L.cols_off) + rl;
     const double* sv = reinterpret_cast<const double*>(st + L.vals_off) + rl;
     const uint32_t win = smem_u32(st) + L.tile_bytes + (uint32_t)t * 32;
