@@ -330,6 +330,11 @@ def run_ours(args):
             Wd = gtb.window_ell(H, w.R)              # part of the timed step; None: no locality, K7t stays
             if Wd is not None:
                 Hk, kmode, state["windowed"] = Wd, gtb.MODE_WINDOW, Wd
+        state["paired"] = False
+        if Hk is H and ORBITALS == "pz" and w.R == 4 and H.width <= 48:
+            # plain ELL at R = 4: the same matrix with the slots of rows 2q, 2q + 1 alternating in column parity
+            # (gtb_pair_slots: their 64-byte gathers then share an L1 wavefront); part of the timed step
+            Hk, state["paired"] = gtb.pair_slots(H, w.R), True
         gtb.kpm_moments(Hk, a, b, w.M, w.R, w.R, seed, mode=kmode, ws=ws_kpm, mu=mu, opt=opt)
         if "E" not in state:
             state["E"] = torch.from_numpy(W.energy_grid(w, a, b)).to(dev)
@@ -461,7 +466,8 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": w.name, "atoms": n, "orbitals_per_atom": n_orb // n,
                        "ell_width": H.width,
-                       "representation": REP if ORBITALS == "spd" else "packed rows" if packed is not None else "ell",
+                       "representation": REP if ORBITALS == "spd" else "packed rows" if packed is not None else
+                                         "ell, slots paired for R = 4" if state.get("paired") else "ell",
                        "cutoff_A": w.cutoff, "numbering": ("tile-major %dx%d cells" % TILE_NUMBERING) if TILE_NUMBERING else "row-major",
                        "moments": w.M,
                        "vectors": w.R, "energies": w.n_energies, "passes_per_step": (w.M + 1) // 2,
@@ -552,6 +558,8 @@ def run_vac(args):
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
+        if ORBITALS == "pz" and w.R == 4 and H.width <= 48 and not (WINDOW and H.width >= 16) and not (PACK and H.width <= 4):
+            H = gtb.pair_slots(H, w.R)    # plain-ELL passes at R = 4: the same matrix, slots paired for the gathers
         vv = gtb.velocity_ell(H, vpos, inp.box, inp.pbc, 0)
         vopt, state["alt"] = opt, None
         if ORBITALS == "pz" and w.R in (2, 4, 8):   # the fused passes on the compressed form, as the DOS path

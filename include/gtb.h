@@ -439,6 +439,16 @@ size_t gtb_window_bytes(int64_t n, int32_t width, int32_t R, int32_t with_diag);
 int gtb_window_ell(const gtb_ell* H, int32_t R, gtb_ell* Wd, int32_t* scratch, void* stream,
                    int32_t* blocks_needed);
 
+/* ---- the same matrix with its slots in an order the gathers like (north_star (1): the ELL layout leaves the
+ * order of a row's slots free) ----
+ * ASYNC.  Hp (caller-allocated cols / vals of H's shape, distinct from H's; Hp->diag is set to H->diag) receives
+ * the same rows with their entries in another slot order: at R = 4 vectors per pass (a gathered neighbour is half
+ * an L1 line) the slots of rows 2q and 2q + 1 are arranged so that, position by position, one column is even and
+ * the other odd, and the two gathers share one L1 wavefront.  Padding slots stay (column = the row, value 0).  Any
+ * other R, or a width above 48: a plain copy.  Hp is an ordinary gtb_ell for every call of this header; sums over
+ * a row run in the new order, so results equal those on H to rounding, not bit for bit. */
+int gtb_pair_slots(const gtb_ell* H, int32_t R, gtb_ell* Hp, void* stream);
+
 /* ---- Eq. 2 feeding the s,p Slater-Koster blocks: the paper's hopping formula ----
  *   H_ij^{lm,l'm'} = sum_lambda MLP_lambda(e_ij) P_lambda^{lm,l'm'}(r^_ij),   H_ii^{lm,lm} = MLP_{l,alpha}(v_i):
  * MLP_lambda has four outputs, the bond integrals ss_sigma, sp_sigma, pp_sigma, pp_pi of the pair (reading E6),

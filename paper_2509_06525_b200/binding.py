@@ -36,7 +36,7 @@ EXPORTS = (
     "gtb_spd_workspace_bytes", "gtb_spd_hamiltonian", "gtb_spd_bonds_bytes", "gtb_spd_bonds",
     "gtb_spd_blocks", "gtb_spd_bounds_workspace_bytes", "gtb_spd_bounds",
     "gtb_pack_workspace_bytes", "gtb_packed_rows_bytes", "gtb_packed_dict_bytes", "gtb_pack_ell",
-    "gtb_window_bytes", "gtb_window_ell", "gtb_mlp_spd_weight_count", "gtb_mlp_spd_blocks",
+    "gtb_window_bytes", "gtb_window_ell", "gtb_pair_slots", "gtb_mlp_spd_weight_count", "gtb_mlp_spd_blocks",
     "gtb_strip_plan", "gtb_ring_halo", "gtb_strips_workspace_bytes", "gtb_kpm_moments_strips",
     "gtb_mlp_sk_weight_count", "gtb_mlp_sk_hamiltonian", "gtb_carrier_density", "gtb_mobility",
 )
@@ -768,6 +768,15 @@ def pack_ell(H: Ell, ws: Optional[torch.Tensor] = None) -> Optional[Ell]:
     P.width = int(pc.width)          # K | 0x100: 8-byte rows (K <= 3 and at most 16 distinct values)
     P.short_rows = bool(P.width & 0x100)
     return P
+
+
+def pair_slots(H: Ell, R: int) -> Ell:
+    """gtb_pair_slots: the same matrix as a plain ELL with the slots of neighbouring rows ordered for the gathers
+    of an R-vector pass (R = 4: rows 2q, 2q + 1 alternate in column parity); a copy for any other R."""
+    Hp = Ell(H.n, H.width, torch.empty_like(H.cols), torch.empty_like(H.vals), H.diag)
+    hc, pc = H._c(), Hp._c()
+    _check(lib().gtb_pair_slots(C.byref(hc), C.c_int32(R), C.byref(pc), _stream()), "pair_slots")
+    return Hp
 
 
 def window_ell(H: Ell, R: int) -> Optional[Ell]:

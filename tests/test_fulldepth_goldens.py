@@ -1,6 +1,6 @@
 """CPU-side checks of the full-size, full-depth goldens (tests/golden/<cfg>_moments_M*.txt, _dos_G*.txt,
 written by tests/golden/make_fullsize_goldens.py from the oracle alone): they exist for all five
-configs, parse, carry the config's (M, G), satisfy what the mathematics fixes (mu_0 = 1, |mu_n| <= 1,
+configs (and for the variants 2b, 3b), parse, carry the config's (M, G), satisfy what the mathematics fixes (mu_0 = 1, |mu_n| <= 1,
 rho >= 0, int rho dE = 1 within the Jackson resolution) and -- at the 10^6-atom configs, where the
 lattice is cheap to regenerate -- the input digest they were made from."""
 import os
@@ -12,7 +12,7 @@ from paper_2509_06525_b200 import workloads as W
 from test_gpu_fulldepth import KEYS, _paths, read_fulldepth_golden
 
 
-REQUIRED = ("c4", "c2b", "c2", "c5", "c3")        # extended as make_fullsize_goldens.py finishes each config
+REQUIRED = ("c4", "c2b", "c2", "c5", "c3", "c3b")        # extended as make_fullsize_goldens.py finishes each config
 
 
 def test_goldens_exist():

@@ -24,7 +24,7 @@ from paper_2509_06525_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-KEYS = ("c4", "c2b", "c2", "c3", "c5")
+KEYS = ("c4", "c2b", "c2", "c3", "c5", "c3b")
 
 
 def _paths(key):
@@ -72,10 +72,10 @@ def _record(key, **kv):
 _HAVE = [k for k in KEYS if all(os.path.exists(p) for p in _paths(k))]
 
 
-@pytest.mark.parametrize("key,packed", [(k, False) for k in _HAVE] + [(k, True) for k in _HAVE if k in ("c4", "c5", "c2", "c3")])
+@pytest.mark.parametrize("key,packed", [(k, False) for k in _HAVE] + [(k, True) for k in _HAVE if k in ("c4", "c5", "c2", "c3", "c3b")])
 def test_full_size_full_depth_moments_and_dos_match_the_oracle(key, packed):
-    """packed: the same run through the compressed form bench.py times -- packed rows (gtb_pack_ell, K7x2p) at
-    c4 / c5, windowed tiles (gtb_window_ell, K7w) at c2 / c3."""
+    """packed: the same run through the form bench.py times -- packed rows (gtb_pack_ell, K7x2p) at c4 / c5,
+    windowed tiles (gtb_window_ell, K7w) at c2 / c3, the plain ELL with paired slots (gtb_pair_slots) at c3b."""
     w = W.CONFIGS[key]
     g = read_fulldepth_golden(key)
     assert g["mu"].shape == (w.M,) and g["E"].shape == (w.n_energies,)
@@ -96,6 +96,8 @@ def test_full_size_full_depth_moments_and_dos_match_the_oracle(key, packed):
     if packed and H.width <= 4:
         Hk, kmode = gtb.pack_ell(H), gtb.MODE_PACKED
         assert Hk is not None
+    elif packed and H.width < 16:
+        Hk = gtb.pair_slots(H, w.R)
     elif packed:
         Hk, kmode = gtb.window_ell(H, w.R), gtb.MODE_WINDOW
         assert Hk is not None
