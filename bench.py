@@ -322,7 +322,9 @@ def run_ours(args):
         state["packed"] = None
         # (R = 8 narrow rows run K7t faster than the packed pass: c4 0.0703 against 0.0748 ms)
         if PACK and KERNEL == "auto" and ORBITALS == "pz" and H.width <= 4 and w.R in (2, 4) and n * (w.R // 2) > 148 * 8 * 256:
-            P = gtb.pack_ell(H, ws=ws_pack)          # part of the timed step; None: does not fit, plain path
+            # R = 2: first the slots of rows 4q .. 4q + 3 permuted so that the four 32-byte gathers share an L1 wavefront
+            Hs = gtb.pair_slots(H, w.R) if w.R == 2 else H
+            P = gtb.pack_ell(Hs, ws=ws_pack)         # part of the timed step; None: does not fit, plain path
             if P is not None:
                 Hk, kmode, state["packed"] = P, gtb.MODE_PACKED, P
         state["windowed"] = None

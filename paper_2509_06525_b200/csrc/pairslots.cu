@@ -69,6 +69,64 @@ __global__ void __launch_bounds__(kBlock) pair_slots_kernel(const int32_t* __res
   }
 }
 
+// R = 2: a gathered neighbour is 32 bytes, a quarter of a line, and a row has one thread: the gathers of rows
+// 4q .. 4q + 3 share one L1 wavefront when their columns differ in the two low bits (address bits 5 and 6).  In the
+// sorted slot order of a honeycomb lattice they almost never do (2.4 % of the positions at config 5); one
+// permutation of each row's slots, chosen row by row, makes them all differ.  K <= 4: every permutation is tried.
+constexpr int kQuadMaxSlots = 4;
+
+__device__ __forceinline__ void unrank_permutation(int rank, int K, int* perm) {   // lexicographic, K <= 4
+  int pool[kQuadMaxSlots] = {0, 1, 2, 3};
+  int f = 1;
+  for (int i = 2; i < K; ++i) f *= i;   // (K - 1)!
+  for (int i = 0; i < K; ++i) {
+    const int pick = rank / f;
+    rank -= pick * f;
+    perm[i] = pool[pick];
+    for (int j = pick; j < K - 1 - i; ++j) pool[j] = pool[j + 1];
+    if (K - 1 - i > 0) f /= (K - 1 - i);
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) quad_slots_kernel(const int32_t* __restrict__ cols,
+                                                            const double* __restrict__ vals, int64_t n, int32_t K,
+                                                            int32_t* __restrict__ ocols, double* __restrict__ ovals) {
+  const int64_t quads = (n + 3) / 4;
+  int nperm = 1;
+  for (int i = 2; i <= K; ++i) nperm *= i;
+  for (int64_t q = (int64_t)blockIdx.x * kBlock + threadIdx.x; q < quads; q += (int64_t)gridDim.x * kBlock) {
+    int32_t c[4][kQuadMaxSlots];
+    double v[4][kQuadMaxSlots];
+    int chosen[4][kQuadMaxSlots];
+    const int rows = (int)min((int64_t)4, n - 4 * q);
+    for (int r = 0; r < rows; ++r)
+      for (int k = 0; k < K; ++k) {
+        c[r][k] = cols[(size_t)k * n + 4 * q + r];
+        v[r][k] = vals[(size_t)k * n + 4 * q + r];
+      }
+    for (int k = 0; k < K; ++k) chosen[0][k] = k;
+    for (int r = 1; r < rows; ++r) {   // the permutation of row r that clashes least with the rows before it
+      int best = 1 << 30, best_rank = 0;
+      for (int rank = 0; rank < nperm; ++rank) {
+        int perm[kQuadMaxSlots];
+        unrank_permutation(rank, K, perm);
+        int clashes = 0;
+        for (int k = 0; k < K; ++k) {
+          const int mine = c[r][perm[k]] & 3;
+          for (int j = 0; j < r; ++j) clashes += (c[j][chosen[j][k]] & 3) == mine;
+        }
+        if (clashes < best) { best = clashes; best_rank = rank; }
+      }
+      unrank_permutation(best_rank, K, chosen[r]);
+    }
+    for (int r = 0; r < rows; ++r)
+      for (int k = 0; k < K; ++k) {
+        ocols[(size_t)k * n + 4 * q + r] = c[r][chosen[r][k]];
+        ovals[(size_t)k * n + 4 * q + r] = v[r][chosen[r][k]];
+      }
+  }
+}
+
 __global__ void __launch_bounds__(kBlock) copy_slots_kernel(const int32_t* __restrict__ cols,
                                                             const double* __restrict__ vals, int64_t count,
                                                             int32_t* __restrict__ ocols, double* __restrict__ ovals) {
@@ -97,6 +155,10 @@ extern "C" int gtb_pair_slots(const gtb_ell* H, int32_t R, gtb_ell* Hp, void* st
     const int64_t pairs = (n + 1) / 2;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((pairs + kBlock - 1) / kBlock, kMaxGrid));
     pair_slots_kernel<<<grid, kBlock, 0, st>>>(H->cols, H->vals, n, H->width, Hp->cols, Hp->vals);
+  } else if (R == 2 && H->width <= kQuadMaxSlots) {
+    const int64_t quads = (n + 3) / 4;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((quads + kBlock - 1) / kBlock, kMaxGrid));
+    quad_slots_kernel<<<grid, kBlock, 0, st>>>(H->cols, H->vals, n, H->width, Hp->cols, Hp->vals);
   } else {   // nothing to gain (R = 8 gathers whole lines) or too wide for the kernel's local arrays: a copy
     const int64_t count = n * H->width;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((count + kBlock - 1) / kBlock, kMaxGrid));

@@ -66,6 +66,46 @@ def test_paired_slots_are_the_same_matrix_and_run_to_the_oracle(key, nx, ny):
     assert lo2 == pytest.approx(lo, rel=1e-14) and hi2 == pytest.approx(hi, rel=1e-14)
 
 
+@pytest.mark.parametrize("key,nx,ny,diag", [("c5", 57, 43, False), ("c4", 48, 21, True), ("c1", 24, 24, False)])
+def test_quads_of_rows_at_two_vectors_per_pass(key, nx, ny, diag):
+    """R = 2: the slots of rows 4q .. 4q + 3 are permuted so that the four gathered columns differ in their two low
+    bits; same matrix, same results through the plain and the packed pass."""
+    kw = {"stripe": 6} if key == "c4" else {}
+    w = W.CONFIGS[key].scaled(nx, ny, R=2, **kw)
+    inp = W.make_inputs(w)
+    Ho = oracle.build_hamiltonian(inp.pos, inp.species, inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0, w.beta,
+                                  inp.onsite_shift, with_diag=diag)
+    Hg = gtb.build_hamiltonian(_dev(inp.pos), _dev(inp.species), inp.box, inp.pbc, w.cutoff, w.onsite, w.t0, w.r0,
+                               w.beta, _dev(inp.onsite_shift) if inp.onsite_shift is not None else None,
+                               with_diag=diag)
+    Hq = gtb.pair_slots(Hg, 2)
+    n, K = Ho.n, Ho.width
+    assert K <= 4 and n % 4 == 0
+    c0, v0 = Hg.cols.cpu().numpy(), Hg.vals.cpu().numpy()
+    c1, v1 = Hq.cols.cpu().numpy(), Hq.vals.cpu().numpy()
+    o0, o1 = np.lexsort((v0, c0), axis=0), np.lexsort((v1, c1), axis=0)
+    assert np.array_equal(np.take_along_axis(c0, o0, 0), np.take_along_axis(c1, o1, 0))
+    assert np.array_equal(np.take_along_axis(v0, o0, 0), np.take_along_axis(v1, o1, 0))
+
+    def distinct(c):
+        s = np.sort((c & 3).reshape(K, n // 4, 4), axis=2)
+        return float((np.diff(s, axis=2) != 0).all(axis=2).mean())
+    assert distinct(c1) >= 0.95 and distinct(c0) <= 0.2
+    if w.a is not None:
+        a, b = w.a, w.b
+    else:
+        lo, hi = oracle.spectral_bounds(Ho)
+        a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    M, R = 65, 2
+    ref = oracle.kpm_moments(Ho, a, b, M, R, 5, mode=0, algo=0)
+    got = gtb.kpm_moments(Hq, a, b, M, R, R, 5, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+    P = gtb.pack_ell(Hq)
+    assert P is not None
+    got = gtb.kpm_moments(P, a, b, M, R, R, 5, mode=gtb.MODE_PACKED, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+
+
 def test_other_vector_counts_get_a_copy_and_bad_arguments_are_refused():
     w = W.CONFIGS["c2b"].scaled(21, 17)
     inp = W.make_inputs(w)
