@@ -300,6 +300,8 @@ def run_ours(args):
                                     onsite_shift=shift)
         elif ORBITALS == "spd":      # bond form (matrix-free) or stored 9x9 blocks on the same neighbour lists
             ns = len(w.onsite)
+            if w.R in (2, 4):         # neighbour slots arranged so that the gathers of adjacent atoms share L1 wavefronts
+                H = gtb.pair_slots(H, w.R)
             Hm = gtb.spd_bonds(H, pos, spec, inp.box, inp.pbc, W.SK_ONSITE_S[:ns], W.SK_ONSITE_P[:ns],
                                W.SK_ONSITE_D[:ns], W.spd_table(ns), r0=1.42, beta=w.beta, onsite_shift=shift)
             H = Hm if REP == "bonds" else gtb.spd_blocks(Hm)

@@ -444,8 +444,9 @@ int gtb_window_ell(const gtb_ell* H, int32_t R, gtb_ell* Wd, int32_t* scratch, v
  * ASYNC.  Hp (caller-allocated cols / vals of H's shape, distinct from H's; Hp->diag is set to H->diag) receives
  * the same rows with their entries in another slot order: at R = 4 vectors per pass (a gathered neighbour is half
  * an L1 line) the slots of rows 2q and 2q + 1 are arranged so that, position by position, one column is even and
- * the other odd, and the two gathers share one L1 wavefront; at R = 2 (a quarter of a line) and width <= 4 the slots
- * of rows 4q .. 4q + 3 are permuted so that the four columns differ in their two low bits.  Padding slots stay
+ * the other odd, and the two gathers share one L1 wavefront; at R = 2 (a quarter of a line) the slots
+ * of rows 4q .. 4q + 3 are permuted so that the four columns differ in their two low bits (width <= 4: every
+ * permutation tried; up to 48: position by position).  Padding slots stay
  * (column = the row, value 0).  Any other R, or a wider matrix (48 at R = 4): a plain copy.  Hp is an ordinary gtb_ell for every call of this header; sums over
  * a row run in the new order, so results equal those on H to rounding, not bit for bit. */
 int gtb_pair_slots(const gtb_ell* H, int32_t R, gtb_ell* Hp, void* stream);

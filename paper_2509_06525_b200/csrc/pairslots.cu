@@ -127,6 +127,57 @@ __global__ void __launch_bounds__(kBlock) quad_slots_kernel(const int32_t* __res
   }
 }
 
+// R = 2, wider rows (neighbour lists of the s,p,d bond form: K = 12): position by position the four rows of a quad
+// take entries whose columns differ in their two low bits -- of the 24 ways to hand the four residues to the four
+// rows the one that most rows can serve (ties: from the fullest piles); a row that cannot serve takes what it has.
+__global__ void __launch_bounds__(kBlock) quad_greedy_kernel(const int32_t* __restrict__ cols,
+                                                             const double* __restrict__ vals, int64_t n, int32_t K,
+                                                             int32_t* __restrict__ ocols, double* __restrict__ ovals) {
+  const int64_t quads = (n + 3) / 4;
+  for (int64_t q = (int64_t)blockIdx.x * kBlock + threadIdx.x; q < quads; q += (int64_t)gridDim.x * kBlock) {
+    int32_t c[4][kPairMaxSlots];
+    unsigned long long used[4] = {0ull, 0ull, 0ull, 0ull};
+    int count[4][4];
+    const int rows = (int)min((int64_t)4, n - 4 * q);
+    for (int r = 0; r < 4; ++r)
+      for (int m = 0; m < 4; ++m) count[r][m] = 0;
+    for (int r = 0; r < rows; ++r)
+      for (int k = 0; k < K; ++k) {
+        c[r][k] = cols[(size_t)k * n + 4 * q + r];
+        ++count[r][c[r][k] & 3];
+      }
+    for (int pos = 0; pos < K; ++pos) {
+      int best_served = -1, best_pile = -1, best_rank = 0;
+      for (int rank = 0; rank < 24; ++rank) {
+        int perm[4];
+        unrank_permutation(rank, 4, perm);
+        int served = 0, pile = 0;
+        for (int r = 0; r < rows; ++r) {
+          const int have = count[r][perm[r]];
+          served += have > 0;
+          pile += have;
+        }
+        if (served > best_served || (served == best_served && pile > best_pile)) {
+          best_served = served; best_pile = pile; best_rank = rank;
+        }
+      }
+      int perm[4];
+      unrank_permutation(best_rank, 4, perm);
+      for (int r = 0; r < rows; ++r) {
+        int pick = -1;
+        for (int k = 0; k < K && pick < 0; ++k)
+          if (!((used[r] >> k) & 1ull) && (c[r][k] & 3) == perm[r]) pick = k;
+        for (int k = 0; k < K && pick < 0; ++k)
+          if (!((used[r] >> k) & 1ull)) pick = k;
+        used[r] |= 1ull << pick;
+        --count[r][c[r][pick] & 3];
+        ocols[(size_t)pos * n + 4 * q + r] = c[r][pick];
+        ovals[(size_t)pos * n + 4 * q + r] = vals[(size_t)pick * n + 4 * q + r];
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(kBlock) copy_slots_kernel(const int32_t* __restrict__ cols,
                                                             const double* __restrict__ vals, int64_t count,
                                                             int32_t* __restrict__ ocols, double* __restrict__ ovals) {
@@ -159,6 +210,10 @@ extern "C" int gtb_pair_slots(const gtb_ell* H, int32_t R, gtb_ell* Hp, void* st
     const int64_t quads = (n + 3) / 4;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((quads + kBlock - 1) / kBlock, kMaxGrid));
     quad_slots_kernel<<<grid, kBlock, 0, st>>>(H->cols, H->vals, n, H->width, Hp->cols, Hp->vals);
+  } else if (R == 2 && H->width <= kPairMaxSlots) {
+    const int64_t quads = (n + 3) / 4;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((quads + kBlock - 1) / kBlock, kMaxGrid));
+    quad_greedy_kernel<<<grid, kBlock, 0, st>>>(H->cols, H->vals, n, H->width, Hp->cols, Hp->vals);
   } else {   // nothing to gain (R = 8 gathers whole lines) or too wide for the kernel's local arrays: a copy
     const int64_t count = n * H->width;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((count + kBlock - 1) / kBlock, kMaxGrid));
