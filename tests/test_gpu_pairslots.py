@@ -106,6 +106,32 @@ def test_quads_of_rows_at_two_vectors_per_pass(key, nx, ny, diag):
     assert np.abs(got - ref).max() <= 1e-12
 
 
+def test_wide_rows_at_two_vectors_per_pass_are_arranged_position_by_position():
+    """R = 2, K > 4 (the neighbour lists of the s,p,d bond form): same rows, four distinct residues per quad and
+    position nearly everywhere, and the moments of the oracle."""
+    w = W.CONFIGS["c2b"].scaled(41, 29, R=2)
+    inp = W.make_inputs(w)
+    Ho, Hg = _both(w, inp)
+    Hq = gtb.pair_slots(Hg, 2)
+    n, K = Ho.n, Ho.width
+    assert K > 4 and n % 4 == 0
+    c0, v0 = Hg.cols.cpu().numpy(), Hg.vals.cpu().numpy()
+    c1, v1 = Hq.cols.cpu().numpy(), Hq.vals.cpu().numpy()
+    o0, o1 = np.lexsort((v0, c0), axis=0), np.lexsort((v1, c1), axis=0)
+    assert np.array_equal(np.take_along_axis(c0, o0, 0), np.take_along_axis(c1, o1, 0))
+    assert np.array_equal(np.take_along_axis(v0, o0, 0), np.take_along_axis(v1, o1, 0))
+
+    def distinct(c):
+        s = np.sort((c & 3).reshape(K, n // 4, 4), axis=2)
+        return float((np.diff(s, axis=2) != 0).all(axis=2).mean())
+    assert distinct(c1) >= 0.8 and distinct(c1) >= 4 * distinct(c0)
+    lo, hi = oracle.spectral_bounds(Ho)
+    a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
+    ref = oracle.kpm_moments(Ho, a, b, 65, 2, 5, mode=0, algo=0)
+    got = gtb.kpm_moments(Hq, a, b, 65, 2, 2, 5, check=True).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12
+
+
 def test_other_vector_counts_get_a_copy_and_bad_arguments_are_refused():
     w = W.CONFIGS["c2b"].scaled(21, 17)
     inp = W.make_inputs(w)
