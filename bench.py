@@ -569,7 +569,7 @@ def run_vac(args):
         if ORBITALS == "pz" and w.R in (2, 4, 8):   # the fused passes on the compressed form, as the DOS path
             alt = None
             if PACK and H.width <= 4 and w.R in (2, 4):
-                alt, amode, aname = gtb.pack_ell(H), gtb.MODE_PACKED, "packed rows (K7x2p)"
+                alt, amode, aname = gtb.pack_ell(gtb.pair_slots(H, w.R) if w.R == 2 else H), gtb.MODE_PACKED, "packed rows (K7x2p)"
             elif WINDOW and H.width >= 16:
                 alt, amode, aname = gtb.window_ell(H, w.R), gtb.MODE_WINDOW, "windowed tiles (K7w)"
             if alt is not None:
