@@ -13,7 +13,7 @@
 //     instead of 2 K + 1, and H costs 10 bytes per slot instead of 12.
 // The pass copies each window block with one cp.async.bulk (1 KB, from L2 after the first tile that needs it)
 // next to the tile's H part into a shared-memory stage; the consumers then gather with LDS only -- no tag
-// lookup, no miss, ~30 cycles -- in the ELL's own slot order, so the vectors equal K7's bit for bit wherever
+// lookup, no miss, ~30 cycles -- in the ELL's own slot order (R = 4: see the builder), so the vectors equal K7's bit for bit wherever
 // no padding slot is involved.
 // A tile whose columns need more than kMaxBlocks blocks makes the matrix GTB_ERR_NOT_PACKABLE: K7t stays.
 #include <algorithm>
