@@ -132,6 +132,26 @@ def test_wide_rows_at_two_vectors_per_pass_are_arranged_position_by_position():
     assert np.abs(got - ref).max() <= 1e-12
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 1023])
+@pytest.mark.parametrize("K,R", [(3, 2), (4, 2), (9, 2), (7, 4), (1, 4)])
+def test_ragged_sizes_keep_every_row(n, K, R):
+    """Row counts that are not a multiple of the group (2 or 4 rows): the last group is short; every row still
+    comes out as a permutation of itself."""
+    rng = np.random.default_rng(100 * n + 10 * K + R)
+    cols = rng.integers(0, n, size=(K, n)).astype(np.int32)
+    vals = rng.standard_normal((K, n))
+    pad = rng.random((K, n)) < 0.2
+    cols[pad] = np.broadcast_to(np.arange(n, dtype=np.int32), (K, n))[pad]
+    vals[pad] = 0.0
+    vals[cols == np.arange(n)[None, :]] = 0.0            # a slot on the diagonal is a padding slot
+    H = gtb.Ell.from_host(cols, vals)
+    Hp = gtb.pair_slots(H, R)
+    c1, v1 = Hp.cols.cpu().numpy(), Hp.vals.cpu().numpy()
+    o0, o1 = np.lexsort((vals, cols), axis=0), np.lexsort((v1, c1), axis=0)
+    assert np.array_equal(np.take_along_axis(cols, o0, 0), np.take_along_axis(c1, o1, 0))
+    assert np.array_equal(np.take_along_axis(vals, o0, 0), np.take_along_axis(v1, o1, 0))
+
+
 def test_other_vector_counts_get_a_copy_and_bad_arguments_are_refused():
     w = W.CONFIGS["c2b"].scaled(21, 17)
     inp = W.make_inputs(w)
