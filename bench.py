@@ -562,14 +562,14 @@ def run_vac(args):
             a, b = 1.01 * (hi - lo) / 2, (hi + lo) / 2
         else:
             a, b = w.a, w.b
-        if ORBITALS == "pz" and w.R == 4 and H.width <= 48 and not (WINDOW and H.width >= 16) and not (PACK and H.width <= 4):
-            H = gtb.pair_slots(H, w.R)    # plain-ELL passes at R = 4: the same matrix, slots paired for the gathers
+        if ORBITALS == "pz" and w.R in (2, 4) and H.width <= 48:
+            H = gtb.pair_slots(H, w.R)    # the same matrix with its slots arranged for the gathers of an R-vector pass
         vv = gtb.velocity_ell(H, vpos, inp.box, inp.pbc, 0)
         vopt, state["alt"] = opt, None
         if ORBITALS == "pz" and w.R in (2, 4, 8):   # the fused passes on the compressed form, as the DOS path
             alt = None
             if PACK and H.width <= 4 and w.R in (2, 4):
-                alt, amode, aname = gtb.pack_ell(gtb.pair_slots(H, w.R) if w.R == 2 else H), gtb.MODE_PACKED, "packed rows (K7x2p)"
+                alt, amode, aname = gtb.pack_ell(H), gtb.MODE_PACKED, "packed rows (K7x2p)"
             elif WINDOW and H.width >= 16:
                 alt, amode, aname = gtb.window_ell(H, w.R), gtb.MODE_WINDOW, "windowed tiles (K7w)"
             if alt is not None:
