@@ -276,7 +276,7 @@ cheb_window_kernel(const StepArgs a, const int nstages) {
   constexpr int TR = CT / T;
   constexpr int G = kBlockBytes / (R * 16);
   constexpr uint32_t kRowBytes = R * 16;
-  constexpr int CH = R == 8 ? 4 : 5;   // gathers in flight per chunk (A/B on one box: 4 / 5 / 6 / 7 -> c2 0.138 / 0.141 / 0.141 / 0.141 ms, c3 0.950 / 0.943 / 0.957 / 0.955)
+  constexpr int CH = R == 8 ? 4 : 6;   // gathers in flight per chunk (A/B on one box at c2, R = 8: 4 / 5 / 6 / 7 -> 0.138 / 0.141 / 0.141 / 0.141 ms; at c3, R = 4, after the slot re-ordering: 5 / 6 / 9 -> 0.834 / 0.822 / 0.832 ms)
   constexpr bool kDotL = kMode == 1, kAxpy = kMode == 2;
   extern __shared__ __align__(128) unsigned char smem[];
   const int64_t n = a.n;
